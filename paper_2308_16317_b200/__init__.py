@@ -1,0 +1,264 @@
+"""Thin Python binding of liblsms_tau.so (include/lsms_tau.h) -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of csrc/; PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing or a call
+returns non-zero this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblsms_tau.so")
+_lib = None
+
+EXPORTS = (
+    "lsms_version", "lsms_workspace_bytes", "lsms_solve_workspace_bytes", "lsms_host_call_scratch_bytes",
+    "lsms_tinv_from_phase_shifts", "lsms_build_M_batched", "lsms_tau00_batched",
+    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_set_blocking",
+    "lsms_last_launch_count", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe", "lsms_schur_update_batched",
+    "lsms_debug_gaunt_closed_form",
+)
+
+
+class LsmsError(RuntimeError):
+    pass
+
+
+def lib() -> ctypes.CDLL:
+    """Load liblsms_tau.so (built in-tree by paper_2308_16317_b200/build.py); fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise LsmsError(f"{LIB_PATH} is missing: run `python paper_2308_16317_b200/build.py` "
+                            "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+        L.lsms_version.restype = ctypes.c_char_p
+        L.lsms_workspace_bytes.restype = sz
+        L.lsms_workspace_bytes.argtypes = [ci, ci, ci, ci]
+        L.lsms_solve_workspace_bytes.restype = sz
+        L.lsms_solve_workspace_bytes.argtypes = [ci, ci, ci, ci]
+        L.lsms_host_call_scratch_bytes.restype = sz
+        L.lsms_host_call_scratch_bytes.argtypes = [ci, ci, ci, ci, ci]
+        L.lsms_tinv_from_phase_shifts.argtypes = [vp, vp, vp, ci, ci, ci, ci, ci, vp, vp, vp]
+        L.lsms_build_M_batched.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, vp, vp, sz, vp]
+        L.lsms_tau00_batched.argtypes = [vp, ci, ci, ci, ci, vp, vp, vp, sz, vp]
+        L.lsms_solve_central_column_batched.argtypes = [vp, ci, ci, ci, ci, vp, vp, vp, sz, vp]
+        L.lsms_tau00_from_host.argtypes = [vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, vp, vp, vp, sz, vp,
+                                           ctypes.POINTER(sz), ctypes.POINTER(sz)]
+        L.lsms_set_blocking.argtypes = [ci, ci]
+        L.lsms_fp64_peak_probe.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double), vp]
+        L.lsms_schur_update_batched.argtypes = [vp, ci, ci, ci, ci, vp]
+        L.lsms_debug_gaunt_closed_form.restype = ctypes.c_double
+        L.lsms_debug_gaunt_closed_form.argtypes = [ci, ci, ci, ci, ci]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise LsmsError(f"{what} returned {rc} "
+                        f"({'argument %d invalid' % -rc if rc < 0 else 'CUDA error code'})")
+
+
+def _stream(stream=None) -> int:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _ptr(t) -> int:
+    return 0 if t is None else int(t.data_ptr())
+
+
+def lsms_version() -> str:
+    return lib().lsms_version().decode()
+
+
+def lsms_workspace_bytes(n_sites: int, lmax: int, spin_canted: bool, batch: int) -> int:
+    return int(lib().lsms_workspace_bytes(n_sites, lmax, int(bool(spin_canted)), batch))
+
+
+def lsms_solve_workspace_bytes(n_sites: int, kmax: int, spin_canted: bool, batch: int) -> int:
+    return int(lib().lsms_solve_workspace_bytes(n_sites, kmax, int(bool(spin_canted)), batch))
+
+
+def lsms_host_call_scratch_bytes(n_sites, lmax, spin_canted, n_species, batch) -> int:
+    return int(lib().lsms_host_call_scratch_bytes(n_sites, lmax, int(bool(spin_canted)), n_species, batch))
+
+
+def lsms_set_blocking(nb_outer: int = 0, ib_inner: int = 0) -> None:
+    _check(lib().lsms_set_blocking(nb_outer, ib_inner), "lsms_set_blocking")
+
+
+def lsms_last_launch_count() -> int:
+    return int(lib().lsms_last_launch_count())
+
+
+KERNEL_CLASSES = ("K1_assemble", "K2_panel", "K3_swap_trsm", "K4_inner_gemm", "K4_schur_gemm", "K5_final_inverse")
+
+
+def lsms_profile_begin() -> None:
+    _check(lib().lsms_profile_begin(), "lsms_profile_begin")
+
+
+def lsms_profile_end() -> dict:
+    ms = (ctypes.c_double * 8)()
+    cnt = (ctypes.c_int * 8)()
+    fl = (ctypes.c_double * 8)()
+    _check(lib().lsms_profile_end(ms, cnt, fl), "lsms_profile_end")
+    return {name: {"ms": ms[i], "launches": cnt[i], "flops": fl[i]} for i, name in enumerate(KERNEL_CLASSES)}
+
+
+def lsms_debug_gaunt_closed_form(l, m, lp, mp, lpp) -> float:
+    return float(lib().lsms_debug_gaunt_closed_form(l, m, lp, mp, lpp))
+
+
+def lsms_fp64_peak_probe(which: int, iters: int = 20000, stream=None) -> float:
+    out = ctypes.c_double(0.0)
+    _check(lib().lsms_fp64_peak_probe(which, iters, ctypes.byref(out), _stream(stream)), "lsms_fp64_peak_probe")
+    return out.value
+
+
+def _workspace(nbytes: int, device):
+    import torch
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def lsms_tinv_from_phase_shifts(delta, species, z, lmax, n_sites, spin_canted, n_species, batch,
+                                tinv_diag=None, kappa=None, stream=None):
+    """delta c128 [n_species, n_spin, lmax+1], species i32 [batch, n_sites], z c128 [batch] (device tensors)
+    -> (tinv_diag c128 [batch, n_sites, n_spin, lmax+1], kappa c128 [batch])."""
+    import torch
+    nspin = 2 if spin_canted else 1
+    if tinv_diag is None:
+        tinv_diag = torch.empty((batch, n_sites, nspin, lmax + 1), dtype=torch.complex128, device=z.device)
+    if kappa is None:
+        kappa = torch.empty((batch,), dtype=torch.complex128, device=z.device)
+    _check(lib().lsms_tinv_from_phase_shifts(_ptr(delta), _ptr(species), _ptr(z), lmax, n_sites, int(bool(spin_canted)),
+                                             n_species, batch, _ptr(tinv_diag), _ptr(kappa), _stream(stream)),
+           "lsms_tinv_from_phase_shifts")
+    return tinv_diag, kappa
+
+
+def lsms_build_M_batched(tinv_diag, site_pos, moment_dir, kappa, lmax, n_sites, spin_canted, batch,
+                         M_out=None, workspace=None, stream=None):
+    """-> M_out c128 [batch, n, n]; M_out[b, c, r] is element (row r, col c) (column-major storage)."""
+    import torch
+    k = (lmax + 1) ** 2 * (2 if spin_canted else 1)
+    n = n_sites * k
+    if M_out is None:
+        M_out = torch.empty((batch, n, n), dtype=torch.complex128, device=kappa.device)
+    if workspace is None:
+        workspace = _workspace(lsms_workspace_bytes(n_sites, lmax, spin_canted, batch), kappa.device)
+    _check(lib().lsms_build_M_batched(_ptr(tinv_diag), _ptr(site_pos), _ptr(moment_dir), _ptr(kappa), lmax, n_sites,
+                                      int(bool(spin_canted)), batch, _ptr(M_out), _ptr(workspace), workspace.numel(),
+                                      _stream(stream)), "lsms_build_M_batched")
+    return M_out
+
+
+def lsms_tau00_batched(M, n_sites, kmax, spin_canted, batch, tau00_out=None, info=None, workspace=None, stream=None):
+    """M c128 [batch, n, n] column-major, OVERWRITTEN -> (tau00 c128 [batch, k, k] with tau00[b, c, r] = element
+    (row r, col c), info i32 [batch])."""
+    import torch
+    k = kmax * (2 if spin_canted else 1)
+    lmax = int(round(kmax ** 0.5)) - 1
+    if tau00_out is None:
+        tau00_out = torch.empty((batch, k, k), dtype=torch.complex128, device=M.device)
+    if info is None:
+        info = torch.empty((batch,), dtype=torch.int32, device=M.device)
+    if workspace is None:
+        workspace = _workspace(lsms_workspace_bytes(n_sites, max(lmax, 0), spin_canted, batch), M.device)
+    _check(lib().lsms_tau00_batched(_ptr(M), n_sites, kmax, int(bool(spin_canted)), batch, _ptr(tau00_out), _ptr(info),
+                                    _ptr(workspace), workspace.numel(), _stream(stream)), "lsms_tau00_batched")
+    return tau00_out, info
+
+
+def lsms_solve_central_column_batched(M, n_sites, kmax, spin_canted, batch, X_out=None, info=None, workspace=None,
+                                      stream=None):
+    """-> (X c128 [batch, k, n] with X[b, c, r] = element (row r, col c) of M^{-1} E, info)."""
+    import torch
+    k = kmax * (2 if spin_canted else 1)
+    n = n_sites * k
+    if X_out is None:
+        X_out = torch.empty((batch, k, n), dtype=torch.complex128, device=M.device)
+    if info is None:
+        info = torch.empty((batch,), dtype=torch.int32, device=M.device)
+    if workspace is None:
+        workspace = _workspace(lsms_solve_workspace_bytes(n_sites, kmax, spin_canted, batch), M.device)
+    _check(lib().lsms_solve_central_column_batched(_ptr(M), n_sites, kmax, int(bool(spin_canted)), batch, _ptr(X_out),
+                                                   _ptr(info), _ptr(workspace), workspace.numel(), _stream(stream)),
+           "lsms_solve_central_column_batched")
+    return X_out, info
+
+
+def lsms_schur_update_batched(M, n, c0, kk, batch, stream=None):
+    _check(lib().lsms_schur_update_batched(_ptr(M), n, c0, kk, batch, _stream(stream)), "lsms_schur_update_batched")
+    return M
+
+
+class HostCall:
+    """Pinned host buffers + device scratch for lsms_tau00_from_host (the end-to-end entry point)."""
+
+    def __init__(self, n_sites, lmax, spin_canted, n_species, batch, device="cuda:0"):
+        import torch
+        self.shape = (n_sites, lmax, bool(spin_canted), n_species, batch)
+        nspin = 2 if spin_canted else 1
+        k = (lmax + 1) ** 2 * nspin
+        pin = dict(pin_memory=True)
+        self.delta = torch.empty((n_species, nspin, lmax + 1), dtype=torch.complex128, **pin)
+        self.species = torch.empty((batch, n_sites), dtype=torch.int32, **pin)
+        self.z = torch.empty((batch,), dtype=torch.complex128, **pin)
+        self.site_pos = torch.empty((batch, n_sites, 3), dtype=torch.float64, **pin)
+        self.moment_dir = torch.empty((batch, n_sites, 3), dtype=torch.float64, **pin)
+        self.tau00 = torch.empty((batch, k, k), dtype=torch.complex128, **pin)
+        self.info = torch.empty((batch,), dtype=torch.int32, **pin)
+        self.scratch = _workspace(lsms_host_call_scratch_bytes(n_sites, lmax, spin_canted, n_species, batch), device)
+        self.h2d_bytes = 0
+        self.d2h_bytes = 0
+
+    def load(self, liz_batch) -> None:
+        import torch
+        self.delta.copy_(torch.from_numpy(np.ascontiguousarray(liz_batch.delta)))
+        self.species.copy_(torch.from_numpy(np.ascontiguousarray(liz_batch.species)))
+        self.z.copy_(torch.from_numpy(np.ascontiguousarray(liz_batch.z)))
+        self.site_pos.copy_(torch.from_numpy(np.ascontiguousarray(liz_batch.site_pos)))
+        self.moment_dir.copy_(torch.from_numpy(np.ascontiguousarray(liz_batch.moment_dir)))
+
+    def run(self, stream=None):
+        n_sites, lmax, canted, n_species, batch = self.shape
+        h2d, d2h = ctypes.c_size_t(0), ctypes.c_size_t(0)
+        _check(lib().lsms_tau00_from_host(_ptr(self.delta), _ptr(self.species), _ptr(self.z), _ptr(self.site_pos),
+                                          _ptr(self.moment_dir) if canted else 0, lmax, n_sites, int(canted), n_species,
+                                          batch, _ptr(self.tau00), _ptr(self.info), _ptr(self.scratch),
+                                          self.scratch.numel(), _stream(stream), ctypes.byref(h2d), ctypes.byref(d2h)),
+               "lsms_tau00_from_host")
+        self.h2d_bytes, self.d2h_bytes = int(h2d.value), int(d2h.value)
+        return self.tau00, self.info
+
+
+def device_inputs(liz_batch, device="cuda:0"):
+    """Copy a synth_liz.LizBatch to device tensors (delta, species, z, site_pos, moment_dir)."""
+    import torch
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
+    return t(liz_batch.delta), t(liz_batch.species), t(liz_batch.z), t(liz_batch.site_pos), t(liz_batch.moment_dir)
+
+
+def tau00_from_liz_batch(liz_batch, device="cuda:0", keep_M=False):
+    """Convenience: device-resident whole path for a synth_liz.LizBatch.
+    Returns (tau00 [batch,k,k] numpy indexed [b,row,col], info numpy, M copy or None)."""
+    import torch
+    cfg = liz_batch.cfg
+    B = liz_batch.batch
+    delta, species, z, pos, mom = device_inputs(liz_batch, device)
+    tinv, kappa = lsms_tinv_from_phase_shifts(delta, species, z, cfg.lmax, cfg.n_sites, cfg.spin_canted, 2, B)
+    M = lsms_build_M_batched(tinv, pos, mom if cfg.spin_canted else None, kappa, cfg.lmax, cfg.n_sites,
+                             cfg.spin_canted, B)
+    Mcopy = M.clone() if keep_M else None
+    tau, info = lsms_tau00_batched(M, cfg.n_sites, cfg.kmax, cfg.spin_canted, B)
+    torch.cuda.synchronize()
+    return tau.cpu().numpy().transpose(0, 2, 1).copy(), info.cpu().numpy(), Mcopy

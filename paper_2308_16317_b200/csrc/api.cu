@@ -1,0 +1,352 @@
+// api.cu -- the C ABI of include/lsms_tau.h: argument checks, workspace layout and the batch
+// scheduler that walks the blocked right-looking elimination.
+#include <math.h>
+#include <stdint.h>
+#include <vector>
+#include "../../include/lsms_tau.h"
+#include "common.cuh"
+#include "internal.h"
+
+namespace lsms {
+thread_local LaunchCounter g_launches = {0};
+static int g_nb_outer = 0, g_ib_inner = 0;
+
+// ---- optional per-kernel-class timing (lsms_profile_begin / lsms_profile_end): CUDA events recorded on
+// the caller's stream around each launch, so bench.py can report the Schur update's duration and share
+// measured inside the step.  Classes: 0 K1 assembly, 1 K2 panel, 2 K3 swap/trsm, 3 K4 inner (K <= IB),
+// 4 K4 Schur update (K = NB), 5 K5 final inverse.
+struct Prof {
+    bool on = false;
+    std::vector<cudaEvent_t> ev;     // pairs
+    std::vector<int> cls;
+    size_t used = 0;
+    double flops[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+static Prof g_prof;
+struct ProfScope {
+    cudaStream_t st; bool live;
+    ProfScope(int cls, cudaStream_t s, double flops = 0.0) : st(s), live(g_prof.on) {
+        if (!live) return;
+        if (g_prof.ev.size() < 2 * (g_prof.used + 1)) {
+            cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+            g_prof.ev.push_back(a); g_prof.ev.push_back(b); g_prof.cls.push_back(cls);
+        }
+        g_prof.cls[g_prof.used] = cls;
+        g_prof.flops[cls] += flops;
+        cudaEventRecord(g_prof.ev[2 * g_prof.used], st);
+    }
+    ~ProfScope() { if (live) { cudaEventRecord(g_prof.ev[2 * g_prof.used + 1], st); ++g_prof.used; } }
+};
+
+static inline size_t align256(size_t x) { return (x + 255) / 256 * 256; }
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+static int isqrt_exact(int v) { int r = (int)lround(sqrt((double)v)); return (r * r == v) ? r : -1; }
+
+// Workspace layout for lsms_tau00_batched: [pivots int32 batch*n][K5 scratch]
+static size_t tau_ws_bytes(int n, int k, int batch) {
+    return align256((size_t)batch * n * sizeof(int)) + align256(final_inverse_ws_bytes(k, batch));
+}
+
+// Blocked right-looking elimination of the first ne = n-k columns of every item, in lock-step over
+// the batch: each launch covers all items, so the latency-bound panel kernels (one CTA per item)
+// fill the chip through the batch dimension while the update kernels tile every trailing matrix.
+//   outer panel [J, J+W), W <= NB:
+//     for each inner panel [c0, c0+w), w <= IB:                       (inside the outer panel only)
+//        K2  factor the (n-c0) x w panel, pivots restricted to rows < ne
+//        K3  interchanges on the outer panel's other columns; TRSM on those to the right
+//        K4  rank-w update of the outer panel's remaining columns
+//     K3  all W interchanges on the trailing columns [J+W, n)         (before any update: rows
+//                                                                      that cross J+W must be equal)
+//     for each inner block: K3 TRSM of its w rows, K4 rank-w update of rows [c0+w, J+W)
+//     K4  Schur update A22 -= L21 U12 with inner dimension W          (>95% of the flops)
+static int eliminate(c128* M, int n, int k, int batch, int* piv, int* info, cudaStream_t st) {
+    const int ne = n - k;
+    int NB = g_nb_outer > 0 ? g_nb_outer : 64;
+    int IB = g_ib_inner > 0 ? g_ib_inner : 16;
+    const size_t stride = (size_t)n * n;
+    GemmShape g; g.base = M; g.batch_stride = stride; g.ld = n; g.batch = batch;
+    for (int J = 0; J < ne; J += NB) {
+        const int W = (ne - J < NB) ? ne - J : NB;
+        const int Jend = J + W;
+        for (int jj = 0; jj < W; jj += IB) {
+            const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
+            int rc; { ProfScope ps(1, st); rc = launch_panel(M, stride, n, c0, w, ne, batch, piv, info, st); } if (rc) return rc;
+            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, J, c0, 1, batch, piv, st); } if (rc) return rc;
+            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, c0 + w, Jend, 3, batch, piv, st); } if (rc) return rc;
+            const int rem = Jend - (c0 + w);
+            if (rem > 0) {
+                g.Mr = n - (c0 + w); g.Nc = rem; g.K = w;
+                g.offA = (size_t)(c0 + w) + (size_t)c0 * n;
+                g.offB = (size_t)c0 + (size_t)(c0 + w) * n;
+                g.offC = (size_t)(c0 + w) + (size_t)(c0 + w) * n;
+                { ProfScope ps(3, st, 8.0 * g.Mr * g.Nc * g.K * batch); rc = launch_schur_gemm(g, st); } if (rc) return rc;
+            }
+        }
+        if (Jend < n) {
+            for (int jj = 0; jj < W; jj += IB) {
+                const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
+                int rc; { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, Jend, n, 1, batch, piv, st); } if (rc) return rc;
+            }
+            for (int jj = 0; jj < W; jj += IB) {
+                const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
+                int rc; { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, Jend, n, 2, batch, piv, st); } if (rc) return rc;
+                const int rem = Jend - (c0 + w);
+                if (rem > 0) {
+                    g.Mr = rem; g.Nc = n - Jend; g.K = w;
+                    g.offA = (size_t)(c0 + w) + (size_t)c0 * n;
+                    g.offB = (size_t)c0 + (size_t)Jend * n;
+                    g.offC = (size_t)(c0 + w) + (size_t)Jend * n;
+                    { ProfScope ps(3, st, 8.0 * g.Mr * g.Nc * g.K * batch); rc = launch_schur_gemm(g, st); } if (rc) return rc;
+                }
+            }
+            g.Mr = n - Jend; g.Nc = n - Jend; g.K = W;
+            g.offA = (size_t)Jend + (size_t)J * n;
+            g.offB = (size_t)J + (size_t)Jend * n;
+            g.offC = (size_t)Jend + (size_t)Jend * n;
+            int rc; { ProfScope ps(4, st, 8.0 * g.Mr * g.Nc * g.K * batch); rc = launch_schur_gemm(g, st); } if (rc) return rc;
+        }
+    }
+    return 0;
+}
+
+}  // namespace lsms
+
+using namespace lsms;
+
+extern "C" {
+
+const char* lsms_version(void) { return "lsms_tau 0.1 (sm_100a; DMMA.8x8x4 Schur update, TMA-staged)"; }
+
+size_t lsms_workspace_bytes(int n_sites, int lmax, int spin_canted, int batch) {
+    if (n_sites < 1 || lmax < 0 || lmax > 8 || batch < 1) return 0;
+    int kmax = (lmax + 1) * (lmax + 1), k = kmax * (spin_canted ? 2 : 1);
+    size_t n = (size_t)n_sites * k;
+    size_t a = align256(gaunt_table_bytes(lmax));
+    size_t t = tau_ws_bytes((int)n, k, batch);
+    return a > t ? a : t;
+}
+
+size_t lsms_solve_workspace_bytes(int n_sites, int kmax, int spin_canted, int batch) {
+    if (n_sites < 1 || kmax < 1 || batch < 1) return 0;
+    int k = kmax * (spin_canted ? 2 : 1);
+    size_t n = (size_t)n_sites * k;
+    return align256((size_t)batch * n * n * sizeof(c128)) + align256((size_t)batch * k * k * sizeof(c128)) + tau_ws_bytes((int)n, k, batch);
+}
+
+int lsms_tinv_from_phase_shifts(const lsms_c128* delta, const int* species, const lsms_c128* z,
+                                int lmax, int n_sites, int spin_canted, int n_species, int batch,
+                                lsms_c128* tinv_diag, lsms_c128* kappa, void* cuda_stream) {
+    if (!delta || !aligned16(delta)) return -1;
+    if (!species) return -2;
+    if (!z || !aligned16(z)) return -3;
+    if (lmax < 0 || lmax > 8) return -4;
+    if (n_sites < 1) return -5;
+    if (n_species < 1) return -7;
+    if (batch < 1) return -8;
+    if (!tinv_diag || !aligned16(tinv_diag)) return -9;
+    if (!kappa || !aligned16(kappa)) return -10;
+    g_launches.n = 0;
+    return launch_tinv((const c128*)delta, species, (const c128*)z, lmax, n_sites, spin_canted ? 2 : 1, batch,
+                       (c128*)tinv_diag, (c128*)kappa, (cudaStream_t)cuda_stream);
+}
+
+int lsms_build_M_batched(const lsms_c128* tinv_diag, const double* site_pos, const double* moment_dir,
+                         const lsms_c128* kappa, int lmax, int n_sites, int spin_canted, int batch,
+                         lsms_c128* M_out, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!tinv_diag || !aligned16(tinv_diag)) return -1;
+    if (!site_pos) return -2;
+    if (spin_canted && !moment_dir) return -3;
+    if (!kappa || !aligned16(kappa)) return -4;
+    if (lmax < 0 || lmax > 8) return -5;
+    if (n_sites < 1) return -6;
+    if (batch < 1) return -8;
+    if (!M_out || !aligned16(M_out)) return -9;
+    if (!workspace || !aligned16(workspace)) return -10;
+    if (workspace_bytes < align256(gaunt_table_bytes(lmax))) return -11;
+    g_launches.n = 0;
+    ProfScope ps(0, (cudaStream_t)cuda_stream);
+    return launch_assemble((const c128*)tinv_diag, site_pos, moment_dir, (const c128*)kappa, lmax, n_sites,
+                           spin_canted ? 1 : 0, batch, (c128*)M_out, workspace, (cudaStream_t)cuda_stream);
+}
+
+int lsms_tau00_batched(lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
+                       lsms_c128* tau00_out, int* info, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!M || !aligned16(M)) return -1;
+    if (n_sites < 1) return -2;
+    if (kmax < 1 || isqrt_exact(kmax) < 0 || kmax > 81) return -3;
+    if (batch < 1) return -5;
+    if (!tau00_out || !aligned16(tau00_out)) return -6;
+    if (!info) return -7;
+    const int k = kmax * (spin_canted ? 2 : 1);
+    const long long nll = (long long)n_sites * k;
+    if (nll > 46340) return -2;
+    const int n = (int)nll;
+    if (!workspace || !aligned16(workspace)) return -8;
+    if (workspace_bytes < tau_ws_bytes(n, k, batch)) return -9;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    g_launches.n = 0;
+    int* piv = (int*)workspace;
+    void* k5ws = (char*)workspace + align256((size_t)batch * n * sizeof(int));
+    LSMS_CUDA_OK(cudaMemsetAsync(info, 0, (size_t)batch * sizeof(int), st));
+    int rc = eliminate((c128*)M, n, k, batch, piv, info, st);
+    if (rc) return rc;
+    ProfScope ps(5, st);
+    return launch_final_inverse((c128*)M, (size_t)n * n, n, k, batch, (c128*)tau00_out, info, k5ws, st);
+}
+
+int lsms_solve_central_column_batched(const lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
+                                      lsms_c128* X_out, int* info, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!M || !aligned16(M)) return -1;
+    if (n_sites < 1) return -2;
+    if (kmax < 1 || isqrt_exact(kmax) < 0 || kmax > 81) return -3;
+    if (batch < 1) return -5;
+    if (!X_out || !aligned16(X_out)) return -6;
+    if (!info) return -7;
+    if (!workspace || !aligned16(workspace)) return -8;
+    if (workspace_bytes < lsms_solve_workspace_bytes(n_sites, kmax, spin_canted, batch)) return -9;
+    const int k = kmax * (spin_canted ? 2 : 1);
+    const int n = n_sites * k;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char* p = (char*)workspace;
+    c128* copy = (c128*)p; p += align256((size_t)batch * n * n * sizeof(c128));
+    c128* tau = (c128*)p; p += align256((size_t)batch * k * k * sizeof(c128));
+    LSMS_CUDA_OK(cudaMemcpyAsync(copy, M, (size_t)batch * n * n * sizeof(c128), cudaMemcpyDeviceToDevice, st));
+    int rc = lsms_tau00_batched((lsms_c128*)copy, n_sites, kmax, spin_canted, batch, (lsms_c128*)tau, info, p,
+                                tau_ws_bytes(n, k, batch), cuda_stream);
+    if (rc) return rc;
+    return launch_backsolve_central(copy, (size_t)n * n, n, k, batch, tau, (c128*)X_out, st);
+}
+
+size_t lsms_host_call_scratch_bytes(int n_sites, int lmax, int spin_canted, int n_species, int batch) {
+    if (n_sites < 1 || lmax < 0 || lmax > 8 || batch < 1 || n_species < 1) return 0;
+    int nspin = spin_canted ? 2 : 1, nl = lmax + 1, kmax = nl * nl, k = kmax * nspin;
+    size_t n = (size_t)n_sites * k;
+    size_t s = 0;
+    s += align256((size_t)n_species * nspin * nl * sizeof(c128));          // delta
+    s += align256((size_t)batch * n_sites * sizeof(int));                 // species
+    s += align256((size_t)batch * sizeof(c128));                          // z
+    s += align256((size_t)batch * n_sites * 3 * sizeof(double)) * 2;      // site_pos, moment_dir
+    s += align256((size_t)batch * n_sites * nspin * nl * sizeof(c128));   // tinv
+    s += align256((size_t)batch * sizeof(c128));                          // kappa
+    s += align256((size_t)batch * n * n * sizeof(c128));                  // M
+    s += align256((size_t)batch * k * k * sizeof(c128));                  // tau00
+    s += align256((size_t)batch * sizeof(int));                           // info
+    s += lsms_workspace_bytes(n_sites, lmax, spin_canted, batch);
+    return s;
+}
+
+int lsms_tau00_from_host(const lsms_c128* delta_host, const int* species_host, const lsms_c128* z_host,
+                         const double* site_pos_host, const double* moment_dir_host,
+                         int lmax, int n_sites, int spin_canted, int n_species, int batch,
+                         lsms_c128* tau00_out_host, int* info_host,
+                         void* device_scratch, size_t scratch_bytes, void* cuda_stream,
+                         size_t* h2d_bytes, size_t* d2h_bytes) {
+    if (!delta_host) return -1;
+    if (!species_host) return -2;
+    if (!z_host) return -3;
+    if (!site_pos_host) return -4;
+    if (spin_canted && !moment_dir_host) return -5;
+    if (lmax < 0 || lmax > 8) return -6;
+    if (n_sites < 1) return -7;
+    if (n_species < 1) return -9;
+    if (batch < 1) return -10;
+    if (!tau00_out_host) return -11;
+    if (!info_host) return -12;
+    if (!device_scratch || !aligned16(device_scratch)) return -13;
+    if (scratch_bytes < lsms_host_call_scratch_bytes(n_sites, lmax, spin_canted, n_species, batch)) return -14;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int nspin = spin_canted ? 2 : 1, nl = lmax + 1, kmax = nl * nl, k = kmax * nspin;
+    const size_t n = (size_t)n_sites * k;
+    char* p = (char*)device_scratch;
+    auto take = [&](size_t bytes) { char* q = p; p += align256(bytes); return (void*)q; };
+    const size_t b_delta = (size_t)n_species * nspin * nl * sizeof(c128), b_spec = (size_t)batch * n_sites * sizeof(int),
+                 b_z = (size_t)batch * sizeof(c128), b_pos = (size_t)batch * n_sites * 3 * sizeof(double),
+                 b_tau = (size_t)batch * k * k * sizeof(c128), b_info = (size_t)batch * sizeof(int);
+    c128* d_delta = (c128*)take(b_delta); int* d_spec = (int*)take(b_spec); c128* d_z = (c128*)take(b_z);
+    double* d_pos = (double*)take(b_pos); double* d_mom = (double*)take(b_pos);
+    c128* d_tinv = (c128*)take((size_t)batch * n_sites * nspin * nl * sizeof(c128)); c128* d_kappa = (c128*)take(b_z);
+    c128* d_M = (c128*)take((size_t)batch * n * n * sizeof(c128));
+    c128* d_tau = (c128*)take(b_tau); int* d_info = (int*)take(b_info);
+    void* ws = p; const size_t ws_bytes = lsms_workspace_bytes(n_sites, lmax, spin_canted, batch);
+    size_t h2d = 0;
+    LSMS_CUDA_OK(cudaMemcpyAsync(d_delta, delta_host, b_delta, cudaMemcpyHostToDevice, st)); h2d += b_delta;
+    LSMS_CUDA_OK(cudaMemcpyAsync(d_spec, species_host, b_spec, cudaMemcpyHostToDevice, st)); h2d += b_spec;
+    LSMS_CUDA_OK(cudaMemcpyAsync(d_z, z_host, b_z, cudaMemcpyHostToDevice, st)); h2d += b_z;
+    LSMS_CUDA_OK(cudaMemcpyAsync(d_pos, site_pos_host, b_pos, cudaMemcpyHostToDevice, st)); h2d += b_pos;
+    if (spin_canted) { LSMS_CUDA_OK(cudaMemcpyAsync(d_mom, moment_dir_host, b_pos, cudaMemcpyHostToDevice, st)); h2d += b_pos; }
+    int rc = lsms_tinv_from_phase_shifts((lsms_c128*)d_delta, d_spec, (lsms_c128*)d_z, lmax, n_sites, spin_canted, n_species, batch,
+                                         (lsms_c128*)d_tinv, (lsms_c128*)d_kappa, cuda_stream);
+    if (rc) return rc;
+    int launches = g_launches.n;
+    rc = lsms_build_M_batched((lsms_c128*)d_tinv, d_pos, spin_canted ? d_mom : nullptr, (lsms_c128*)d_kappa, lmax, n_sites, spin_canted,
+                              batch, (lsms_c128*)d_M, ws, ws_bytes, cuda_stream);
+    if (rc) return rc;
+    launches += g_launches.n;
+    rc = lsms_tau00_batched((lsms_c128*)d_M, n_sites, kmax, spin_canted, batch, (lsms_c128*)d_tau, d_info, ws, ws_bytes, cuda_stream);
+    if (rc) return rc;
+    launches += g_launches.n;
+    g_launches.n = launches;
+    LSMS_CUDA_OK(cudaMemcpyAsync(tau00_out_host, d_tau, b_tau, cudaMemcpyDeviceToHost, st));
+    LSMS_CUDA_OK(cudaMemcpyAsync(info_host, d_info, b_info, cudaMemcpyDeviceToHost, st));
+    LSMS_CUDA_OK(cudaStreamSynchronize(st));
+    if (h2d_bytes) *h2d_bytes = h2d;
+    if (d2h_bytes) *d2h_bytes = b_tau + b_info;
+    return 0;
+}
+
+int lsms_set_blocking(int nb_outer, int ib_inner) {
+    if (nb_outer < 0 || nb_outer > 256 || (nb_outer % 4) != 0) return -1;
+    if (ib_inner < 0 || ib_inner > 16) return -2;
+    g_nb_outer = nb_outer; g_ib_inner = ib_inner;
+    return 0;
+}
+
+int lsms_last_launch_count(void) { return g_launches.n; }
+
+int lsms_profile_begin(void) {
+    g_prof.on = true; g_prof.used = 0;
+    for (int i = 0; i < 8; ++i) g_prof.flops[i] = 0.0;
+    return 0;
+}
+
+int lsms_profile_end(double* ms_by_class_host, int* launches_by_class_host, double* flops_by_class_host) {
+    if (!ms_by_class_host) return -1;
+    if (!launches_by_class_host) return -2;
+    if (!flops_by_class_host) return -3;
+    g_prof.on = false;
+    for (int i = 0; i < 8; ++i) { ms_by_class_host[i] = 0.0; launches_by_class_host[i] = 0; flops_by_class_host[i] = g_prof.flops[i]; }
+    for (size_t i = 0; i < g_prof.used; ++i) {
+        LSMS_CUDA_OK(cudaEventSynchronize(g_prof.ev[2 * i + 1]));
+        float ms = 0.f;
+        LSMS_CUDA_OK(cudaEventElapsedTime(&ms, g_prof.ev[2 * i], g_prof.ev[2 * i + 1]));
+        ms_by_class_host[g_prof.cls[i]] += ms; launches_by_class_host[g_prof.cls[i]] += 1;
+    }
+    g_prof.used = 0;
+    return 0;
+}
+
+int lsms_fp64_peak_probe(int which, int iters, double* tflops_host, void* cuda_stream) {
+    if (which < 0 || which > 1) return -1;
+    if (iters < 1) return -2;
+    if (!tflops_host) return -3;
+    return run_peak_probe(which, iters, tflops_host, (cudaStream_t)cuda_stream);
+}
+
+int lsms_schur_update_batched(lsms_c128* M, int n, int c0, int kk, int batch, void* cuda_stream) {
+    if (!M || !aligned16(M)) return -1;
+    if (n < 2) return -2;
+    if (c0 < 0 || kk < 1 || c0 + kk >= n) return -3;
+    if (batch < 1) return -5;
+    GemmShape g; g.base = (c128*)M; g.batch_stride = (size_t)n * n; g.ld = n; g.batch = batch;
+    const int r0 = c0 + kk;
+    g.Mr = n - r0; g.Nc = n - r0; g.K = kk;
+    g.offA = (size_t)r0 + (size_t)c0 * n; g.offB = (size_t)c0 + (size_t)r0 * n; g.offC = (size_t)r0 + (size_t)r0 * n;
+    g_launches.n = 0;
+    return launch_schur_gemm(g, (cudaStream_t)cuda_stream);
+}
+
+/* host-only debug export for the CPU test-suite: the closed-form Gaunt number used by K1 */
+double lsms_debug_gaunt_closed_form(int l, int m, int lp, int mp, int lpp) { return gaunt_closed_form_host(l, m, lp, mp, lpp); }
+
+}  // extern "C"

@@ -1,0 +1,264 @@
+// assemble.cu -- K1: device-side assembly of the KKR matrices M = t^{-1} - g0,
+// "Further code acceleration is expected if the KKR matrix is constructed on GPUs".
+//
+//   g0_{LL'}(R) = -4 pi i kappa sum_{l''} i^{l-l'+l''} h_{l''}(kappa R) Y_{l'',m'-m}(R^) C(L,L',L'')
+//   (DESIGN.md "Readings" A1-A4).
+//
+// Gaunt numbers come from the closed form (two Wigner 3j symbols, Racah's sum) -- a different
+// route from the oracle's quadrature.  HBM-write-bound: 16 n^2 bytes per item.
+#include "common.cuh"
+#include "internal.h"
+
+namespace lsms {
+
+// ---------------------------------------------------------------- Gaunt numbers, closed form
+
+__host__ __device__ inline double fact(int n) { double f = 1.0; for (int i = 2; i <= n; ++i) f *= (double)i; return f; }
+
+// Wigner 3j symbol (j1 j2 j3; m1 m2 m3), integer arguments, Racah's formula.
+__host__ __device__ double wigner3j(int j1, int j2, int j3, int m1, int m2, int m3) {
+    if (m1 + m2 + m3 != 0) return 0.0;
+    if (j3 < abs(j1 - j2) || j3 > j1 + j2) return 0.0;
+    if (abs(m1) > j1 || abs(m2) > j2 || abs(m3) > j3) return 0.0;
+    double delta = fact(j1 + j2 - j3) * fact(j1 - j2 + j3) * fact(-j1 + j2 + j3) / fact(j1 + j2 + j3 + 1);
+    double pre = sqrt(delta * fact(j1 + m1) * fact(j1 - m1) * fact(j2 + m2) * fact(j2 - m2) * fact(j3 + m3) * fact(j3 - m3));
+    int tmin = 0;
+    if (j2 - j3 - m1 > tmin) tmin = j2 - j3 - m1;
+    if (j1 - j3 + m2 > tmin) tmin = j1 - j3 + m2;
+    int tmax = j1 + j2 - j3;
+    if (j1 - m1 < tmax) tmax = j1 - m1;
+    if (j2 + m2 < tmax) tmax = j2 + m2;
+    double s = 0.0;
+    for (int t = tmin; t <= tmax; ++t) {
+        double d = fact(t) * fact(j3 - j2 + t + m1) * fact(j3 - j1 + t - m2) * fact(j1 + j2 - j3 - t) * fact(j1 - t - m1) * fact(j2 - t + m2);
+        s += ((t & 1) ? -1.0 : 1.0) / d;
+    }
+    int ph = j1 - j2 - m3;
+    return ((ph & 1) ? -1.0 : 1.0) * pre * s;
+}
+
+// C(L,L',L'') = Int Y_L^* Y_L' Y_L''^* dOmega, m'' = m' - m.
+__host__ __device__ double gaunt_closed_form(int l, int m, int lp, int mp, int lpp) {
+    int mpp = mp - m;
+    if (abs(mpp) > lpp || ((l + lp + lpp) & 1)) return 0.0;
+    const double FOUR_PI = 12.566370614359172953850573533118;
+    double pref = sqrt((2.0 * l + 1.0) * (2.0 * lp + 1.0) * (2.0 * lpp + 1.0) / FOUR_PI);
+    double v = pref * wigner3j(l, lp, lpp, 0, 0, 0) * wigner3j(l, lp, lpp, -m, mp, -mpp);
+    return ((m + mpp) & 1) ? -v : v;
+}
+
+double gaunt_closed_form_host(int l, int m, int lp, int mp, int lpp) { return gaunt_closed_form(l, m, lp, mp, lpp); }
+
+__host__ __device__ inline void l_m_of(int L, int& l, int& m) { l = 0; while ((l + 1) * (l + 1) <= L) ++l; m = L - l * (l + 1); }
+
+// Table entry t (0..lmax) of the pair (L,L'), stored at [(t*kmax + L')*kmax + L]:
+//   coef = -4 pi i * i^{l-l'+l''} * C(L,L',L''),  idx = L'' = l''(l''+1) + m' - m,  l'' = |l-l'| + 2t.
+__global__ void k_gaunt_table(int lmax, c128* __restrict__ coef, int* __restrict__ idx) {
+    int kmax = (lmax + 1) * (lmax + 1), nt = lmax + 1;
+    int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= kmax * kmax * nt) return;
+    int L = e % kmax, Lp = (e / kmax) % kmax, t = e / (kmax * kmax);
+    int l, m, lp, mp; l_m_of(L, l, m); l_m_of(Lp, lp, mp);
+    int lpp = abs(l - lp) + 2 * t, mpp = mp - m;
+    c128 c = cmake(0.0, 0.0); int id = 0;
+    if (lpp <= l + lp && abs(mpp) <= lpp) {
+        double g = gaunt_closed_form(l, m, lp, mp, lpp);
+        const double FOUR_PI = 12.566370614359172953850573533118;
+        // -4 pi i * i^p,  p = l - l' + l'' >= 0:  i^(p+1) * (-4 pi)
+        int p = (l - lp + lpp + 1) & 3;
+        double v = -FOUR_PI * g;
+        c = (p == 0) ? cmake(v, 0.0) : (p == 1) ? cmake(0.0, v) : (p == 2) ? cmake(-v, 0.0) : cmake(0.0, -v);
+        id = lpp * (lpp + 1) + mpp;
+    }
+    coef[e] = c; idx[e] = id;
+}
+
+// ---------------------------------------------------------------- t^{-1} from phase shifts
+
+__device__ inline c128 csqrt_upper(c128 z) {       // principal root with Im >= 0 for Im z >= 0
+    double r = hypot(z.x, z.y);
+    c128 k;
+    if (r == 0.0) return cmake(0.0, 0.0);
+    if (z.x >= 0.0) { double t = sqrt(0.5 * (r + z.x)); k = cmake(t, z.y / (2.0 * t)); }
+    else { double t = sqrt(0.5 * (r - z.x)); k = cmake(fabs(z.y) / (2.0 * t), copysign(t, z.y)); }
+    if (k.y < 0.0) k = cneg(k);
+    return k;
+}
+
+__global__ void k_tinv(const c128* __restrict__ delta, const int* __restrict__ species, const c128* __restrict__ z,
+                       int lmax, int n_sites, int nspin, int batch, c128* __restrict__ tinv, c128* __restrict__ kappa) {
+    int nl = lmax + 1;
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long total = (long long)batch * n_sites * nspin * nl;
+    if (e < batch) kappa[e] = csqrt_upper(z[e]);
+    if (e >= total) return;
+    int l = (int)(e % nl); long long r = e / nl;
+    int s = (int)(r % nspin); r /= nspin;
+    int site = (int)(r % n_sites); int b = (int)(r / n_sites);
+    c128 kap = csqrt_upper(z[b]);
+    c128 d = delta[((size_t)species[(size_t)b * n_sites + site] * nspin + s) * nl + l];
+    // sin(a+ib) = sin a cosh b + i cos a sinh b ;  e^{i(a+ib)} = e^{-b}(cos a + i sin a)
+    double sa, ca; sincos(d.x, &sa, &ca);
+    double eb = exp(-d.y);
+    c128 sn = cmake(sa * cosh(d.y), ca * sinh(d.y));
+    c128 ex = cmake(eb * ca, eb * sa);
+    tinv[e] = cneg(cdiv(kap, cmul(sn, ex)));       // -kappa / (sin d e^{i d})
+}
+
+// ---------------------------------------------------------------- K1: block assembly
+
+constexpr int ASM_WARPS = 8;
+
+__global__ void __launch_bounds__(ASM_WARPS * 32)
+k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, const double* __restrict__ moment,
+           const c128* __restrict__ kappa, const c128* __restrict__ coef, const int* __restrict__ idx,
+           int lmax, int n_sites, int canted, c128* __restrict__ Mout) {
+    extern __shared__ c128 smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int kmax = (lmax + 1) * (lmax + 1), nt = lmax + 1, l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
+    const int nspin = canted ? 2 : 1, k = kmax * nspin;
+    const size_t n = (size_t)n_sites * k;
+    const int b = blockIdx.z, sj = blockIdx.x, si = blockIdx.y * ASM_WARPS + warp;
+    if (si >= n_sites) return;
+    c128* hY = smem + (size_t)warp * (nl2 + l2 + 1);
+    c128* hs = hY + nl2;
+    c128* M = Mout + (size_t)b * n * n;
+    const size_t r0 = (size_t)(si == 0 ? n_sites - 1 : si - 1) * k, c0 = (size_t)(sj == 0 ? n_sites - 1 : sj - 1) * k;
+    const c128 zero = cmake(0.0, 0.0);
+
+    if (si == sj) {
+        // site-diagonal block: t^{-1} (g0^{ii} = 0, "between two different atom sites")
+        const c128* ti = tinv + ((size_t)b * n_sites + si) * nspin * nt;
+        double ex = 0, ey = 0, ez = 0;
+        if (canted) { const double* mv = moment + ((size_t)b * n_sites + si) * 3; ex = mv[0]; ey = mv[1]; ez = mv[2]; }
+        for (int e = lane; e < k * k; e += 32) {
+            int r = e % k, c = e / k;
+            int Lr = r % kmax, Lc = c % kmax, sr = r / kmax, sc = c / kmax;
+            c128 v = zero;
+            if (Lr == Lc) {
+                int l = 0; while ((l + 1) * (l + 1) <= Lr) ++l;
+                if (!canted) v = ti[l];
+                else {
+                    c128 a = ti[l], bb = ti[nt + l];
+                    c128 hsum = cscale(0.5, cadd(a, bb)), hdif = cscale(0.5, csub(a, bb));
+                    if (sr == 0 && sc == 0) v = cadd(hsum, cscale(ez, hdif));
+                    else if (sr == 1 && sc == 1) v = csub(hsum, cscale(ez, hdif));
+                    else if (sr == 0) v = cmul(hdif, cmake(ex, -ey));       // (up,down): e_x - i e_y
+                    else v = cmul(hdif, cmake(ex, ey));                      // (down,up): e_x + i e_y
+                }
+            }
+            M[(r0 + r) + n * (c0 + c)] = v;
+        }
+        return;
+    }
+
+    // ---- per-R tables (a1): h_l(kappa R) for l <= 2 lmax, Y_lm(R^) for (2 lmax+1)^2 entries
+    const double* pi = site_pos + ((size_t)b * n_sites + si) * 3;
+    const double* pj = site_pos + ((size_t)b * n_sites + sj) * 3;
+    const double Rx = pi[0] - pj[0], Ry = pi[1] - pj[1], Rz = pi[2] - pj[2];
+    const double R = sqrt(Rx * Rx + Ry * Ry + Rz * Rz);
+    const c128 kap = kappa[b];
+    if (lane == 0) {
+        c128 x = cscale(R, kap);
+        double s, c; sincos(x.x, &s, &c);
+        double ed = exp(-x.y);
+        c128 eix = cmake(ed * c, ed * s);
+        c128 xinv = crecip(x);
+        c128 h0 = cmul(cmake(0.0, -1.0), cmul(eix, xinv));                       // -i e^{ix}/x
+        c128 h1 = cneg(cmul(cadd(cmake(1.0, 0.0), cmul(cmake(0.0, 1.0), xinv)), cmul(eix, xinv)));   // -(1+i/x) e^{ix}/x
+        hs[0] = h0; if (l2 >= 1) hs[1] = h1;
+        for (int l = 1; l < l2; ++l) {
+            c128 hn = csub(cscale((double)(2 * l + 1), cmul(xinv, h1)), h0);
+            hs[l + 1] = hn; h0 = h1; h1 = hn;
+        }
+    }
+    __syncwarp();
+    if (lane <= l2) {
+        // column m = lane of the normalised Legendre triangle; Y_lm = Pbar_lm e^{i m phi}
+        const int m = lane;
+        const double ct = Rz / R;
+        const double rho = sqrt(Rx * Rx + Ry * Ry);
+        const double st = rho / R;
+        double cphi = 1.0, sphi = 0.0;
+        if (rho > 0.0) { cphi = Rx / rho; sphi = Ry / rho; }
+        double pmm = 0.28209479177387814347403972578039;      // 1/sqrt(4 pi)
+        double er = 1.0, ei = 0.0;                             // e^{i m phi}
+        for (int i = 1; i <= m; ++i) {
+            pmm = -sqrt((2.0 * i + 1.0) / (2.0 * i)) * st * pmm;
+            double t = er * cphi - ei * sphi; ei = er * sphi + ei * cphi; er = t;
+        }
+        double p2 = 0.0, p1 = pmm;
+        for (int l = m; l <= l2; ++l) {
+            double p;
+            if (l == m) p = pmm;
+            else {
+                double a = sqrt((4.0 * l * l - 1.0) / ((double)l * l - (double)m * m));
+                double bq = sqrt((((double)l - 1.0) * (l - 1.0) - (double)m * m) / (4.0 * (l - 1.0) * (l - 1.0) - 1.0));
+                p = a * (ct * p1 - bq * p2);
+                p2 = p1; p1 = p;
+            }
+            c128 y = cmake(p * er, p * ei);
+            c128 h = hs[l];
+            hY[l * (l + 1) + m] = cmul(h, y);
+            if (m > 0) { c128 ym = (m & 1) ? cmake(-y.x, y.y) : cmake(y.x, -y.y); hY[l * (l + 1) - m] = cmul(h, ym); }   // (-1)^m conj
+        }
+    }
+    __syncwarp();
+
+    // ---- block elements (a2): M_ij = -g0 = -kappa * sum_t coef_t * hY[idx_t]
+    const int kk2 = kmax * kmax;
+    for (int e = lane; e < kk2; e += 32) {
+        c128 s = zero;
+        for (int t = 0; t < nt; ++t) cfma(s, coef[t * kk2 + e], hY[idx[t * kk2 + e]]);
+        c128 g = cneg(cmul(kap, s));
+        int L = e % kmax, Lp = e / kmax;
+        M[(r0 + L) + n * (c0 + Lp)] = g;
+        if (canted) {
+            M[(r0 + kmax + L) + n * (c0 + kmax + Lp)] = g;
+            M[(r0 + kmax + L) + n * (c0 + Lp)] = zero;
+            M[(r0 + L) + n * (c0 + kmax + Lp)] = zero;
+        }
+    }
+}
+
+// ---------------------------------------------------------------- host launchers
+
+size_t gaunt_table_bytes(int lmax) {
+    size_t kmax = (size_t)(lmax + 1) * (lmax + 1), nt = lmax + 1;
+    size_t e = kmax * kmax * nt;
+    return ((e * sizeof(c128) + 255) / 256) * 256 + ((e * sizeof(int) + 255) / 256) * 256;
+}
+
+int launch_tinv(const c128* delta, const int* species, const c128* z, int lmax, int n_sites, int nspin, int batch,
+                c128* tinv, c128* kappa, cudaStream_t st) {
+    long long total = (long long)batch * n_sites * nspin * (lmax + 1);
+    if (total < batch) total = batch;
+    int thr = 256; long long blocks = (total + thr - 1) / thr;
+    k_tinv<<<(unsigned)blocks, thr, 0, st>>>(delta, species, z, lmax, n_sites, nspin, batch, tinv, kappa);
+    LSMS_LAUNCH_CHECK();
+    return 0;
+}
+
+int launch_assemble(const c128* tinv, const double* site_pos, const double* moment, const c128* kappa, int lmax,
+                    int n_sites, int canted, int batch, c128* M, void* ws, cudaStream_t st) {
+    size_t kmax = (size_t)(lmax + 1) * (lmax + 1), nt = lmax + 1, e = kmax * kmax * nt;
+    c128* coef = (c128*)ws;
+    int* idx = (int*)((char*)ws + ((e * sizeof(c128) + 255) / 256) * 256);
+    k_gaunt_table<<<(unsigned)((e + 127) / 128), 128, 0, st>>>(lmax, coef, idx);
+    LSMS_LAUNCH_CHECK();
+    int l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
+    size_t smem = (size_t)ASM_WARPS * (nl2 + l2 + 1) * sizeof(c128);
+    for (int b0 = 0; b0 < batch; b0 += 65535) {
+        int nb = batch - b0 < 65535 ? batch - b0 : 65535;
+        dim3 grid(n_sites, (n_sites + ASM_WARPS - 1) / ASM_WARPS, nb);
+        size_t k = kmax * (canted ? 2 : 1), n = (size_t)n_sites * k;
+        k_assemble<<<grid, ASM_WARPS * 32, smem, st>>>(tinv + (size_t)b0 * n_sites * (canted ? 2 : 1) * nt,
+                                                       site_pos + (size_t)b0 * n_sites * 3,
+                                                       moment ? moment + (size_t)b0 * n_sites * 3 : nullptr, kappa + b0, coef, idx,
+                                                       lmax, n_sites, canted, M + (size_t)b0 * n * n);
+        LSMS_LAUNCH_CHECK();
+    }
+    return 0;
+}
+
+}  // namespace lsms

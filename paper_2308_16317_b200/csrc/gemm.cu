@@ -1,0 +1,175 @@
+// gemm.cu -- K4: the trailing Schur-complement update A22 <- A22 - L21 * U12,
+// the contraction in which "more than 90% of the computing time" goes.
+//
+// complex128 GEMM on the FP64 tensor path: PTX mma.sync.m8n8k4.f64 -> SASS DMMA.8x8x4 (tcgen05 has
+// no f64 kind, so the warp-level DMMA is the FP64 tensor instruction on sm_100a).  One complex MAC =
+// 4 real MMAs:  Cr += Ar*(-Br) + Ai*Bi ;  Ci += Ar*(-Bi) + Ai*(-Br)   (so that C -= A*B).
+// Operand tiles are staged into shared memory by the TMA engine (cp.async.bulk, one bulk copy per
+// tile column, completion on an mbarrier) in a 3-stage ring.
+// A and B are read where the LU left them (column-major, interleaved complex), C lives in the
+// accumulators: it is loaded once, updated over the whole inner dimension, stored once.
+#include "common.cuh"
+#include "internal.h"
+
+namespace lsms {
+
+constexpr int BM = 64, BN = 64, KS = 16, STAGES = 3;
+constexpr int LDA_S = BM + 2;      // complex units; == 2 (mod 8): conflict-free LDS.128 of A fragments
+constexpr int LDB_S = KS + 4;      // complex units; == 4 (mod 8): conflict-free LDS.128 of B fragments
+constexpr int A_STAGE = KS * LDA_S;        // complex elements
+constexpr int B_STAGE = BN * LDB_S;
+constexpr int STAGE_ELEMS = A_STAGE + B_STAGE;
+constexpr int GEMM_THREADS = 256;
+constexpr size_t GEMM_SMEM = (size_t)STAGES * STAGE_ELEMS * sizeof(c128) + STAGES * sizeof(uint64_t);
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void tma_bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// Fill ring slot s with K-chunk kc of the A and B tiles: one bulk copy per tile column, issued by
+// threads 0..KS+BN-1; thread 0 also posts the expected byte count on the slot's mbarrier.
+__device__ __forceinline__ void issue_chunk(const GemmShape& g, const c128* A, const c128* B, c128* ring, uint64_t* full,
+                                            int kc, int mvalid, int nvalid) {
+    const int s = kc % STAGES, t = threadIdx.x;
+    const int k0 = kc * KS, kvalid = min(KS, g.K - k0);
+    c128* As = ring + (size_t)s * STAGE_ELEMS;
+    c128* Bs = As + A_STAGE;
+    if (t == 0) mbar_expect_tx(&full[s], (uint32_t)((kvalid * mvalid + nvalid * kvalid) * sizeof(c128)));
+    if (t < KS) {
+        if (t < kvalid)      // column k0+t of A: mvalid contiguous elements
+            tma_bulk_g2s(As + t * LDA_S, A + (size_t)(k0 + t) * g.ld, (uint32_t)(mvalid * sizeof(c128)), &full[s]);
+    } else if (t < KS + BN) {
+        const int nn = t - KS;
+        if (nn < nvalid)     // column n0+nn of B: kvalid contiguous elements
+            tma_bulk_g2s(Bs + nn * LDB_S, B + (size_t)nn * g.ld + k0, (uint32_t)(kvalid * sizeof(c128)), &full[s]);
+    }
+}
+
+__global__ void __launch_bounds__(GEMM_THREADS, 2)
+k_schur_gemm(GemmShape g, int tiles_m) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    c128* ring = reinterpret_cast<c128*>(smem_raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)STAGES * STAGE_ELEMS * sizeof(c128));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tm = blockIdx.x % tiles_m, tn = blockIdx.x / tiles_m;
+    const int m0 = tm * BM, n0 = tn * BN;
+    const int mvalid = min(BM, g.Mr - m0), nvalid = min(BN, g.Nc - n0);
+    c128* item = g.base + (size_t)blockIdx.y * g.batch_stride;
+    const c128* A = item + g.offA + m0;                       // A(m0, 0)
+    const c128* B = item + g.offB + (size_t)n0 * g.ld;        // B(0, n0)
+    c128* C = item + g.offC + m0 + (size_t)n0 * g.ld;         // C(m0, n0)
+    const int nchunks = (g.K + KS - 1) / KS;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    for (int kc = 0; kc < STAGES && kc < nchunks; ++kc) issue_chunk(g, A, B, ring, full, kc, mvalid, nvalid);
+
+    // C tile -> accumulators (issued before the first wait so that it overlaps the TMA fill)
+    const int gq = lane >> 2, q = lane & 3;              // fragment coordinates: A[gq][q], B[q][gq], C[gq][2q..2q+1]
+    const int wm = (warp & 1) * 32, wn = (warp >> 1) * 16;
+    double cr[4][2][2], ci[4][2][2];
+#pragma unroll
+    for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int r = wm + mt * 8 + gq, c = wn + nt * 8 + 2 * q + e;
+                c128 v = cmake(0.0, 0.0);
+                if (r < mvalid && c < nvalid) v = C[r + (size_t)c * g.ld];
+                cr[mt][nt][e] = v.x; ci[mt][nt][e] = v.y;
+            }
+
+    for (int kc = 0; kc < nchunks; ++kc) {
+        const int s = kc % STAGES;
+        mbar_wait(&full[s], (kc / STAGES) & 1);
+        const int kvalid = min(KS, g.K - kc * KS);
+        const c128* As = ring + (size_t)s * STAGE_ELEMS;
+        const c128* Bs = As + A_STAGE;
+        const int nsteps = (kvalid + 3) >> 2;
+#pragma unroll 1
+        for (int ks = 0; ks < nsteps; ++ks) {
+            const int k0 = ks * 4;
+            const bool live = (k0 + q) < kvalid;
+            c128 a[4], b[2];
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) { a[mt] = As[(k0 + q) * LDA_S + wm + mt * 8 + gq]; if (!live) a[mt] = cmake(0.0, 0.0); }
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) { b[nt] = Bs[(wn + nt * 8 + gq) * LDB_S + k0 + q]; if (!live) b[nt] = cmake(0.0, 0.0); }
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) {
+                const double nbr = -b[nt].x, nbi = -b[nt].y, bi = b[nt].y;
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    dmma884(cr[mt][nt][0], cr[mt][nt][1], a[mt].x, nbr);
+                    dmma884(ci[mt][nt][0], ci[mt][nt][1], a[mt].x, nbi);
+                    dmma884(cr[mt][nt][0], cr[mt][nt][1], a[mt].y, bi);
+                    dmma884(ci[mt][nt][0], ci[mt][nt][1], a[mt].y, nbr);
+                }
+            }
+        }
+        if (kc + STAGES < nchunks) {          // refill this slot once every warp is done with it
+            __syncthreads();
+            issue_chunk(g, A, B, ring, full, kc + STAGES, mvalid, nvalid);
+        }
+    }
+
+#pragma unroll
+    for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int r = wm + mt * 8 + gq, c = wn + nt * 8 + 2 * q + e;
+                if (r < mvalid && c < nvalid) C[r + (size_t)c * g.ld] = cmake(cr[mt][nt][e], ci[mt][nt][e]);
+            }
+}
+
+int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
+    if (g.Mr <= 0 || g.Nc <= 0 || g.K <= 0 || g.batch <= 0) return 0;
+    static bool attr_set = false;
+    if (!attr_set) {
+        LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEMM_SMEM));
+        attr_set = true;
+    }
+    const int tiles_m = (g.Mr + BM - 1) / BM, tiles_n = (g.Nc + BN - 1) / BN;
+    for (int b0 = 0; b0 < g.batch; b0 += 65535) {
+        GemmShape h = g;
+        h.base = g.base + (size_t)b0 * g.batch_stride;
+        h.batch = g.batch - b0 < 65535 ? g.batch - b0 : 65535;
+        dim3 grid((unsigned)(tiles_m * tiles_n), (unsigned)h.batch);
+        k_schur_gemm<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(h, tiles_m);
+        LSMS_LAUNCH_CHECK();
+    }
+    return 0;
+}
+
+}  // namespace lsms

@@ -1,0 +1,300 @@
+// lu.cu -- K2 (panel LU with restricted partial pivoting), K3 (row interchanges + unit-lower
+// triangular solve), K5 (inverse of the final k x k Schur complement) and the verification-only
+// back-substitution.  SURVEY.md 8(a) a3, a4, a6; "LU factorization of the matrix" PAPER.md:92;
+// "only the first block of the inverted matrix is needed" PAPER.md:62.
+//
+// Pivot rule (reading A14): for the first ne = n-k columns the pivot search covers rows
+// [j, ne) only, so the central-site rows are updated but never selected; the trailing k x k block
+// is then exactly the Schur complement D - C A^{-1} B of the central site.
+#include "common.cuh"
+#include "internal.h"
+
+namespace lsms {
+
+constexpr int PANEL_THREADS = 1024;
+constexpr int MAX_IB = 16;
+
+// ---------------------------------------------------------------- K2: panel factorisation
+// One CTA per matrix.  Columns [c0, c0+w) of rows [c0, n); w <= MAX_IB.  Unblocked right-looking
+// elimination inside the panel; the max search of column j+1 is fused into the update of step j.
+__global__ void __launch_bounds__(PANEL_THREADS)
+k_panel(c128* __restrict__ base, size_t stride, int n, int c0, int w, int ne, int* __restrict__ piv, int* __restrict__ info) {
+    c128* A = base + (size_t)blockIdx.x * stride;
+    int* pv = piv + (size_t)blockIdx.x * n;
+    __shared__ c128 urow[MAX_IB];
+    __shared__ double red_v[PANEL_THREADS / 32];
+    __shared__ int red_i[PANEL_THREADS / 32];
+    __shared__ int s_piv;
+    __shared__ int s_bad;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    // candidate of this thread for the current column: (value, row); rows j..ne-1
+    double bv = -1.0; int bi = 0x7fffffff;
+    for (int i = c0 + tid; i < ne; i += PANEL_THREADS) {
+        double v = cabs1(A[i + (size_t)c0 * n]);
+        if (v > bv) { bv = v; bi = i; }
+    }
+    for (int jj = 0; jj < w; ++jj) {
+        const int j = c0 + jj;
+        // ---- block arg-max (ties -> smallest row)
+        double v = bv; int ix = bi;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            double ov = __shfl_xor_sync(0xffffffffu, v, o); int oi = __shfl_xor_sync(0xffffffffu, ix, o);
+            if (ov > v || (ov == v && oi < ix)) { v = ov; ix = oi; }
+        }
+        if (lane == 0) { red_v[warp] = v; red_i[warp] = ix; }
+        __syncthreads();
+        if (warp == 0) {
+            v = red_v[lane]; ix = red_i[lane];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                double ov = __shfl_xor_sync(0xffffffffu, v, o); int oi = __shfl_xor_sync(0xffffffffu, ix, o);
+                if (ov > v || (ov == v && oi < ix)) { v = ov; ix = oi; }
+            }
+            if (lane == 0) {
+                const bool bad = !(v > 0.0) || !(v < 1.0e300 * 1.0e300);     // zero, NaN or Inf pivot
+                s_bad = bad ? 1 : 0;
+                s_piv = bad ? j : ix;
+                pv[j] = bad ? j : ix;
+                if (bad) atomicCAS(&info[blockIdx.x], 0, j + 1);
+            }
+        }
+        __syncthreads();
+        const int p = s_piv;
+        const bool bad = s_bad != 0;
+        // ---- swap rows j and p inside the panel, publish the pivot row
+        if (tid < w) {
+            c128 a = A[j + (size_t)(c0 + tid) * n];
+            if (p != j) { c128 bq = A[p + (size_t)(c0 + tid) * n]; A[p + (size_t)(c0 + tid) * n] = a; A[j + (size_t)(c0 + tid) * n] = bq; a = bq; }
+            urow[tid] = a;
+        }
+        __syncthreads();
+        // ---- scale column j, rank-1 update of the remaining panel columns, next column's max
+        bv = -1.0; bi = 0x7fffffff;
+        if (!bad) {
+            const c128 rp = crecip(urow[jj]);
+            for (int i = j + 1 + tid; i < n; i += PANEL_THREADS) {
+                c128 l = cmul(A[i + (size_t)j * n], rp);
+                A[i + (size_t)j * n] = l;
+                for (int t = jj + 1; t < w; ++t) {
+                    c128 a = A[i + (size_t)(c0 + t) * n];
+                    cfms(a, l, urow[t]);
+                    A[i + (size_t)(c0 + t) * n] = a;
+                    if (t == jj + 1 && i < ne) { double vv = cabs1(a); if (vv > bv) { bv = vv; bi = i; } }
+                }
+            }
+        } else if (jj + 1 < w) {
+            for (int i = j + 1 + tid; i < ne; i += PANEL_THREADS) {
+                double vv = cabs1(A[i + (size_t)(j + 1) * n]);
+                if (vv > bv) { bv = vv; bi = i; }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------- K3: interchanges + U12 = L11^{-1} A12
+// One thread per target column c in [col_lo, col_hi) (columns of the panel itself are skipped by the
+// caller's ranges).  mode bit 0: apply the w interchanges of panel [c0, c0+w) in order; mode bit 1:
+// solve the w x w unit-lower triangle L11 against rows [c0, c0+w) of the column.
+constexpr int K3_THREADS = 128;
+
+__global__ void __launch_bounds__(K3_THREADS)
+k_swap_trsm(c128* __restrict__ base, size_t stride, int n, int c0, int w, int col_lo, int col_hi, int mode,
+            const int* __restrict__ piv) {
+    const bool do_swap = mode & 1, do_trsm = mode & 2;
+    c128* A = base + (size_t)blockIdx.y * stride;
+    const int* pv = piv + (size_t)blockIdx.y * n + c0;
+    __shared__ c128 L[MAX_IB * MAX_IB];
+    __shared__ int sp[MAX_IB];
+    if (threadIdx.x < w) sp[threadIdx.x] = pv[threadIdx.x];
+    if (do_trsm)
+        for (int e = threadIdx.x; e < w * w; e += K3_THREADS) { int r = e % w, c = e / w; L[r + MAX_IB * c] = A[(c0 + r) + (size_t)(c0 + c) * n]; }
+    __syncthreads();
+    const int c = col_lo + blockIdx.x * K3_THREADS + threadIdx.x;
+    if (c >= col_hi) return;
+    c128* col = A + (size_t)c * n;
+    c128 x[MAX_IB];
+#pragma unroll
+    for (int i = 0; i < MAX_IB; ++i) x[i] = (i < w) ? col[c0 + i] : cmake(0.0, 0.0);
+    // interchanges, in order (a row index may appear more than once)
+#pragma unroll
+    for (int i = 0; i < MAX_IB; ++i) {
+        if (do_swap && i < w) {
+            const int p = sp[i];
+            if (p != c0 + i) {
+                if (p < c0 + w) {
+                    // both rows are in registers: static indexing through a select chain
+                    c128 xi = x[i], xp = xi;
+#pragma unroll
+                    for (int t = 0; t < MAX_IB; ++t) if (t == p - c0) xp = x[t];
+#pragma unroll
+                    for (int t = 0; t < MAX_IB; ++t) if (t == p - c0) x[t] = xi;
+                    x[i] = xp;
+                } else {
+                    c128 t = col[p]; col[p] = x[i]; x[i] = t;
+                }
+            }
+        }
+    }
+    if (do_trsm) {
+#pragma unroll
+        for (int j = 0; j < MAX_IB; ++j)
+#pragma unroll
+            for (int i = j + 1; i < MAX_IB; ++i)
+                if (i < w) cfms(x[i], L[i + MAX_IB * j], x[j]);
+    }
+#pragma unroll
+    for (int i = 0; i < MAX_IB; ++i) if (i < w) col[c0 + i] = x[i];
+}
+
+// ---------------------------------------------------------------- K5: tau00 = S^{-1}
+// One CTA per matrix: in-place Gauss-Jordan inversion with partial pivoting of the trailing k x k
+// block, in shared memory when it fits (k <= 96), else in a global scratch buffer.
+constexpr int K5_THREADS = 256;
+
+__global__ void __launch_bounds__(K5_THREADS)
+k_final_inverse(const c128* __restrict__ base, size_t stride, int n, int k, c128* __restrict__ tau, int* __restrict__ info,
+                c128* __restrict__ gscratch, int use_smem) {
+    extern __shared__ __align__(16) unsigned char k5_smem[];
+    const c128* A = base + (size_t)blockIdx.x * stride;
+    const int ne = n - k;
+    c128* S = use_smem ? reinterpret_cast<c128*>(k5_smem) : gscratch + (size_t)blockIdx.x * k * k;
+    __shared__ int cpiv[256];
+    __shared__ int s_p;
+    __shared__ c128 s_rp;
+    __shared__ double wv[K5_THREADS / 32];
+    __shared__ int wi[K5_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int e = tid; e < k * k; e += K5_THREADS) { int r = e % k, c = e / k; S[e] = A[(ne + r) + (size_t)(ne + c) * n]; }
+    __syncthreads();
+    bool failed = false;
+    for (int j = 0; j < k; ++j) {
+        double bv = -1.0; int bi = 0x7fffffff;
+        for (int i = j + tid; i < k; i += K5_THREADS) { double v = cabs1(S[i + (size_t)j * k]); if (v > bv) { bv = v; bi = i; } }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            double ov = __shfl_xor_sync(0xffffffffu, bv, o); int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+        }
+        if (lane == 0) { wv[warp] = bv; wi[warp] = bi; }
+        __syncthreads();
+        if (tid == 0) {
+            for (int t = 1; t < K5_THREADS / 32; ++t) if (wv[t] > bv || (wv[t] == bv && wi[t] < bi)) { bv = wv[t]; bi = wi[t]; }
+            const bool bad = !(bv > 0.0) || !(bv < 1.0e300 * 1.0e300);
+            s_p = bad ? -1 : bi;
+            if (bad) atomicCAS(&info[blockIdx.x], 0, ne + j + 1);
+            else { cpiv[j] = bi; s_rp = crecip(S[bi + (size_t)j * k]); }
+        }
+        __syncthreads();
+        const int p = s_p;
+        if (p < 0) { failed = true; break; }
+        // swap rows j <-> p
+        if (p != j) for (int c = tid; c < k; c += K5_THREADS) { c128 t = S[j + (size_t)c * k]; S[j + (size_t)c * k] = S[p + (size_t)c * k]; S[p + (size_t)c * k] = t; }
+        __syncthreads();
+        // row j <- row j / pivot, with a_jj := 1 first
+        const c128 rp = s_rp;
+        for (int c = tid; c < k; c += K5_THREADS) {
+            c128 v = (c == j) ? cmake(1.0, 0.0) : S[j + (size_t)c * k];
+            S[j + (size_t)c * k] = cmul(v, rp);
+        }
+        __syncthreads();
+        // eliminate column j from every other row: f = a_ij, a_ij := 0, row_i -= f * row_j
+        for (int e = tid; e < k * k; e += K5_THREADS) {
+            int i = e % k, c = e / k;
+            if (i == j) continue;
+            c128 f = S[i + (size_t)j * k];
+            if (c == j) continue;                  // column j itself is handled after the sweep
+            c128 v = S[i + (size_t)c * k];
+            cfms(v, f, S[j + (size_t)c * k]);
+            S[i + (size_t)c * k] = v;
+        }
+        __syncthreads();
+        for (int i = tid; i < k; i += K5_THREADS) {
+            if (i == j) continue;
+            c128 f = S[i + (size_t)j * k];
+            S[i + (size_t)j * k] = cneg(cmul(f, S[j + (size_t)j * k]));
+        }
+        __syncthreads();
+    }
+    if (!failed) {
+        // undo the row interchanges as column interchanges, in reverse order
+        for (int j = k - 1; j >= 0; --j) {
+            const int p = cpiv[j];
+            if (p != j) for (int r = tid; r < k; r += K5_THREADS) { c128 t = S[r + (size_t)j * k]; S[r + (size_t)j * k] = S[r + (size_t)p * k]; S[r + (size_t)p * k] = t; }
+            __syncthreads();
+        }
+    }
+    c128* out = tau + (size_t)blockIdx.x * k * k;
+    for (int e = tid; e < k * k; e += K5_THREADS) out[e] = S[e];
+}
+
+size_t final_inverse_ws_bytes(int k, int batch) { return k > 96 ? (size_t)batch * k * k * sizeof(c128) : 0; }
+
+// ---------------------------------------------------------------- verification: X = M^{-1} E
+// After the restricted-pivot elimination the system reads [U11 U12; 0 S] X = [0; I] (the
+// interchanges never touch the central rows, where E is non-zero), so X2 = S^{-1} = tau00 and
+// X1 = -U11^{-1} (U12 X2).  One CTA per (item, column of X).  Slow by design; not timed.
+__global__ void __launch_bounds__(256)
+k_backsolve_central(const c128* __restrict__ LU, size_t stride, int n, int k, const c128* __restrict__ tau, c128* __restrict__ X) {
+    const c128* A = LU + (size_t)blockIdx.y * stride;
+    const c128* T = tau + (size_t)blockIdx.y * k * k + (size_t)blockIdx.x * k;     // column of tau00
+    c128* x = X + ((size_t)blockIdx.y * k + blockIdx.x) * n;
+    const int ne = n - k, tid = threadIdx.x;
+    __shared__ c128 s_x;
+    for (int i = tid; i < k; i += 256) x[ne + i] = T[i];
+    // rhs = -U12 * X2
+    for (int i = tid; i < ne; i += 256) {
+        c128 s = cmake(0.0, 0.0);
+        for (int c = 0; c < k; ++c) cfms(s, A[i + (size_t)(ne + c) * n], T[c]);
+        x[i] = s;
+    }
+    __syncthreads();
+    for (int j = ne - 1; j >= 0; --j) {
+        if (tid == 0) { c128 v = cdiv(x[j], A[j + (size_t)j * n]); x[j] = v; s_x = v; }
+        __syncthreads();
+        const c128 xj = s_x;
+        for (int i = tid; i < j; i += 256) { c128 v = x[i]; cfms(v, A[i + (size_t)j * n], xj); x[i] = v; }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------- host launchers
+
+int launch_panel(c128* base, size_t stride, int n, int c0, int w, int ne, int batch, int* piv, int* info, cudaStream_t st) {
+    k_panel<<<batch, PANEL_THREADS, 0, st>>>(base, stride, n, c0, w, ne, piv, info);
+    LSMS_LAUNCH_CHECK();
+    return 0;
+}
+
+int launch_swap_trsm(c128* base, size_t stride, int n, int c0, int w, int col_lo, int col_hi, int mode, int batch,
+                     const int* piv, cudaStream_t st) {
+    if (col_hi <= col_lo) return 0;
+    for (int b0 = 0; b0 < batch; b0 += 65535) {
+        int nb = batch - b0 < 65535 ? batch - b0 : 65535;
+        dim3 grid((col_hi - col_lo + K3_THREADS - 1) / K3_THREADS, nb);
+        k_swap_trsm<<<grid, K3_THREADS, 0, st>>>(base + (size_t)b0 * stride, stride, n, c0, w, col_lo, col_hi, mode, piv + (size_t)b0 * n);
+        LSMS_LAUNCH_CHECK();
+    }
+    return 0;
+}
+
+int launch_final_inverse(c128* base, size_t stride, int n, int k, int batch, c128* tau, int* info, void* ws, cudaStream_t st) {
+    const int use_smem = k <= 96;
+    size_t smem = use_smem ? (size_t)k * k * sizeof(c128) : 0;
+    static bool attr_set = false;
+    if (!attr_set) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_final_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 96 * 16)); attr_set = true; }
+    k_final_inverse<<<batch, K5_THREADS, smem, st>>>(base, stride, n, k, tau, info, (c128*)ws, use_smem);
+    LSMS_LAUNCH_CHECK();
+    return 0;
+}
+
+int launch_backsolve_central(const c128* LU, size_t stride, int n, int k, int batch, const c128* tau, c128* X, cudaStream_t st) {
+    dim3 grid(k, batch);
+    k_backsolve_central<<<grid, 256, 0, st>>>(LU, stride, n, k, tau, X);
+    LSMS_LAUNCH_CHECK();
+    return 0;
+}
+
+}  // namespace lsms

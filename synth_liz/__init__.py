@@ -196,8 +196,9 @@ class LizBatch:
 
 
 def make_batch(cfg: LizConfig | str, n_atoms: int | None = None,
-               n_energies: int | None = None) -> LizBatch:
-    """Full synthetic batch of a config (optionally fewer atoms / energies)."""
+               n_energies: int | None = None, atom_offset: int = 0) -> LizBatch:
+    """Full synthetic batch of a config (optionally fewer atoms / energies; atom_offset shifts the
+    central-atom index, i.e. the occupancy/moment streams -- used to give every rank its own atoms)."""
     if isinstance(cfg, str):
         cfg = CONFIGS[cfg]
     na = cfg.n_atoms if n_atoms is None else n_atoms
@@ -213,7 +214,7 @@ def make_batch(cfg: LizConfig | str, n_atoms: int | None = None,
     mom = np.zeros((B, cfg.n_sites, 3), dtype=np.float64)
     z = np.zeros(B, dtype=np.complex128)
     for a in range(na):
-        sp, m = atom_occupancy_and_moments(cfg, a)
+        sp, m = atom_occupancy_and_moments(cfg, a + atom_offset)
         species[a * ne:(a + 1) * ne] = sp
         mom[a * ne:(a + 1) * ne] = m
         z[a * ne:(a + 1) * ne] = zq
