@@ -151,6 +151,7 @@ def main() -> None:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--nb", type=int, default=0, help="outer panel width override (0 = library default)")
     ap.add_argument("--ib", type=int, default=0, help="inner panel width override")
+    ap.add_argument("--no-lookahead", action="store_true", help="factor the next panel in front of, not under, the update")
     args = ap.parse_args()
     cfg = sl.CONFIGS[args.workload]
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -176,6 +177,7 @@ def main() -> None:
     lt.lib()
     if args.nb or args.ib:
         lt.lsms_set_blocking(args.nb, args.ib)
+    lt.lsms_set_lookahead(not args.no_lookahead)
 
     # ---- inputs: every rank gets its own central atoms (weak scaling: per-GPU work fixed)
     batch = sl.make_batch(cfg, atom_offset=rank * cfg.n_atoms)

@@ -119,8 +119,15 @@ int lsms_tau00_from_host(const lsms_c128* delta_host, const int* species_host, c
                          size_t* h2d_bytes, size_t* d2h_bytes);
 
 /* Tuning knobs (process-wide, not thread-safe; defaults chosen per shape when 0):
- *   outer panel width NB (multiple of 16, <= 128) and inner panel width IB (<= 16).             */
+ *   outer panel width NB (multiple of 4, <= 96; the workspace size depends on it: query
+ *   lsms_workspace_bytes after setting it) and inner panel width IB (<= 16).             */
 int lsms_set_blocking(int nb_outer, int ib_inner);
+
+/* Look-ahead (default on): the next panel is factored on a library-owned high-priority stream while the
+ * caller's stream runs the Schur update of the remaining columns; the two are joined with events before
+ * the call returns to the next panel, so the caller still sees one ordered stream.  The auxiliary stream
+ * and two events are created on first use and are the library's only persistent objects. */
+int lsms_set_lookahead(int on);
 
 /* How many kernels the last lsms_tau00_batched / lsms_build_M_batched call on this thread enqueued. */
 int lsms_last_launch_count(void);
@@ -130,7 +137,8 @@ int lsms_last_launch_count(void);
  * events on the caller's stream.  lsms_profile_end synchronises those events and returns, per class,
  * the summed device time in ms, the number of launches and the algorithmic flops (K4 classes only):
  *   0 K1 assembly, 1 K2 panel LU, 2 K3 interchanges+TRSM, 3 K4 inner rank-IB updates,
- *   4 K4 Schur update (inner dimension NB), 5 K5 final inverse; entries 6,7 unused.
+ *   4 K4 Schur update (inner dimension NB), 5 K5 final inverse, 6 K3a/K3b net row permutation + -(L11^-1),
+ *   7 K4 used as the triangular solve U12 = -(Ninv * A12).
  * All three arrays are HOST arrays of 8 entries. */
 int lsms_profile_begin(void);
 int lsms_profile_end(double* ms_by_class_host, int* launches_by_class_host, double* flops_by_class_host);

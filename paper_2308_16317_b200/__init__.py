@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "lsms_version", "lsms_workspace_bytes", "lsms_solve_workspace_bytes", "lsms_host_call_scratch_bytes",
     "lsms_tinv_from_phase_shifts", "lsms_build_M_batched", "lsms_tau00_batched",
-    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_set_blocking",
+    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_set_blocking", "lsms_set_lookahead",
     "lsms_last_launch_count", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe", "lsms_schur_update_batched",
     "lsms_debug_gaunt_closed_form",
 )
@@ -95,11 +95,16 @@ def lsms_set_blocking(nb_outer: int = 0, ib_inner: int = 0) -> None:
     _check(lib().lsms_set_blocking(nb_outer, ib_inner), "lsms_set_blocking")
 
 
+def lsms_set_lookahead(on: bool = True) -> None:
+    _check(lib().lsms_set_lookahead(int(bool(on))), "lsms_set_lookahead")
+
+
 def lsms_last_launch_count() -> int:
     return int(lib().lsms_last_launch_count())
 
 
-KERNEL_CLASSES = ("K1_assemble", "K2_panel", "K3_swap_trsm", "K4_inner_gemm", "K4_schur_gemm", "K5_final_inverse")
+KERNEL_CLASSES = ("K1_assemble", "K2_panel", "K3_swap_trsm", "K4_inner_gemm", "K4_schur_gemm", "K5_final_inverse",
+                  "K3_permute_ninv", "K4_trsm_gemm")
 
 
 def lsms_profile_begin() -> None:

@@ -14,7 +14,7 @@ static int g_nb_outer = 0, g_ib_inner = 0;
 // ---- optional per-kernel-class timing (lsms_profile_begin / lsms_profile_end): CUDA events recorded on
 // the caller's stream around each launch, so bench.py can report the Schur update's duration and share
 // measured inside the step.  Classes: 0 K1 assembly, 1 K2 panel, 2 K3 swap/trsm, 3 K4 inner (K <= IB),
-// 4 K4 Schur update (K = NB), 5 K5 final inverse.
+// 4 K4 Schur update (K = NB), 5 K5 final inverse, 6 K3a/K3b net permutation + Ninv, 7 K4 as TRSM (U12 = -Ninv*A12).
 struct Prof {
     bool on = false;
     std::vector<cudaEvent_t> ev;     // pairs
@@ -43,10 +43,24 @@ static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t
 
 static int isqrt_exact(int v) { int r = (int)lround(sqrt((double)v)); return (r * r == v) ? r : -1; }
 
-// Workspace layout for lsms_tau00_batched: [pivots int32 batch*n][K5 scratch]
-static size_t tau_ws_bytes(int n, int k, int batch) {
-    return align256((size_t)batch * n * sizeof(int)) + align256(final_inverse_ws_bytes(k, batch));
+static inline int eff_nb() { return g_nb_outer > 0 ? g_nb_outer : 64; }
+static inline int eff_ib() { return g_ib_inner > 0 ? g_ib_inner : 16; }
+
+// Workspace layout for lsms_tau00_batched:
+//   [pivots int32 batch*n][perm int32 batch*(4+3NB)][Ninv c128 batch*NB*NB][Tperm c128 batch*NB*n][K5 scratch]
+struct TauWs { int* piv; int* perm; c128* ninv; c128* tperm; void* k5; size_t total; };
+static TauWs tau_ws_layout(void* base, int n, int k, int batch) {
+    const int NB = eff_nb();
+    TauWs w; char* p = (char*)base;
+    w.piv = (int*)p; p += align256((size_t)batch * n * sizeof(int));
+    w.perm = (int*)p; p += align256((size_t)batch * (4 + 3 * NB) * sizeof(int));
+    w.ninv = (c128*)p; p += align256((size_t)batch * NB * NB * sizeof(c128));
+    w.tperm = (c128*)p; p += align256((size_t)batch * NB * n * sizeof(c128));
+    w.k5 = p; p += align256(final_inverse_ws_bytes(k, batch));
+    w.total = (size_t)(p - (char*)base);
+    return w;
 }
+static size_t tau_ws_bytes(int n, int k, int batch) { return tau_ws_layout(nullptr, n, k, batch).total; }
 
 // Blocked right-looking elimination of the first ne = n-k columns of every item, in lock-step over
 // the batch: each launch covers all items, so the latency-bound panel kernels (one CTA per item)
@@ -56,55 +70,98 @@ static size_t tau_ws_bytes(int n, int k, int batch) {
 //        K2  factor the (n-c0) x w panel, pivots restricted to rows < ne
 //        K3  interchanges on the outer panel's other columns; TRSM on those to the right
 //        K4  rank-w update of the outer panel's remaining columns
-//     K3  all W interchanges on the trailing columns [J+W, n)         (before any update: rows
-//                                                                      that cross J+W must be equal)
-//     for each inner block: K3 TRSM of its w rows, K4 rank-w update of rows [c0+w, J+W)
+//     K3a fold the W interchanges into one row permutation; Ninv = -(L11^{-1})
+//     K3b permute the trailing columns [J+W, n): new top block -> Tperm, displaced rows scattered
+//     K4  U12 = -(Ninv * Tperm)        (the triangular solve as a DMMA GEMM, written into the matrix)
 //     K4  Schur update A22 -= L21 U12 with inner dimension W          (>95% of the flops)
-static int eliminate(c128* M, int n, int k, int batch, int* piv, int* info, cudaStream_t st) {
-    const int ne = n - k;
-    int NB = g_nb_outer > 0 ? g_nb_outer : 64;
-    int IB = g_ib_inner > 0 ? g_ib_inner : 16;
+//
+// Look-ahead (the batch scheduler's overlap): after the triangular solve of panel J the
+// Schur update is split in two.  The columns of the NEXT panel are updated first; then the next panel is
+// factored on a high-priority auxiliary stream while the main stream updates the remaining columns.  The
+// latency/L2-bound panel kernels thus run underneath the DMMA-bound update instead of in front of it.
+// The two streams touch disjoint columns (the panel's interchanges reach the trailing columns only in K3b,
+// after the join).  The auxiliary stream and two events are the library's only persistent objects.
+static int g_lookahead = 1;
+static cudaStream_t g_aux = nullptr;
+static cudaEvent_t g_ev_fork = nullptr, g_ev_join = nullptr;
+
+static int ensure_aux() {
+    if (g_aux) return 0;
+    int lo = 0, hi = 0;
+    LSMS_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    LSMS_CUDA_OK(cudaStreamCreateWithPriority(&g_aux, cudaStreamNonBlocking, hi));
+    LSMS_CUDA_OK(cudaEventCreateWithFlags(&g_ev_fork, cudaEventDisableTiming));
+    LSMS_CUDA_OK(cudaEventCreateWithFlags(&g_ev_join, cudaEventDisableTiming));
+    return 0;
+}
+
+// factor the outer panel [J, J+W) on stream st: inner panels of width <= IB
+static int factor_panel(c128* M, int n, int batch, int J, int W, int ne, int IB, int* piv, int* info, cudaStream_t st) {
     const size_t stride = (size_t)n * n;
-    GemmShape g; g.base = M; g.batch_stride = stride; g.ld = n; g.batch = batch;
+    const int Jend = J + W;
+    GemmShape g; g.strideA = g.strideB = g.strideC = stride; g.ldA = g.ldB = g.ldC = n; g.batch = batch; g.beta0 = 0;
+    for (int jj = 0; jj < W; jj += IB) {
+        const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
+        int rc; { ProfScope ps(1, st); rc = launch_panel(M, stride, n, c0, w, ne, batch, piv, info, st); } if (rc) return rc;
+        { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, J, c0, 1, batch, piv, st); } if (rc) return rc;
+        { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, c0 + w, Jend, 3, batch, piv, st); } if (rc) return rc;
+        const int rem = Jend - (c0 + w);
+        if (rem > 0) {
+            g.Mr = n - (c0 + w); g.Nc = rem; g.K = w;
+            g.A = M + (size_t)(c0 + w) + (size_t)c0 * n;
+            g.B = M + (size_t)c0 + (size_t)(c0 + w) * n;
+            g.C = M + (size_t)(c0 + w) + (size_t)(c0 + w) * n;
+            { ProfScope ps(3, st, 8.0 * g.Mr * g.Nc * g.K * batch); rc = launch_schur_gemm(g, st); } if (rc) return rc;
+        }
+    }
+    return 0;
+}
+
+// A22[:, c_lo:c_hi) -= L21 * U12[:, c_lo:c_hi) for the outer panel [J, J+W)
+static int schur_update(c128* M, int n, int batch, int J, int W, int c_lo, int c_hi, cudaStream_t st) {
+    if (c_hi <= c_lo) return 0;
+    const int Jend = J + W;
+    GemmShape g; g.strideA = g.strideB = g.strideC = (size_t)n * n; g.ldA = g.ldB = g.ldC = n; g.batch = batch; g.beta0 = 0;
+    g.Mr = n - Jend; g.Nc = c_hi - c_lo; g.K = W;
+    g.A = M + (size_t)Jend + (size_t)J * n;
+    g.B = M + (size_t)J + (size_t)c_lo * n;
+    g.C = M + (size_t)Jend + (size_t)c_lo * n;
+    ProfScope ps(4, st, 8.0 * g.Mr * g.Nc * g.K * batch);
+    return launch_schur_gemm(g, st);
+}
+
+static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* info, cudaStream_t st) {
+    const int ne = n - k;
+    const int NB = eff_nb(), IB = eff_ib();
+    const size_t stride = (size_t)n * n;
+    int* piv = ws.piv;
+    const bool la = g_lookahead != 0;
+    if (la) { int rc = ensure_aux(); if (rc) return rc; }
+    if (ne <= 0) return 0;
+    int rc = factor_panel(M, n, batch, 0, ne < NB ? ne : NB, ne, IB, piv, info, st); if (rc) return rc;
     for (int J = 0; J < ne; J += NB) {
         const int W = (ne - J < NB) ? ne - J : NB;
-        const int Jend = J + W;
-        for (int jj = 0; jj < W; jj += IB) {
-            const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
-            int rc; { ProfScope ps(1, st); rc = launch_panel(M, stride, n, c0, w, ne, batch, piv, info, st); } if (rc) return rc;
-            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, J, c0, 1, batch, piv, st); } if (rc) return rc;
-            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, c0 + w, Jend, 3, batch, piv, st); } if (rc) return rc;
-            const int rem = Jend - (c0 + w);
-            if (rem > 0) {
-                g.Mr = n - (c0 + w); g.Nc = rem; g.K = w;
-                g.offA = (size_t)(c0 + w) + (size_t)c0 * n;
-                g.offB = (size_t)c0 + (size_t)(c0 + w) * n;
-                g.offC = (size_t)(c0 + w) + (size_t)(c0 + w) * n;
-                { ProfScope ps(3, st, 8.0 * g.Mr * g.Nc * g.K * batch); rc = launch_schur_gemm(g, st); } if (rc) return rc;
-            }
-        }
-        if (Jend < n) {
-            for (int jj = 0; jj < W; jj += IB) {
-                const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
-                int rc; { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, Jend, n, 1, batch, piv, st); } if (rc) return rc;
-            }
-            for (int jj = 0; jj < W; jj += IB) {
-                const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
-                int rc; { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, Jend, n, 2, batch, piv, st); } if (rc) return rc;
-                const int rem = Jend - (c0 + w);
-                if (rem > 0) {
-                    g.Mr = rem; g.Nc = n - Jend; g.K = w;
-                    g.offA = (size_t)(c0 + w) + (size_t)c0 * n;
-                    g.offB = (size_t)c0 + (size_t)Jend * n;
-                    g.offC = (size_t)(c0 + w) + (size_t)Jend * n;
-                    { ProfScope ps(3, st, 8.0 * g.Mr * g.Nc * g.K * batch); rc = launch_schur_gemm(g, st); } if (rc) return rc;
-                }
-            }
-            g.Mr = n - Jend; g.Nc = n - Jend; g.K = W;
-            g.offA = (size_t)Jend + (size_t)J * n;
-            g.offB = (size_t)J + (size_t)Jend * n;
-            g.offC = (size_t)Jend + (size_t)Jend * n;
-            int rc; { ProfScope ps(4, st, 8.0 * g.Mr * g.Nc * g.K * batch); rc = launch_schur_gemm(g, st); } if (rc) return rc;
+        const int Jend = J + W;                               // Jend <= ne < n
+        { ProfScope ps(6, st); rc = launch_panel_post(M, stride, n, J, W, batch, piv, ws.perm, ws.ninv, NB, st); } if (rc) return rc;
+        { ProfScope ps(6, st); rc = launch_row_permute(M, stride, n, J, W, Jend, n, batch, ws.perm, ws.tperm, (size_t)NB * n, NB, st); } if (rc) return rc;
+        GemmShape t; t.batch = batch; t.beta0 = 1;
+        t.A = ws.ninv; t.strideA = (size_t)NB * NB; t.ldA = NB;
+        t.B = ws.tperm + (size_t)Jend * NB; t.strideB = (size_t)NB * n; t.ldB = NB;
+        t.C = M + (size_t)J + (size_t)Jend * n; t.strideC = stride; t.ldC = n;
+        t.Mr = W; t.Nc = n - Jend; t.K = W;
+        { ProfScope ps(7, st, 8.0 * t.Mr * t.Nc * t.K * batch); rc = launch_schur_gemm(t, st); } if (rc) return rc;
+        const int W2 = (Jend < ne) ? ((ne - Jend < NB) ? ne - Jend : NB) : 0;     // width of the next panel
+        if (W2 > 0 && la) {
+            rc = schur_update(M, n, batch, J, W, Jend, Jend + W2, st); if (rc) return rc;
+            LSMS_CUDA_OK(cudaEventRecord(g_ev_fork, st));
+            LSMS_CUDA_OK(cudaStreamWaitEvent(g_aux, g_ev_fork, 0));
+            rc = factor_panel(M, n, batch, Jend, W2, ne, IB, piv, info, g_aux); if (rc) return rc;
+            LSMS_CUDA_OK(cudaEventRecord(g_ev_join, g_aux));
+            rc = schur_update(M, n, batch, J, W, Jend + W2, n, st); if (rc) return rc;
+            LSMS_CUDA_OK(cudaStreamWaitEvent(st, g_ev_join, 0));
+        } else {
+            rc = schur_update(M, n, batch, J, W, Jend, n, st); if (rc) return rc;
+            if (W2 > 0) { rc = factor_panel(M, n, batch, Jend, W2, ne, IB, piv, info, st); if (rc) return rc; }
         }
     }
     return 0;
@@ -186,10 +243,10 @@ int lsms_tau00_batched(lsms_c128* M, int n_sites, int kmax, int spin_canted, int
     if (workspace_bytes < tau_ws_bytes(n, k, batch)) return -9;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     g_launches.n = 0;
-    int* piv = (int*)workspace;
-    void* k5ws = (char*)workspace + align256((size_t)batch * n * sizeof(int));
+    const TauWs ws = tau_ws_layout(workspace, n, k, batch);
+    void* k5ws = ws.k5;
     LSMS_CUDA_OK(cudaMemsetAsync(info, 0, (size_t)batch * sizeof(int), st));
-    int rc = eliminate((c128*)M, n, k, batch, piv, info, st);
+    int rc = eliminate((c128*)M, n, k, batch, ws, info, st);
     if (rc) return rc;
     ProfScope ps(5, st);
     return launch_final_inverse((c128*)M, (size_t)n * n, n, k, batch, (c128*)tau00_out, info, k5ws, st);
@@ -296,11 +353,13 @@ int lsms_tau00_from_host(const lsms_c128* delta_host, const int* species_host, c
 }
 
 int lsms_set_blocking(int nb_outer, int ib_inner) {
-    if (nb_outer < 0 || nb_outer > 256 || (nb_outer % 4) != 0) return -1;
+    if (nb_outer < 0 || nb_outer > 96 || (nb_outer % 4) != 0) return -1;
     if (ib_inner < 0 || ib_inner > 16) return -2;
     g_nb_outer = nb_outer; g_ib_inner = ib_inner;
     return 0;
 }
+
+int lsms_set_lookahead(int on) { g_lookahead = on ? 1 : 0; return 0; }
 
 int lsms_last_launch_count(void) { return g_launches.n; }
 
@@ -338,10 +397,11 @@ int lsms_schur_update_batched(lsms_c128* M, int n, int c0, int kk, int batch, vo
     if (n < 2) return -2;
     if (c0 < 0 || kk < 1 || c0 + kk >= n) return -3;
     if (batch < 1) return -5;
-    GemmShape g; g.base = (c128*)M; g.batch_stride = (size_t)n * n; g.ld = n; g.batch = batch;
+    GemmShape g; g.strideA = g.strideB = g.strideC = (size_t)n * n; g.ldA = g.ldB = g.ldC = n; g.batch = batch; g.beta0 = 0;
     const int r0 = c0 + kk;
+    c128* base = (c128*)M;
     g.Mr = n - r0; g.Nc = n - r0; g.K = kk;
-    g.offA = (size_t)r0 + (size_t)c0 * n; g.offB = (size_t)c0 + (size_t)r0 * n; g.offC = (size_t)r0 + (size_t)r0 * n;
+    g.A = base + (size_t)r0 + (size_t)c0 * n; g.B = base + (size_t)c0 + (size_t)r0 * n; g.C = base + (size_t)r0 + (size_t)r0 * n;
     g_launches.n = 0;
     return launch_schur_gemm(g, (cudaStream_t)cuda_stream);
 }

@@ -105,128 +105,144 @@ __global__ void k_tinv(const c128* __restrict__ delta, const int* __restrict__ s
     tinv[e] = cneg(cdiv(kap, cmul(sn, ex)));       // -kappa / (sin d e^{i d})
 }
 
-// ---------------------------------------------------------------- K1: block assembly
+// ---------------------------------------------------------------- Legendre recurrence table
+// Fully normalised recurrence  Pbar_lm = a_lm (x Pbar_{l-1,m} - b_lm Pbar_{l-2,m}),
+// Pbar_mm = d_m sin(theta) Pbar_{m-1,m-1}; a, b, d tabulated once so that K1 has no sqrt/div inside.
+//   leg[0*S + l*(l2+1)+m] = a_lm, leg[1*S + ...] = b_lm, leg[2*S + m] = d_m,  S = (l2+1)^2
+__global__ void k_legendre_table(int l2, double* __restrict__ leg) {
+    const int S = (l2 + 1) * (l2 + 1);
+    for (int e = threadIdx.x; e < S; e += blockDim.x) {
+        const int l = e / (l2 + 1), m = e % (l2 + 1);
+        double a = 0.0, b = 0.0;
+        if (l > m) {
+            a = sqrt((4.0 * l * l - 1.0) / ((double)l * l - (double)m * m));
+            b = sqrt((((double)l - 1.0) * (l - 1.0) - (double)m * m) / (4.0 * (l - 1.0) * (l - 1.0) - 1.0));
+        }
+        leg[e] = a; leg[S + e] = b;
+        if (l == 0) leg[2 * S + m] = (m > 0) ? -sqrt((2.0 * m + 1.0) / (2.0 * m)) : 1.0;
+    }
+}
 
-constexpr int ASM_WARPS = 8;
+// ---------------------------------------------------------------- K1: column-strip assembly
+// One CTA per (column site sj, item b): it writes the k full columns of M that belong to site sj,
+// i.e. n*16 B contiguous per column (HBM-write-bound).
+//   phase 1 (a1): one thread per row site si != sj builds hY[si][L''] = h_{l''}(kappa R) Y_{L''}(R^) in smem
+//   phase 2 (a2): one thread per matrix row (si, s, L) walks the k columns (s', L') of the strip:
+//                 -g0 = -kappa sum_t coef_t hY[idx_t]   (s == s'),  0 (s != s'),  t^{-1} on the site diagonal.
+// Row sites are processed in chunks that fit shared memory.
+constexpr int ASM_THREADS = 256;
 
-__global__ void __launch_bounds__(ASM_WARPS * 32)
+__global__ void __launch_bounds__(ASM_THREADS)
 k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, const double* __restrict__ moment,
            const c128* __restrict__ kappa, const c128* __restrict__ coef, const int* __restrict__ idx,
-           int lmax, int n_sites, int canted, c128* __restrict__ Mout) {
-    extern __shared__ c128 smem[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+           const double* __restrict__ leg, int lmax, int n_sites, int canted, int chunk, c128* __restrict__ Mout) {
+    extern __shared__ __align__(16) unsigned char asm_smem[];
     const int kmax = (lmax + 1) * (lmax + 1), nt = lmax + 1, l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
-    const int nspin = canted ? 2 : 1, k = kmax * nspin;
+    const int nspin = canted ? 2 : 1, k = kmax * nspin, kk2 = kmax * kmax, S = nl2;
     const size_t n = (size_t)n_sites * k;
-    const int b = blockIdx.z, sj = blockIdx.x, si = blockIdx.y * ASM_WARPS + warp;
-    if (si >= n_sites) return;
-    c128* hY = smem + (size_t)warp * (nl2 + l2 + 1);
-    c128* hs = hY + nl2;
+    const int b = blockIdx.y, sj = blockIdx.x, tid = threadIdx.x;
+    c128* hY = reinterpret_cast<c128*>(asm_smem);                 // [chunk][nl2]
     c128* M = Mout + (size_t)b * n * n;
-    const size_t r0 = (size_t)(si == 0 ? n_sites - 1 : si - 1) * k, c0 = (size_t)(sj == 0 ? n_sites - 1 : sj - 1) * k;
+    const size_t c0 = (size_t)(sj == 0 ? n_sites - 1 : sj - 1) * k;
+    const c128 kap = kappa[b];
     const c128 zero = cmake(0.0, 0.0);
+    const double* pj = site_pos + ((size_t)b * n_sites + sj) * 3;
+    const double xj = pj[0], yj = pj[1], zj = pj[2];
 
-    if (si == sj) {
-        // site-diagonal block: t^{-1} (g0^{ii} = 0, "between two different atom sites")
-        const c128* ti = tinv + ((size_t)b * n_sites + si) * nspin * nt;
-        double ex = 0, ey = 0, ez = 0;
-        if (canted) { const double* mv = moment + ((size_t)b * n_sites + si) * 3; ex = mv[0]; ey = mv[1]; ez = mv[2]; }
-        for (int e = lane; e < k * k; e += 32) {
-            int r = e % k, c = e / k;
-            int Lr = r % kmax, Lc = c % kmax, sr = r / kmax, sc = c / kmax;
-            c128 v = zero;
-            if (Lr == Lc) {
-                int l = 0; while ((l + 1) * (l + 1) <= Lr) ++l;
-                if (!canted) v = ti[l];
-                else {
-                    c128 a = ti[l], bb = ti[nt + l];
-                    c128 hsum = cscale(0.5, cadd(a, bb)), hdif = cscale(0.5, csub(a, bb));
-                    if (sr == 0 && sc == 0) v = cadd(hsum, cscale(ez, hdif));
-                    else if (sr == 1 && sc == 1) v = csub(hsum, cscale(ez, hdif));
-                    else if (sr == 0) v = cmul(hdif, cmake(ex, -ey));       // (up,down): e_x - i e_y
-                    else v = cmul(hdif, cmake(ex, ey));                      // (down,up): e_x + i e_y
+    for (int s0 = 0; s0 < n_sites; s0 += chunk) {
+        const int ns = min(chunk, n_sites - s0);
+        __syncthreads();
+        // ---- phase 1: per-R tables
+        for (int q = tid; q < ns; q += ASM_THREADS) {
+            const int si = s0 + q;
+            if (si == sj) continue;
+            const double* pi = site_pos + ((size_t)b * n_sites + si) * 3;
+            const double Rx = pi[0] - xj, Ry = pi[1] - yj, Rz = pi[2] - zj;
+            const double R = sqrt(Rx * Rx + Ry * Ry + Rz * Rz);
+            c128* out = hY + (size_t)q * nl2;
+            // Y_lm(R^) by columns m (both signs), l = m..l2
+            const double ct = Rz / R, rho = sqrt(Rx * Rx + Ry * Ry), st = rho / R;
+            double cphi = 1.0, sphi = 0.0;
+            if (rho > 0.0) { cphi = Rx / rho; sphi = Ry / rho; }
+            double pmm = 0.28209479177387814347403972578039, er = 1.0, ei = 0.0;
+            for (int m = 0; m <= l2; ++m) {
+                if (m > 0) {
+                    pmm *= leg[2 * S + m] * st;
+                    const double t = er * cphi - ei * sphi; ei = er * sphi + ei * cphi; er = t;
+                }
+                double p2 = 0.0, p1 = pmm;
+                for (int l = m; l <= l2; ++l) {
+                    double pv = pmm;
+                    if (l > m) { pv = leg[l * (l2 + 1) + m] * (ct * p1 - leg[S + l * (l2 + 1) + m] * p2); p2 = p1; p1 = pv; }
+                    const c128 y = cmake(pv * er, pv * ei);
+                    out[l * (l + 1) + m] = y;
+                    if (m > 0) out[l * (l + 1) - m] = (m & 1) ? cmake(-y.x, y.y) : cmake(y.x, -y.y);   // (-1)^m conj
                 }
             }
-            M[(r0 + r) + n * (c0 + c)] = v;
-        }
-        return;
-    }
-
-    // ---- per-R tables (a1): h_l(kappa R) for l <= 2 lmax, Y_lm(R^) for (2 lmax+1)^2 entries
-    const double* pi = site_pos + ((size_t)b * n_sites + si) * 3;
-    const double* pj = site_pos + ((size_t)b * n_sites + sj) * 3;
-    const double Rx = pi[0] - pj[0], Ry = pi[1] - pj[1], Rz = pi[2] - pj[2];
-    const double R = sqrt(Rx * Rx + Ry * Ry + Rz * Rz);
-    const c128 kap = kappa[b];
-    if (lane == 0) {
-        c128 x = cscale(R, kap);
-        double s, c; sincos(x.x, &s, &c);
-        double ed = exp(-x.y);
-        c128 eix = cmake(ed * c, ed * s);
-        c128 xinv = crecip(x);
-        c128 h0 = cmul(cmake(0.0, -1.0), cmul(eix, xinv));                       // -i e^{ix}/x
-        c128 h1 = cneg(cmul(cadd(cmake(1.0, 0.0), cmul(cmake(0.0, 1.0), xinv)), cmul(eix, xinv)));   // -(1+i/x) e^{ix}/x
-        hs[0] = h0; if (l2 >= 1) hs[1] = h1;
-        for (int l = 1; l < l2; ++l) {
-            c128 hn = csub(cscale((double)(2 * l + 1), cmul(xinv, h1)), h0);
-            hs[l + 1] = hn; h0 = h1; h1 = hn;
-        }
-    }
-    __syncwarp();
-    if (lane <= l2) {
-        // column m = lane of the normalised Legendre triangle; Y_lm = Pbar_lm e^{i m phi}
-        const int m = lane;
-        const double ct = Rz / R;
-        const double rho = sqrt(Rx * Rx + Ry * Ry);
-        const double st = rho / R;
-        double cphi = 1.0, sphi = 0.0;
-        if (rho > 0.0) { cphi = Rx / rho; sphi = Ry / rho; }
-        double pmm = 0.28209479177387814347403972578039;      // 1/sqrt(4 pi)
-        double er = 1.0, ei = 0.0;                             // e^{i m phi}
-        for (int i = 1; i <= m; ++i) {
-            pmm = -sqrt((2.0 * i + 1.0) / (2.0 * i)) * st * pmm;
-            double t = er * cphi - ei * sphi; ei = er * sphi + ei * cphi; er = t;
-        }
-        double p2 = 0.0, p1 = pmm;
-        for (int l = m; l <= l2; ++l) {
-            double p;
-            if (l == m) p = pmm;
-            else {
-                double a = sqrt((4.0 * l * l - 1.0) / ((double)l * l - (double)m * m));
-                double bq = sqrt((((double)l - 1.0) * (l - 1.0) - (double)m * m) / (4.0 * (l - 1.0) * (l - 1.0) - 1.0));
-                p = a * (ct * p1 - bq * p2);
-                p2 = p1; p1 = p;
+            // h_l(kappa R), l = 0..l2, multiplied in
+            const c128 x = cscale(R, kap);
+            double sn, cs; sincos(x.x, &sn, &cs);
+            const double ed = exp(-x.y);
+            const c128 eix = cmake(ed * cs, ed * sn);
+            const c128 xinv = crecip(x);
+            c128 h0 = cmul(cmake(0.0, -1.0), cmul(eix, xinv));                                        // -i e^{ix}/x
+            c128 h1 = cneg(cmul(cadd(cmake(1.0, 0.0), cmul(cmake(0.0, 1.0), xinv)), cmul(eix, xinv)));   // -(1+i/x) e^{ix}/x
+            for (int l = 0; l <= l2; ++l) {
+                c128 h = (l == 0) ? h0 : h1;
+                if (l >= 2) { h = csub(cscale((double)(2 * l - 1), cmul(xinv, h1)), h0); h0 = h1; h1 = h; }
+                for (int e = l * l; e < (l + 1) * (l + 1); ++e) out[e] = cmul(h, out[e]);
             }
-            c128 y = cmake(p * er, p * ei);
-            c128 h = hs[l];
-            hY[l * (l + 1) + m] = cmul(h, y);
-            if (m > 0) { c128 ym = (m & 1) ? cmake(-y.x, y.y) : cmake(y.x, -y.y); hY[l * (l + 1) - m] = cmul(h, ym); }   // (-1)^m conj
         }
-    }
-    __syncwarp();
-
-    // ---- block elements (a2): M_ij = -g0 = -kappa * sum_t coef_t * hY[idx_t]
-    const int kk2 = kmax * kmax;
-    for (int e = lane; e < kk2; e += 32) {
-        c128 s = zero;
-        for (int t = 0; t < nt; ++t) cfma(s, coef[t * kk2 + e], hY[idx[t * kk2 + e]]);
-        c128 g = cneg(cmul(kap, s));
-        int L = e % kmax, Lp = e / kmax;
-        M[(r0 + L) + n * (c0 + Lp)] = g;
-        if (canted) {
-            M[(r0 + kmax + L) + n * (c0 + kmax + Lp)] = g;
-            M[(r0 + kmax + L) + n * (c0 + Lp)] = zero;
-            M[(r0 + L) + n * (c0 + kmax + Lp)] = zero;
+        __syncthreads();
+        // ---- phase 2: rows of this chunk, all k columns of the strip
+        const int nrows = ns * k;
+        for (int rr = tid; rr < nrows; rr += ASM_THREADS) {
+            const int q = rr / k, w = rr % k, sr = w / kmax, L = w % kmax;
+            const int si = s0 + q;
+            const size_t row = (size_t)(si == 0 ? n_sites - 1 : si - 1) * k + w;
+            c128* dst = M + row + n * c0;
+            if (si == sj) {
+                // site-diagonal block: t^{-1} (g0^{ii} = 0, "between two different atom sites")
+                const c128* ti = tinv + ((size_t)b * n_sites + si) * nspin * nt;
+                int l = 0; while ((l + 1) * (l + 1) <= L) ++l;
+                c128 vd = ti[l], vo = zero;                      // same-spin and other-spin entry at column L
+                if (canted) {
+                    const double* mv = moment + ((size_t)b * n_sites + si) * 3;
+                    const c128 a = ti[l], bb = ti[nt + l];
+                    const c128 hsum = cscale(0.5, cadd(a, bb)), hdif = cscale(0.5, csub(a, bb));
+                    vd = (sr == 0) ? cadd(hsum, cscale(mv[2], hdif)) : csub(hsum, cscale(mv[2], hdif));
+                    vo = cmul(hdif, (sr == 0) ? cmake(mv[0], -mv[1]) : cmake(mv[0], mv[1]));   // (up,down): ex - i ey
+                }
+                for (int c = 0; c < k; ++c) {
+                    const int sc = c / kmax, Lc = c % kmax;
+                    dst[n * c] = (Lc == L) ? ((sc == sr) ? vd : vo) : zero;
+                }
+            } else {
+                const c128* hy = hY + (size_t)q * nl2;
+                for (int sc = 0; sc < nspin; ++sc)
+                    for (int Lp = 0; Lp < kmax; ++Lp) {
+                        c128 g = zero;
+                        if (sc == sr) {
+                            c128 s = zero;
+                            const int e = Lp * kmax + L;
+                            for (int t = 0; t < nt; ++t) cfma(s, coef[t * kk2 + e], hy[idx[t * kk2 + e]]);
+                            g = cneg(cmul(kap, s));
+                        }
+                        dst[n * (sc * kmax + Lp)] = g;
+                    }
+            }
         }
     }
 }
 
 // ---------------------------------------------------------------- host launchers
 
+static size_t al256(size_t x) { return (x + 255) / 256 * 256; }
+
 size_t gaunt_table_bytes(int lmax) {
     size_t kmax = (size_t)(lmax + 1) * (lmax + 1), nt = lmax + 1;
-    size_t e = kmax * kmax * nt;
-    return ((e * sizeof(c128) + 255) / 256) * 256 + ((e * sizeof(int) + 255) / 256) * 256;
+    size_t e = kmax * kmax * nt, S = (size_t)(2 * lmax + 1) * (2 * lmax + 1);
+    return al256(e * sizeof(c128)) + al256(e * sizeof(int)) + al256(3 * S * sizeof(double));
 }
 
 int launch_tinv(const c128* delta, const int* species, const c128* z, int lmax, int n_sites, int nspin, int batch,
@@ -242,20 +258,30 @@ int launch_tinv(const c128* delta, const int* species, const c128* z, int lmax, 
 int launch_assemble(const c128* tinv, const double* site_pos, const double* moment, const c128* kappa, int lmax,
                     int n_sites, int canted, int batch, c128* M, void* ws, cudaStream_t st) {
     size_t kmax = (size_t)(lmax + 1) * (lmax + 1), nt = lmax + 1, e = kmax * kmax * nt;
+    const int l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
     c128* coef = (c128*)ws;
-    int* idx = (int*)((char*)ws + ((e * sizeof(c128) + 255) / 256) * 256);
+    int* idx = (int*)((char*)ws + al256(e * sizeof(c128)));
+    double* leg = (double*)((char*)ws + al256(e * sizeof(c128)) + al256(e * sizeof(int)));
     k_gaunt_table<<<(unsigned)((e + 127) / 128), 128, 0, st>>>(lmax, coef, idx);
     LSMS_LAUNCH_CHECK();
-    int l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
-    size_t smem = (size_t)ASM_WARPS * (nl2 + l2 + 1) * sizeof(c128);
+    k_legendre_table<<<1, 128, 0, st>>>(l2, leg);
+    LSMS_LAUNCH_CHECK();
+    // row-site chunks: per-R tables of a chunk fit in ~108 KB (two CTAs per SM)
+    int maxchunk = (int)((108 * 1024) / ((size_t)nl2 * sizeof(c128)));
+    if (maxchunk < 1) maxchunk = 1;
+    const int nchunks = (n_sites + maxchunk - 1) / maxchunk;
+    const int chunk = (n_sites + nchunks - 1) / nchunks;      // balanced chunks
+    const size_t smem = (size_t)chunk * nl2 * sizeof(c128);
+    static size_t attr = 0;
+    if (smem > attr) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_assemble, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
+    const size_t k = kmax * (canted ? 2 : 1), n = (size_t)n_sites * k;
     for (int b0 = 0; b0 < batch; b0 += 65535) {
         int nb = batch - b0 < 65535 ? batch - b0 : 65535;
-        dim3 grid(n_sites, (n_sites + ASM_WARPS - 1) / ASM_WARPS, nb);
-        size_t k = kmax * (canted ? 2 : 1), n = (size_t)n_sites * k;
-        k_assemble<<<grid, ASM_WARPS * 32, smem, st>>>(tinv + (size_t)b0 * n_sites * (canted ? 2 : 1) * nt,
-                                                       site_pos + (size_t)b0 * n_sites * 3,
-                                                       moment ? moment + (size_t)b0 * n_sites * 3 : nullptr, kappa + b0, coef, idx,
-                                                       lmax, n_sites, canted, M + (size_t)b0 * n * n);
+        dim3 grid(n_sites, nb);
+        k_assemble<<<grid, ASM_THREADS, smem, st>>>(tinv + (size_t)b0 * n_sites * (canted ? 2 : 1) * nt,
+                                                    site_pos + (size_t)b0 * n_sites * 3,
+                                                    moment ? moment + (size_t)b0 * n_sites * 3 : nullptr, kappa + b0, coef, idx, leg,
+                                                    lmax, n_sites, canted, chunk, M + (size_t)b0 * n * n);
         LSMS_LAUNCH_CHECK();
     }
     return 0;

@@ -61,11 +61,11 @@ __device__ __forceinline__ void issue_chunk(const GemmShape& g, const c128* A, c
     if (t == 0) mbar_expect_tx(&full[s], (uint32_t)((kvalid * mvalid + nvalid * kvalid) * sizeof(c128)));
     if (t < KS) {
         if (t < kvalid)      // column k0+t of A: mvalid contiguous elements
-            tma_bulk_g2s(As + t * LDA_S, A + (size_t)(k0 + t) * g.ld, (uint32_t)(mvalid * sizeof(c128)), &full[s]);
+            tma_bulk_g2s(As + t * LDA_S, A + (size_t)(k0 + t) * g.ldA, (uint32_t)(mvalid * sizeof(c128)), &full[s]);
     } else if (t < KS + BN) {
         const int nn = t - KS;
         if (nn < nvalid)     // column n0+nn of B: kvalid contiguous elements
-            tma_bulk_g2s(Bs + nn * LDB_S, B + (size_t)nn * g.ld + k0, (uint32_t)(kvalid * sizeof(c128)), &full[s]);
+            tma_bulk_g2s(Bs + nn * LDB_S, B + (size_t)nn * g.ldB + k0, (uint32_t)(kvalid * sizeof(c128)), &full[s]);
     }
 }
 
@@ -79,10 +79,9 @@ k_schur_gemm(GemmShape g, int tiles_m) {
     const int tm = blockIdx.x % tiles_m, tn = blockIdx.x / tiles_m;
     const int m0 = tm * BM, n0 = tn * BN;
     const int mvalid = min(BM, g.Mr - m0), nvalid = min(BN, g.Nc - n0);
-    c128* item = g.base + (size_t)blockIdx.y * g.batch_stride;
-    const c128* A = item + g.offA + m0;                       // A(m0, 0)
-    const c128* B = item + g.offB + (size_t)n0 * g.ld;        // B(0, n0)
-    c128* C = item + g.offC + m0 + (size_t)n0 * g.ld;         // C(m0, n0)
+    const c128* A = g.A + (size_t)blockIdx.y * g.strideA + m0;                        // A(m0, 0)
+    const c128* B = g.B + (size_t)blockIdx.y * g.strideB + (size_t)n0 * g.ldB;        // B(0, n0)
+    c128* C = g.C + (size_t)blockIdx.y * g.strideC + m0 + (size_t)n0 * g.ldC;         // C(m0, n0)
     const int nchunks = (g.K + KS - 1) / KS;
 
     if (threadIdx.x == 0) {
@@ -104,7 +103,7 @@ k_schur_gemm(GemmShape g, int tiles_m) {
             for (int e = 0; e < 2; ++e) {
                 const int r = wm + mt * 8 + gq, c = wn + nt * 8 + 2 * q + e;
                 c128 v = cmake(0.0, 0.0);
-                if (r < mvalid && c < nvalid) v = C[r + (size_t)c * g.ld];
+                if (!g.beta0 && r < mvalid && c < nvalid) v = C[r + (size_t)c * g.ldC];
                 cr[mt][nt][e] = v.x; ci[mt][nt][e] = v.y;
             }
 
@@ -149,7 +148,7 @@ k_schur_gemm(GemmShape g, int tiles_m) {
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const int r = wm + mt * 8 + gq, c = wn + nt * 8 + 2 * q + e;
-                if (r < mvalid && c < nvalid) C[r + (size_t)c * g.ld] = cmake(cr[mt][nt][e], ci[mt][nt][e]);
+                if (r < mvalid && c < nvalid) C[r + (size_t)c * g.ldC] = cmake(cr[mt][nt][e], ci[mt][nt][e]);
             }
 }
 
@@ -163,7 +162,7 @@ int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
     const int tiles_m = (g.Mr + BM - 1) / BM, tiles_n = (g.Nc + BN - 1) / BN;
     for (int b0 = 0; b0 < g.batch; b0 += 65535) {
         GemmShape h = g;
-        h.base = g.base + (size_t)b0 * g.batch_stride;
+        h.A = g.A + (size_t)b0 * g.strideA; h.B = g.B + (size_t)b0 * g.strideB; h.C = g.C + (size_t)b0 * g.strideC;
         h.batch = g.batch - b0 < 65535 ? g.batch - b0 : 65535;
         dim3 grid((unsigned)(tiles_m * tiles_n), (unsigned)h.batch);
         k_schur_gemm<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(h, tiles_m);

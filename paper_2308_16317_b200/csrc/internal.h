@@ -16,11 +16,11 @@ int launch_assemble(const c128* tinv, const double* site_pos, const double* mome
 
 // gemm.cu -- K4: C[Mr x Nc] -= A[Mr x K] * B[K x Nc] inside the same column-major matrices (ld = n)
 struct GemmShape {
-    c128* base;            // item 0 of the batch
-    size_t batch_stride;   // elements between items
-    int ld;                // leading dimension (= n)
-    int Mr, Nc, K;         // C is Mr x Nc, inner dimension K
-    size_t offA, offB, offC;   // element offsets of A(0,0), B(0,0), C(0,0) inside an item
+    const c128* A; const c128* B; c128* C;   // item 0 of each operand: A is Mr x K, B is K x Nc, C is Mr x Nc (column-major)
+    size_t strideA, strideB, strideC;        // elements between batch items
+    int ldA, ldB, ldC;
+    int Mr, Nc, K;
+    int beta0;                               // 0: C -= A*B ;  1: C = -(A*B)  (C is not read)
     int batch;
 };
 int launch_schur_gemm(const GemmShape& g, cudaStream_t st);
@@ -29,6 +29,10 @@ int launch_schur_gemm(const GemmShape& g, cudaStream_t st);
 int launch_panel(c128* base, size_t stride, int n, int c0, int w, int ne, int batch, int* piv, int* info, cudaStream_t st);
 int launch_swap_trsm(c128* base, size_t stride, int n, int c0, int w, int col_lo, int col_hi, int mode /*1 swap | 2 trsm*/, int batch,
                      const int* piv, cudaStream_t st);
+int launch_panel_post(const c128* base, size_t stride, int n, int J, int W, int batch, const int* piv, int* perm, c128* ninv,
+                      int nbmax, cudaStream_t st);
+int launch_row_permute(c128* base, size_t stride, int n, int J, int W, int col_lo, int col_hi, int batch, const int* perm,
+                       c128* tperm, size_t tperm_stride, int nbmax, cudaStream_t st);
 int launch_final_inverse(c128* base, size_t stride, int n, int k, int batch, c128* tau, int* info, void* ws, cudaStream_t st);
 int launch_backsolve_central(const c128* LU, size_t stride, int n, int k, int batch, const c128* tau, c128* X, cudaStream_t st);
 size_t final_inverse_ws_bytes(int k, int batch);

@@ -11,7 +11,7 @@
 
 namespace lsms {
 
-constexpr int PANEL_THREADS = 1024;
+constexpr int PANEL_THREADS = 256;     // 256 x 128 regs: fits beside one Schur-update CTA (look-ahead)
 constexpr int MAX_IB = 16;
 
 // ---------------------------------------------------------------- K2: panel factorisation
@@ -46,7 +46,7 @@ k_panel(c128* __restrict__ base, size_t stride, int n, int c0, int w, int ne, in
         if (lane == 0) { red_v[warp] = v; red_i[warp] = ix; }
         __syncthreads();
         if (warp == 0) {
-            v = red_v[lane]; ix = red_i[lane];
+            v = (lane < PANEL_THREADS / 32) ? red_v[lane] : -1.0; ix = (lane < PANEL_THREADS / 32) ? red_i[lane] : 0x7fffffff;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 double ov = __shfl_xor_sync(0xffffffffu, v, o); int oi = __shfl_xor_sync(0xffffffffu, ix, o);
@@ -74,15 +74,23 @@ k_panel(c128* __restrict__ base, size_t stride, int n, int c0, int w, int ne, in
         bv = -1.0; bi = 0x7fffffff;
         if (!bad) {
             const c128 rp = crecip(urow[jj]);
+            // all loads of a row are issued before any of its stores (independent L2 round trips in
+            // flight instead of one dependent load->fma->store chain per column)
             for (int i = j + 1 + tid; i < n; i += PANEL_THREADS) {
-                c128 l = cmul(A[i + (size_t)j * n], rp);
+                c128 a[MAX_IB];
+                const c128 l0 = A[i + (size_t)j * n];
+#pragma unroll
+                for (int t = 1; t < MAX_IB; ++t)
+                    if (jj + t < w) a[t] = A[i + (size_t)(j + t) * n];
+                const c128 l = cmul(l0, rp);
                 A[i + (size_t)j * n] = l;
-                for (int t = jj + 1; t < w; ++t) {
-                    c128 a = A[i + (size_t)(c0 + t) * n];
-                    cfms(a, l, urow[t]);
-                    A[i + (size_t)(c0 + t) * n] = a;
-                    if (t == jj + 1 && i < ne) { double vv = cabs1(a); if (vv > bv) { bv = vv; bi = i; } }
-                }
+#pragma unroll
+                for (int t = 1; t < MAX_IB; ++t)
+                    if (jj + t < w) {
+                        cfms(a[t], l, urow[jj + t]);
+                        A[i + (size_t)(j + t) * n] = a[t];
+                    }
+                if (jj + 1 < w && i < ne) { double vv = cabs1(a[1]); if (vv > bv) { bv = vv; bi = i; } }
             }
         } else if (jj + 1 < w) {
             for (int i = j + 1 + tid; i < ne; i += PANEL_THREADS) {
@@ -147,6 +155,128 @@ k_swap_trsm(c128* __restrict__ base, size_t stride, int n, int c0, int w, int co
     }
 #pragma unroll
     for (int i = 0; i < MAX_IB; ++i) if (i < w) col[c0 + i] = x[i];
+}
+
+// ---------------------------------------------------------------- K3a: after an outer panel
+// One CTA per matrix, once the outer panel [J, J+W) is fully factored:
+//  * warp 0 folds the W interchanges (applied in order) into one row permutation:
+//      perm[0] = nd, top_src[i] = row whose content ends in top position J+i,
+//      (down_dst[j], down_top[j]) = row below the top block that receives original top row J+down_top[j];
+//    (a row that enters the top block at step i stays there, so every displaced row is an original top row)
+//  * threads 0..W-1 compute Ninv = -(L11)^{-1} (unit lower W x W), column per thread, in shared memory,
+//    so that U12 = L11^{-1} A12 becomes a GEMM on the DMMA path:  U12 = -(Ninv * A12).
+constexpr int POST_THREADS = 32 + 128;     // warp 0: permutation; threads 32..32+W-1: one column of Ninv each (W <= 128)
+
+__global__ void __launch_bounds__(POST_THREADS)
+k_panel_post(const c128* __restrict__ base, size_t stride, int n, int J, int W, const int* __restrict__ piv,
+             int* __restrict__ perm_all, c128* __restrict__ ninv_all, int nbmax) {
+    extern __shared__ __align__(16) unsigned char post_smem[];
+    c128* X = reinterpret_cast<c128*>(post_smem);                 // [W][W]: X[i*W + j] = element (i,j)
+    int* cur_top = reinterpret_cast<int*>(post_smem + (size_t)W * W * sizeof(c128));
+    int* bpos = cur_top + W;
+    int* bcon = bpos + W;
+    const c128* A = base + (size_t)blockIdx.x * stride;
+    const int* pv = piv + (size_t)blockIdx.x * n + J;
+    int* perm = perm_all + (size_t)blockIdx.x * (4 + 3 * nbmax);
+    c128* ninv = ninv_all + (size_t)blockIdx.x * nbmax * nbmax;
+    const int tid = threadIdx.x;
+
+    for (int e = tid; e < W * W; e += POST_THREADS) X[e] = cmake(0.0, 0.0);
+    for (int i = tid; i < W; i += POST_THREADS) cur_top[i] = J + i;
+    __syncthreads();
+
+    if (tid < 32) {
+        // ---- net permutation (warp 0; the below-list is searched lane-parallel)
+        const int lane = tid;
+        int nb = 0;
+        for (int i = 0; i < W; ++i) {
+            const int p = pv[i];
+            if (p == J + i) continue;
+            if (p < J + W) {
+                if (lane == 0) { int t = cur_top[i]; cur_top[i] = cur_top[p - J]; cur_top[p - J] = t; }
+            } else {
+                int found = -1;
+                for (int b0 = 0; b0 < nb; b0 += 32) {
+                    const int idx = b0 + lane;
+                    const unsigned m = __ballot_sync(0xffffffffu, idx < nb && bpos[idx] == p);
+                    if (m) { found = b0 + __ffs(m) - 1; break; }
+                }
+                if (found < 0) { found = nb; if (lane == 0) { bpos[nb] = p; bcon[nb] = p; } ++nb; }
+                __syncwarp();
+                if (lane == 0) { int t = cur_top[i]; cur_top[i] = bcon[found]; bcon[found] = t; }
+            }
+            __syncwarp();
+        }
+        __syncwarp();
+        int nd = 0;
+        // compact the displaced rows (content differs from position); serial over <= W entries
+        if (lane == 0) {
+            for (int j = 0; j < nb; ++j)
+                if (bcon[j] != bpos[j]) { perm[1 + nbmax + nd] = bpos[j]; perm[1 + 2 * nbmax + nd] = bcon[j] - J; ++nd; }
+            perm[0] = nd;
+        }
+        for (int i = lane; i < W; i += 32) perm[1 + i] = cur_top[i];
+    } else {
+        // ---- Ninv = -(L11^{-1}); thread 32+j owns column j:  x_j = 1, x_i = -sum_{j<=k<i} L_ik x_k
+        const int j = tid - 32;
+        if (j < W) {
+            X[j * W + j] = cmake(1.0, 0.0);
+            for (int i = j + 1; i < W; ++i) {
+                c128 acc = cmake(0.0, 0.0);
+                const c128* Lrow = A + (size_t)(J + i) + (size_t)J * n;       // L(i, k) at Lrow[k*n]
+                for (int k = j; k < i; ++k) cfms(acc, Lrow[(size_t)k * n], X[k * W + j]);
+                X[i * W + j] = acc;
+            }
+        }
+    }
+    __syncthreads();
+    for (int e = tid; e < W * W; e += POST_THREADS) {
+        const int i = e % W, j = e / W;
+        ninv[i + (size_t)j * nbmax] = cneg(X[i * W + j]);
+    }
+}
+
+// ---------------------------------------------------------------- K3b: apply the net row permutation
+// to the trailing columns [col_lo, col_hi): the new top block (rows J..J+W) goes, packed with ld = nbmax,
+// to tperm (the B operand of the TRSM-GEMM that writes U12 back into the matrix); displaced original top
+// rows are scattered to their final rows below.  One CTA per strip of PERM_TN columns.
+constexpr int PERM_TN = 16, PERM_THREADS = 256;
+
+__global__ void __launch_bounds__(PERM_THREADS)
+k_row_permute(c128* __restrict__ base, size_t stride, int n, int J, int W, int col_lo, int col_hi,
+              const int* __restrict__ perm_all, c128* __restrict__ tperm_all, size_t tperm_stride, int nbmax) {
+    extern __shared__ __align__(16) unsigned char perm_smem[];
+    c128* Told = reinterpret_cast<c128*>(perm_smem);               // [PERM_TN][W]
+    int* s_perm = reinterpret_cast<int*>(perm_smem + (size_t)PERM_TN * W * sizeof(c128));   // [1 + 3W]
+    c128* A = base + (size_t)blockIdx.y * stride;
+    const int* perm = perm_all + (size_t)blockIdx.y * (4 + 3 * nbmax);
+    c128* T = tperm_all + (size_t)blockIdx.y * tperm_stride;
+    const int tid = threadIdx.x;
+    const int c_first = col_lo + blockIdx.x * PERM_TN;
+    const int ncol = min(PERM_TN, col_hi - c_first);
+    const int nd = perm[0];
+    if (tid == 0) s_perm[0] = nd;
+    for (int i = tid; i < W; i += PERM_THREADS) {
+        s_perm[1 + i] = perm[1 + i];
+        if (i < nd) { s_perm[1 + W + i] = perm[1 + nbmax + i]; s_perm[1 + 2 * W + i] = perm[1 + 2 * nbmax + i]; }
+    }
+    for (int e = tid; e < ncol * W; e += PERM_THREADS) {
+        const int i = e % W, c = e / W;
+        Told[c * W + i] = A[(size_t)(J + i) + (size_t)(c_first + c) * n];
+    }
+    __syncthreads();
+    // gather the new top block (rows from below are read before any scatter of this CTA's columns)
+    for (int e = tid; e < ncol * W; e += PERM_THREADS) {
+        const int i = e % W, c = e / W;
+        const int src = s_perm[1 + i];
+        c128 v = (src < J + W) ? Told[c * W + (src - J)] : A[(size_t)src + (size_t)(c_first + c) * n];
+        T[(size_t)i + (size_t)(c_first + c) * nbmax] = v;
+    }
+    __syncthreads();
+    for (int e = tid; e < ncol * nd; e += PERM_THREADS) {
+        const int j = e % nd, c = e / nd;
+        A[(size_t)s_perm[1 + W + j] + (size_t)(c_first + c) * n] = Told[c * W + s_perm[1 + 2 * W + j]];
+    }
 }
 
 // ---------------------------------------------------------------- K5: tau00 = S^{-1}
@@ -275,6 +405,32 @@ int launch_swap_trsm(c128* base, size_t stride, int n, int c0, int w, int col_lo
         int nb = batch - b0 < 65535 ? batch - b0 : 65535;
         dim3 grid((col_hi - col_lo + K3_THREADS - 1) / K3_THREADS, nb);
         k_swap_trsm<<<grid, K3_THREADS, 0, st>>>(base + (size_t)b0 * stride, stride, n, c0, w, col_lo, col_hi, mode, piv + (size_t)b0 * n);
+        LSMS_LAUNCH_CHECK();
+    }
+    return 0;
+}
+
+int launch_panel_post(const c128* base, size_t stride, int n, int J, int W, int batch, const int* piv, int* perm, c128* ninv,
+                      int nbmax, cudaStream_t st) {
+    size_t smem = (size_t)W * W * sizeof(c128) + 3 * (size_t)W * sizeof(int);
+    static size_t attr = 0;
+    if (smem > attr) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_panel_post, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
+    k_panel_post<<<batch, POST_THREADS, smem, st>>>(base, stride, n, J, W, piv, perm, ninv, nbmax);
+    LSMS_LAUNCH_CHECK();
+    return 0;
+}
+
+int launch_row_permute(c128* base, size_t stride, int n, int J, int W, int col_lo, int col_hi, int batch, const int* perm,
+                       c128* tperm, size_t tperm_stride, int nbmax, cudaStream_t st) {
+    if (col_hi <= col_lo) return 0;
+    size_t smem = (size_t)PERM_TN * W * sizeof(c128) + (1 + 3 * (size_t)W) * sizeof(int);
+    static size_t attr = 0;
+    if (smem > attr && smem > 48 * 1024) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_row_permute, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
+    for (int b0 = 0; b0 < batch; b0 += 65535) {
+        int nb = batch - b0 < 65535 ? batch - b0 : 65535;
+        dim3 grid((col_hi - col_lo + PERM_TN - 1) / PERM_TN, nb);
+        k_row_permute<<<grid, PERM_THREADS, smem, st>>>(base + (size_t)b0 * stride, stride, n, J, W, col_lo, col_hi,
+                                                       perm + (size_t)b0 * (4 + 3 * nbmax), tperm + (size_t)b0 * tperm_stride, tperm_stride, nbmax);
         LSMS_LAUNCH_CHECK();
     }
     return 0;

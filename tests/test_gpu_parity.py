@@ -247,13 +247,27 @@ def test_blocking_parameters_do_not_change_the_result(lt):
     batch = sl.make_batch("T").select([0, 9])
     ref, _ = oracle.tau00_batched(batch, "long double")
     try:
-        for nb, ib in ((16, 4), (32, 16), (48, 12), (128, 16), (64, 7)):
+        for nb, ib in ((16, 4), (32, 16), (48, 12), (96, 16), (64, 7)):
             lt.lsms_set_blocking(nb, ib)
             tau, info, _ = lt.tau00_from_liz_batch(batch)
             assert not info.any()
             assert max(relF(tau[b], ref[b]) for b in range(2)) < 1e-12
     finally:
         lt.lsms_set_blocking(0, 0)
+
+
+def test_lookahead_on_and_off_give_identical_results(lt):
+    """The look-ahead split of the Schur update only re-orders independent tiles: bitwise equal tau00."""
+    batch = sl.make_batch("M").select([3, 300])
+    try:
+        lt.lsms_set_lookahead(False)
+        tau0, info0, _ = lt.tau00_from_liz_batch(batch)
+        lt.lsms_set_lookahead(True)
+        tau1, info1, _ = lt.tau00_from_liz_batch(batch)
+    finally:
+        lt.lsms_set_lookahead(True)
+    assert not info0.any() and not info1.any()
+    assert np.array_equal(tau0, tau1)
 
 
 def test_schur_update_alone_matches_numpy(lt):
