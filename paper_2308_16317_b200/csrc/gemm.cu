@@ -113,10 +113,28 @@ k_schur_gemm(GemmShape g, int tiles_m) {
         const int kvalid = min(KS, g.K - kc * KS);
         const c128* As = ring + (size_t)s * STAGE_ELEMS;
         const c128* Bs = As + A_STAGE;
-        const int nsteps = (kvalid + 3) >> 2;
+        const int nfull = kvalid >> 2;
 #pragma unroll 1
-        for (int ks = 0; ks < nsteps; ++ks) {
+        for (int ks = 0; ks < nfull; ++ks) {
             const int k0 = ks * 4;
+            c128 a[4], b[2];
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) a[mt] = As[(k0 + q) * LDA_S + wm + mt * 8 + gq];
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) b[nt] = Bs[(wn + nt * 8 + gq) * LDB_S + k0 + q];
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) {
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    dmma884(cr[mt][nt][0], cr[mt][nt][1], a[mt].x, -b[nt].x);
+                    dmma884(ci[mt][nt][0], ci[mt][nt][1], a[mt].x, -b[nt].y);
+                    dmma884(cr[mt][nt][0], cr[mt][nt][1], a[mt].y, b[nt].y);
+                    dmma884(ci[mt][nt][0], ci[mt][nt][1], a[mt].y, -b[nt].x);
+                }
+            }
+        }
+        if (kvalid & 3) {                      // ragged K tail: fragments beyond kvalid are zeroed
+            const int k0 = nfull * 4;
             const bool live = (k0 + q) < kvalid;
             c128 a[4], b[2];
 #pragma unroll

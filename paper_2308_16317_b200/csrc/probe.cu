@@ -12,12 +12,14 @@ __global__ void __launch_bounds__(256) k_probe_dmma(int iters, double* out) {
     double c0[PROBE_ACC], c1[PROBE_ACC];
 #pragma unroll
     for (int i = 0; i < PROBE_ACC; ++i) { c0[i] = threadIdx.x * 1e-9; c1[i] = i * 1e-9; }
-    double a = 1.0 + threadIdx.x * 1e-12, b = 1.0 - threadIdx.x * 1e-12;
+    double a[PROBE_ACC], b[PROBE_ACC];       // distinct operand registers per accumulator
+#pragma unroll
+    for (int i = 0; i < PROBE_ACC; ++i) { a[i] = 1.0 + (threadIdx.x + i) * 1e-12; b[i] = 1.0 - (threadIdx.x + 3 * i) * 1e-12; }
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int i = 0; i < PROBE_ACC; ++i)
             asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                         : "+d"(c0[i]), "+d"(c1[i]) : "d"(a), "d"(b));
+                         : "+d"(c0[i]), "+d"(c1[i]) : "d"(a[i]), "d"(b[i]));
     }
     double s = 0.0;
 #pragma unroll
@@ -48,7 +50,7 @@ int run_peak_probe(int which, int iters, double* tflops, cudaStream_t st) {
     LSMS_CUDA_OK(cudaMalloc(&dummy, 8));
     cudaEvent_t e0, e1;
     LSMS_CUDA_OK(cudaEventCreate(&e0)); LSMS_CUDA_OK(cudaEventCreate(&e1));
-    const int ctas = sms * 4, thr = 256;
+    const int ctas = sms * 2, thr = 256;      // 16 warps per SM: enough to saturate the DMMA pipe
     for (int rep = 0; rep < 2; ++rep) {      // first pass warms up
         LSMS_CUDA_OK(cudaEventRecord(e0, st));
         if (which == 0) k_probe_dmma<<<ctas, thr, 0, st>>>(iters, dummy);
