@@ -152,6 +152,9 @@ def main() -> None:
     ap.add_argument("--nb", type=int, default=0, help="outer panel width override (0 = library default)")
     ap.add_argument("--ib", type=int, default=0, help="inner panel width override")
     ap.add_argument("--no-lookahead", action="store_true", help="factor the next panel in front of, not under, the update")
+    ap.add_argument("--panel", type=int, default=0, help="K2 variant: 0 register-blocked 256 thr, 1 512 thr, -1 L2-resident")
+    ap.add_argument("--no-align", action="store_true", help="every outer panel NB wide (no tile-aligning first panel)")
+    ap.add_argument("--groups", type=int, default=0, help="batch groups on separate streams (0 = library default)")
     args = ap.parse_args()
     cfg = sl.CONFIGS[args.workload]
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -178,6 +181,9 @@ def main() -> None:
     if args.nb or args.ib:
         lt.lsms_set_blocking(args.nb, args.ib)
     lt.lsms_set_lookahead(not args.no_lookahead)
+    lt.lsms_set_groups(args.groups)
+    lt.lsms_set_panel_variant(args.panel)
+    lt.lsms_set_align_first(not args.no_align)
 
     # ---- inputs: every rank gets its own central atoms (weak scaling: per-GPU work fixed)
     batch = sl.make_batch(cfg, atom_offset=rank * cfg.n_atoms)

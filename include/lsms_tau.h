@@ -125,9 +125,26 @@ int lsms_set_blocking(int nb_outer, int ib_inner);
 
 /* Look-ahead (default on): the next panel is factored on a library-owned high-priority stream while the
  * caller's stream runs the Schur update of the remaining columns; the two are joined with events before
- * the call returns to the next panel, so the caller still sees one ordered stream.  The auxiliary stream
- * and two events are created on first use and are the library's only persistent objects. */
+ * the call returns to the next panel, so the caller still sees one ordered stream.  The auxiliary streams
+ * and their events are created on first use and are the library's only persistent objects. */
 int lsms_set_lookahead(int on);
+
+/* Batch groups (default 0 = chosen per shape): the batch is cut into `groups` (<= 8) contiguous groups that
+ * run the elimination on separate library-owned streams, forked from and joined back into the caller's
+ * stream inside lsms_tau00_batched, so that the poorly parallel phases of one group (net permutation,
+ * triangular solve, look-ahead slice, last panels) run under another group's Schur updates.  Results do
+ * not depend on the setting (every item is eliminated independently).  Errors: -1 groups out of range. */
+int lsms_set_groups(int groups);
+
+/* Panel kernel (K2) variant: 0 (default) register-blocked sub-panels, 256 threads (half an SM, co-resident
+ * with a Schur-update CTA under look-ahead); 1 register-blocked, 512 threads for tall panels; -1 the
+ * L2-resident column-at-a-time kernel.  All variants pick the same pivots (|re|+|im|, ties to the lowest
+ * row) and perform the same arithmetic per element.  Errors: -1 out of range. */
+int lsms_set_panel_variant(int variant);
+
+/* Tile alignment (default on): the first outer panel is n mod 64 columns wide, so that all later trailing
+ * matrices are whole multiples of the 64 x 64 Schur-update tile.  Off: every panel is NB wide. */
+int lsms_set_align_first(int on);
 
 /* How many kernels the last lsms_tau00_batched / lsms_build_M_batched call on this thread enqueued. */
 int lsms_last_launch_count(void);

@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "lsms_version", "lsms_workspace_bytes", "lsms_solve_workspace_bytes", "lsms_host_call_scratch_bytes",
     "lsms_tinv_from_phase_shifts", "lsms_build_M_batched", "lsms_tau00_batched",
-    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_set_blocking", "lsms_set_lookahead",
+    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_set_blocking", "lsms_set_lookahead", "lsms_set_groups", "lsms_set_panel_variant", "lsms_set_align_first",
     "lsms_last_launch_count", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe", "lsms_schur_update_batched",
     "lsms_debug_gaunt_closed_form",
 )
@@ -97,6 +97,18 @@ def lsms_set_blocking(nb_outer: int = 0, ib_inner: int = 0) -> None:
 
 def lsms_set_lookahead(on: bool = True) -> None:
     _check(lib().lsms_set_lookahead(int(bool(on))), "lsms_set_lookahead")
+
+
+def lsms_set_panel_variant(variant: int = 0) -> None:
+    _check(lib().lsms_set_panel_variant(int(variant)), "lsms_set_panel_variant")
+
+
+def lsms_set_align_first(on: bool = True) -> None:
+    _check(lib().lsms_set_align_first(int(bool(on))), "lsms_set_align_first")
+
+
+def lsms_set_groups(groups: int = 0) -> None:
+    _check(lib().lsms_set_groups(int(groups)), "lsms_set_groups")
 
 
 def lsms_last_launch_count() -> int:

@@ -82,16 +82,29 @@ static size_t tau_ws_bytes(int n, int k, int batch) { return tau_ws_layout(nullp
 // The two streams touch disjoint columns (the panel's interchanges reach the trailing columns only in K3b,
 // after the join).  The auxiliary stream and two events are the library's only persistent objects.
 static int g_lookahead = 1;
-static cudaStream_t g_aux = nullptr;
-static cudaEvent_t g_ev_fork = nullptr, g_ev_join = nullptr;
+static int g_groups = 0;                  // 0 = chosen per shape
+static int g_align_first = 1;              // first panel n mod 64 wide (tile-aligned trailing matrices)
+static int g_panel_variant = 0;           // -1 L2-resident k_panel, 0 register-blocked half-SM, 1 register-blocked full-SM
+constexpr int MAX_GROUPS = 8;
+// Stream set of one batch group (see eliminate_groups): group 0 runs on the caller's stream, the others on
+// library-owned streams; every group has a high-priority auxiliary stream for the look-ahead panel.
+struct GroupStreams { cudaStream_t main = nullptr, aux = nullptr; cudaEvent_t fork = nullptr, join = nullptr, done = nullptr; };
+static GroupStreams g_gs[MAX_GROUPS];
+static cudaEvent_t g_ev_start = nullptr;
 
-static int ensure_aux() {
-    if (g_aux) return 0;
+static int ensure_streams(int groups) {
     int lo = 0, hi = 0;
     LSMS_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
-    LSMS_CUDA_OK(cudaStreamCreateWithPriority(&g_aux, cudaStreamNonBlocking, hi));
-    LSMS_CUDA_OK(cudaEventCreateWithFlags(&g_ev_fork, cudaEventDisableTiming));
-    LSMS_CUDA_OK(cudaEventCreateWithFlags(&g_ev_join, cudaEventDisableTiming));
+    if (!g_ev_start) LSMS_CUDA_OK(cudaEventCreateWithFlags(&g_ev_start, cudaEventDisableTiming));
+    for (int g = 0; g < groups; ++g) {
+        GroupStreams& s = g_gs[g];
+        if (s.aux) continue;
+        if (g > 0) LSMS_CUDA_OK(cudaStreamCreateWithFlags(&s.main, cudaStreamNonBlocking));
+        LSMS_CUDA_OK(cudaStreamCreateWithPriority(&s.aux, cudaStreamNonBlocking, hi));
+        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming));
+        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming));
+        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+    }
     return 0;
 }
 
@@ -102,9 +115,16 @@ static int factor_panel(c128* M, int n, int batch, int J, int W, int ne, int IB,
     GemmShape g; g.strideA = g.strideB = g.strideC = stride; g.ldA = g.ldB = g.ldC = n; g.batch = batch; g.beta0 = 0;
     for (int jj = 0; jj < W; jj += IB) {
         const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
-        int rc; { ProfScope ps(1, st); rc = launch_panel(M, stride, n, c0, w, ne, batch, piv, info, st); } if (rc) return rc;
-        { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, J, c0, 1, batch, piv, st); } if (rc) return rc;
-        { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, c0 + w, Jend, 3, batch, piv, st); } if (rc) return rc;
+        int rc;
+        if (g_panel_variant >= 0 && n - c0 <= 16384) {
+            // register-blocked K2: factors the inner panel and applies its interchanges to the whole outer panel
+            { ProfScope ps(1, st); rc = launch_panel_reg(M, stride, n, J, W, c0, w, ne, batch, piv, info, g_panel_variant, st); } if (rc) return rc;
+            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, c0 + w, Jend, 2, batch, piv, st); } if (rc) return rc;
+        } else {
+            { ProfScope ps(1, st); rc = launch_panel(M, stride, n, c0, w, ne, batch, piv, info, st); } if (rc) return rc;
+            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, J, c0, 1, batch, piv, st); } if (rc) return rc;
+            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, c0 + w, Jend, 3, batch, piv, st); } if (rc) return rc;
+        }
         const int rem = Jend - (c0 + w);
         if (rem > 0) {
             g.Mr = n - (c0 + w); g.Nc = rem; g.K = w;
@@ -130,19 +150,23 @@ static int schur_update(c128* M, int n, int batch, int J, int W, int c_lo, int c
     return launch_schur_gemm(g, st);
 }
 
-static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* info, cudaStream_t st) {
+// one batch group [0, batch) of items (pointers already offset to the group's first item)
+static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* info, cudaStream_t st, const GroupStreams& gs) {
     const int ne = n - k;
     const int NB = eff_nb(), IB = eff_ib();
     const size_t stride = (size_t)n * n;
     int* piv = ws.piv;
     const bool la = g_lookahead != 0;
-    if (la) { int rc = ensure_aux(); if (rc) return rc; }
     if (ne <= 0) return 0;
-    int rc = factor_panel(M, n, batch, 0, ne < NB ? ne : NB, ne, IB, piv, info, st); if (rc) return rc;
-    for (int J = 0; J < ne; J += NB) {
-        const int W = (ne - J < NB) ? ne - J : NB;
+    // Tile alignment: the first panel is n mod 64 wide (when that is non-zero), so that every trailing matrix
+    // the Schur update sees has a multiple of the 64 x 64 DMMA tile in both dimensions; only the last,
+    // smallest updates carry a ragged tile (n = 2160: 34 x 34 tiles of which one row and column 3/4 full -> 33 x 33 full).
+    int W0 = ne < NB ? ne : NB;
+    if (g_align_first && NB % 64 == 0 && n % 64 != 0 && n % 64 < W0) W0 = n % 64;
+    int rc = factor_panel(M, n, batch, 0, W0, ne, IB, piv, info, st); if (rc) return rc;
+    { ProfScope ps(6, st); rc = launch_panel_post(M, stride, n, 0, W0, batch, piv, ws.perm, ws.ninv, NB, st); } if (rc) return rc;
+    for (int J = 0, W = W0; J < ne; J += W, W = (ne - J < NB) ? ne - J : NB) {
         const int Jend = J + W;                               // Jend <= ne < n
-        { ProfScope ps(6, st); rc = launch_panel_post(M, stride, n, J, W, batch, piv, ws.perm, ws.ninv, NB, st); } if (rc) return rc;
         { ProfScope ps(6, st); rc = launch_row_permute(M, stride, n, J, W, Jend, n, batch, ws.perm, ws.tperm, (size_t)NB * n, NB, st); } if (rc) return rc;
         GemmShape t; t.batch = batch; t.beta0 = 1;
         t.A = ws.ninv; t.strideA = (size_t)NB * NB; t.ldA = NB;
@@ -153,16 +177,67 @@ static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* inf
         const int W2 = (Jend < ne) ? ((ne - Jend < NB) ? ne - Jend : NB) : 0;     // width of the next panel
         if (W2 > 0 && la) {
             rc = schur_update(M, n, batch, J, W, Jend, Jend + W2, st); if (rc) return rc;
-            LSMS_CUDA_OK(cudaEventRecord(g_ev_fork, st));
-            LSMS_CUDA_OK(cudaStreamWaitEvent(g_aux, g_ev_fork, 0));
-            rc = factor_panel(M, n, batch, Jend, W2, ne, IB, piv, info, g_aux); if (rc) return rc;
-            LSMS_CUDA_OK(cudaEventRecord(g_ev_join, g_aux));
+            LSMS_CUDA_OK(cudaEventRecord(gs.fork, st));
+            LSMS_CUDA_OK(cudaStreamWaitEvent(gs.aux, gs.fork, 0));
+            rc = factor_panel(M, n, batch, Jend, W2, ne, IB, piv, info, gs.aux); if (rc) return rc;
+            // the next panel's net permutation and -(L11^-1) are also built under the update: perm/Ninv of
+            // panel J were last read by the permutation / triangular solve above, before the fork
+            { ProfScope ps(6, gs.aux); rc = launch_panel_post(M, stride, n, Jend, W2, batch, piv, ws.perm, ws.ninv, NB, gs.aux); } if (rc) return rc;
+            LSMS_CUDA_OK(cudaEventRecord(gs.join, gs.aux));
             rc = schur_update(M, n, batch, J, W, Jend + W2, n, st); if (rc) return rc;
-            LSMS_CUDA_OK(cudaStreamWaitEvent(st, g_ev_join, 0));
+            LSMS_CUDA_OK(cudaStreamWaitEvent(st, gs.join, 0));
         } else {
             rc = schur_update(M, n, batch, J, W, Jend, n, st); if (rc) return rc;
-            if (W2 > 0) { rc = factor_panel(M, n, batch, Jend, W2, ne, IB, piv, info, st); if (rc) return rc; }
+            if (W2 > 0) {
+                rc = factor_panel(M, n, batch, Jend, W2, ne, IB, piv, info, st); if (rc) return rc;
+                { ProfScope ps(6, st); rc = launch_panel_post(M, stride, n, Jend, W2, batch, piv, ws.perm, ws.ninv, NB, st); } if (rc) return rc;
+            }
         }
+    }
+    return 0;
+}
+
+// Batch groups (the batch scheduler's second level).  In lock-step over the whole batch
+// the poorly parallel phases of every item (net permutation, triangular solve, the narrow look-ahead slice,
+// the last small panels) coincide and leave the chip idle.  The batch is therefore cut into `groups`
+// contiguous groups that run the same elimination on separate streams: while one group is in such a phase
+// the hardware scheduler fills the SMs with another group's Schur-update tiles.  The groups touch disjoint
+// items; the caller's stream is forked into the group streams and joined again before the call returns.
+static int pick_groups(int n, int batch) {
+    int g = g_groups;
+    if (g <= 0) g = (batch >= 64) ? 4 : (batch >= 16 ? 2 : 1);
+    if (g > MAX_GROUPS) g = MAX_GROUPS;
+    if (g > batch) g = batch;
+    (void)n;
+    return g;
+}
+
+static int eliminate_groups(c128* M, int n, int k, int batch, const TauWs& ws, c128* tau, int* info, cudaStream_t st) {
+    const int NB = eff_nb();
+    const int groups = pick_groups(n, batch);
+    int rc = ensure_streams(groups); if (rc) return rc;
+    const size_t stride = (size_t)n * n;
+    if (groups > 1) LSMS_CUDA_OK(cudaEventRecord(g_ev_start, st));
+    for (int g = 0; g < groups; ++g) {
+        const int b0 = (int)((long long)batch * g / groups), b1 = (int)((long long)batch * (g + 1) / groups);
+        if (b1 <= b0) continue;
+        cudaStream_t gst = (g == 0) ? st : g_gs[g].main;
+        if (g > 0) LSMS_CUDA_OK(cudaStreamWaitEvent(gst, g_ev_start, 0));
+        TauWs w = ws;
+        w.piv = ws.piv + (size_t)b0 * n;
+        w.perm = ws.perm + (size_t)b0 * (4 + 3 * NB);
+        w.ninv = ws.ninv + (size_t)b0 * NB * NB;
+        w.tperm = ws.tperm + (size_t)b0 * NB * n;
+        w.k5 = (char*)ws.k5 + (final_inverse_ws_bytes(k, 1) ? (size_t)b0 * k * k * sizeof(c128) : 0);
+        rc = eliminate(M + (size_t)b0 * stride, n, k, b1 - b0, w, info + b0, gst, g_gs[g]); if (rc) return rc;
+        { ProfScope ps(5, gst);
+          rc = launch_final_inverse(M + (size_t)b0 * stride, stride, n, k, b1 - b0, tau + (size_t)b0 * k * k, info + b0, w.k5, gst); }
+        if (rc) return rc;
+        if (g > 0) LSMS_CUDA_OK(cudaEventRecord(g_gs[g].done, gst));
+    }
+    for (int g = 1; g < groups; ++g) {
+        const int b0 = (int)((long long)batch * g / groups), b1 = (int)((long long)batch * (g + 1) / groups);
+        if (b1 > b0) LSMS_CUDA_OK(cudaStreamWaitEvent(st, g_gs[g].done, 0));
     }
     return 0;
 }
@@ -244,12 +319,8 @@ int lsms_tau00_batched(lsms_c128* M, int n_sites, int kmax, int spin_canted, int
     cudaStream_t st = (cudaStream_t)cuda_stream;
     g_launches.n = 0;
     const TauWs ws = tau_ws_layout(workspace, n, k, batch);
-    void* k5ws = ws.k5;
     LSMS_CUDA_OK(cudaMemsetAsync(info, 0, (size_t)batch * sizeof(int), st));
-    int rc = eliminate((c128*)M, n, k, batch, ws, info, st);
-    if (rc) return rc;
-    ProfScope ps(5, st);
-    return launch_final_inverse((c128*)M, (size_t)n * n, n, k, batch, (c128*)tau00_out, info, k5ws, st);
+    return eliminate_groups((c128*)M, n, k, batch, ws, (c128*)tau00_out, info, st);
 }
 
 int lsms_solve_central_column_batched(const lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
@@ -360,6 +431,20 @@ int lsms_set_blocking(int nb_outer, int ib_inner) {
 }
 
 int lsms_set_lookahead(int on) { g_lookahead = on ? 1 : 0; return 0; }
+
+int lsms_set_align_first(int on) { g_align_first = on ? 1 : 0; return 0; }
+
+int lsms_set_panel_variant(int variant) {
+    if (variant < -1 || variant > 1) return -1;
+    g_panel_variant = variant;
+    return 0;
+}
+
+int lsms_set_groups(int groups) {
+    if (groups < 0 || groups > MAX_GROUPS) return -1;
+    g_groups = groups;
+    return 0;
+}
 
 int lsms_last_launch_count(void) { return g_launches.n; }
 

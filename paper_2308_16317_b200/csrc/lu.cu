@@ -163,16 +163,19 @@ k_swap_trsm(c128* __restrict__ base, size_t stride, int n, int c0, int w, int co
 //      perm[0] = nd, top_src[i] = row whose content ends in top position J+i,
 //      (down_dst[j], down_top[j]) = row below the top block that receives original top row J+down_top[j];
 //    (a row that enters the top block at step i stays there, so every displaced row is an original top row)
-//  * threads 0..W-1 compute Ninv = -(L11)^{-1} (unit lower W x W), column per thread, in shared memory,
-//    so that U12 = L11^{-1} A12 becomes a GEMM on the DMMA path:  U12 = -(Ninv * A12).
-constexpr int POST_THREADS = 32 + 128;     // warp 0: permutation; threads 32..32+W-1: one column of Ninv each (W <= 128)
+//  * the other warps stage L11 (unit lower W x W) in shared memory; then the whole CTA inverts it by 16 x 16
+//    blocks (diagonal blocks by forward substitution, block rows X_{ij} = -D_i^{-1} sum_k L_{ik} X_{kj} in place)
+//    and stores Ninv = -(L11)^{-1}, so that U12 = L11^{-1} A12 becomes a GEMM on the DMMA path: U12 = -(Ninv * A12).
+constexpr int POST_THREADS = 256;
 
 __global__ void __launch_bounds__(POST_THREADS)
 k_panel_post(const c128* __restrict__ base, size_t stride, int n, int J, int W, const int* __restrict__ piv,
              int* __restrict__ perm_all, c128* __restrict__ ninv_all, int nbmax) {
     extern __shared__ __align__(16) unsigned char post_smem[];
-    c128* X = reinterpret_cast<c128*>(post_smem);                 // [W][W]: X[i*W + j] = element (i,j)
-    int* cur_top = reinterpret_cast<int*>(post_smem + (size_t)W * W * sizeof(c128));
+    const int nb16 = (W + 15) / 16, Wp = nb16 * 16;
+    c128* X = reinterpret_cast<c128*>(post_smem);                 // [Wp][Wp] column-major: L11 (padded with I), then L11^{-1} in place
+    c128* T = X + (size_t)Wp * Wp;                                // [16][Wp]   scratch block row
+    int* cur_top = reinterpret_cast<int*>(T + (size_t)16 * Wp);
     int* bpos = cur_top + W;
     int* bcon = bpos + W;
     const c128* A = base + (size_t)blockIdx.x * stride;
@@ -181,13 +184,11 @@ k_panel_post(const c128* __restrict__ base, size_t stride, int n, int J, int W, 
     c128* ninv = ninv_all + (size_t)blockIdx.x * nbmax * nbmax;
     const int tid = threadIdx.x;
 
-    for (int e = tid; e < W * W; e += POST_THREADS) X[e] = cmake(0.0, 0.0);
-    for (int i = tid; i < W; i += POST_THREADS) cur_top[i] = J + i;
-    __syncthreads();
-
     if (tid < 32) {
         // ---- net permutation (warp 0; the below-list is searched lane-parallel)
         const int lane = tid;
+        for (int i = lane; i < W; i += 32) cur_top[i] = J + i;
+        __syncwarp();
         int nb = 0;
         for (int i = 0; i < W; ++i) {
             const int p = pv[i];
@@ -208,31 +209,69 @@ k_panel_post(const c128* __restrict__ base, size_t stride, int n, int J, int W, 
             __syncwarp();
         }
         __syncwarp();
-        int nd = 0;
         // compact the displaced rows (content differs from position); serial over <= W entries
         if (lane == 0) {
+            int nd = 0;
             for (int j = 0; j < nb; ++j)
                 if (bcon[j] != bpos[j]) { perm[1 + nbmax + nd] = bpos[j]; perm[1 + 2 * nbmax + nd] = bcon[j] - J; ++nd; }
             perm[0] = nd;
         }
         for (int i = lane; i < W; i += 32) perm[1 + i] = cur_top[i];
     } else {
-        // ---- Ninv = -(L11^{-1}); thread 32+j owns column j:  x_j = 1, x_i = -sum_{j<=k<i} L_ik x_k
-        const int j = tid - 32;
-        if (j < W) {
-            X[j * W + j] = cmake(1.0, 0.0);
-            for (int i = j + 1; i < W; ++i) {
-                c128 acc = cmake(0.0, 0.0);
-                const c128* Lrow = A + (size_t)(J + i) + (size_t)J * n;       // L(i, k) at Lrow[k*n]
-                for (int k = j; k < i; ++k) cfms(acc, Lrow[(size_t)k * n], X[k * W + j]);
-                X[i * W + j] = acc;
-            }
+        // ---- L11 -> shared memory (strictly lower part; unit diagonal; identity padding up to Wp)
+        for (int e = tid - 32; e < Wp * Wp; e += POST_THREADS - 32) {
+            const int i = e % Wp, j = e / Wp;
+            c128 v = cmake(i == j ? 1.0 : 0.0, 0.0);
+            if (i > j && i < W) v = A[(size_t)(J + i) + (size_t)(J + j) * n];
+            X[i + j * Wp] = v;
         }
     }
     __syncthreads();
+    // ---- diagonal 16 x 16 blocks: D^{-1} in place, one thread per column (unit lower: x_jj = 1)
+    {
+        const int b0 = (tid / 16) * 16, j = tid % 16;
+        c128 x[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = cmake(i == j ? 1.0 : 0.0, 0.0);
+        if (tid < Wp) {
+#pragma unroll
+            for (int i = 1; i < 16; ++i) {
+                if (i > j) {
+                    c128 acc = cmake(0.0, 0.0);
+#pragma unroll
+                    for (int k = 0; k < i; ++k) if (k >= j) cfms(acc, X[(b0 + i) + (b0 + k) * Wp], x[k]);
+                    x[i] = acc;
+                }
+            }
+        }
+        __syncthreads();       // every read of a diagonal block precedes the writes below
+        if (tid < Wp) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) if (i > j) X[(b0 + i) + (b0 + j) * Wp] = x[i];
+        }
+    }
+    __syncthreads();
+    // ---- block rows: X_{bi,bj} = -D_bi^{-1} * sum_{bk = bj}^{bi-1} L_{bi,bk} X_{bk,bj}, written over L_{bi,bj}
+    for (int bi = 1; bi < nb16; ++bi) {
+        const int ncol = bi * 16;
+        for (int e = tid; e < 16 * ncol; e += POST_THREADS) {
+            const int i = e % 16, j = e / 16, bj = j / 16;
+            c128 acc = cmake(0.0, 0.0);
+            for (int k = bj * 16; k < ncol; ++k) cfma(acc, X[(bi * 16 + i) + k * Wp], X[k + j * Wp]);
+            T[i + j * 16] = acc;
+        }
+        __syncthreads();
+        for (int e = tid; e < 16 * ncol; e += POST_THREADS) {
+            const int i = e % 16, j = e / 16;
+            c128 acc = cmake(0.0, 0.0);
+            for (int k = 0; k <= i; ++k) cfms(acc, X[(bi * 16 + i) + (bi * 16 + k) * Wp], T[k + j * 16]);
+            X[(bi * 16 + i) + j * Wp] = acc;       // block row bi of L is dead: only T and D_bi^{-1} are read in this phase
+        }
+        __syncthreads();
+    }
     for (int e = tid; e < W * W; e += POST_THREADS) {
         const int i = e % W, j = e / W;
-        ninv[i + (size_t)j * nbmax] = cneg(X[i * W + j]);
+        ninv[i + (size_t)j * nbmax] = (i >= j) ? cneg(X[i + j * Wp]) : cmake(0.0, 0.0);
     }
 }
 
@@ -412,9 +451,10 @@ int launch_swap_trsm(c128* base, size_t stride, int n, int c0, int w, int col_lo
 
 int launch_panel_post(const c128* base, size_t stride, int n, int J, int W, int batch, const int* piv, int* perm, c128* ninv,
                       int nbmax, cudaStream_t st) {
-    size_t smem = (size_t)W * W * sizeof(c128) + 3 * (size_t)W * sizeof(int);
+    const size_t Wp = (size_t)(W + 15) / 16 * 16;
+    size_t smem = (Wp * Wp + 16 * Wp) * sizeof(c128) + 3 * (size_t)W * sizeof(int);
     static size_t attr = 0;
-    if (smem > attr) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_panel_post, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
+    if (smem > attr && smem > 48 * 1024) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_panel_post, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     k_panel_post<<<batch, POST_THREADS, smem, st>>>(base, stride, n, J, W, piv, perm, ninv, nbmax);
     LSMS_LAUNCH_CHECK();
     return 0;

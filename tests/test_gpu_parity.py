@@ -270,6 +270,59 @@ def test_lookahead_on_and_off_give_identical_results(lt):
     assert np.array_equal(tau0, tau1)
 
 
+@pytest.mark.parametrize("variant", [-1, 0, 1])
+def test_panel_kernel_variants_match_oracle(lt, variant):
+    """Every K2 variant (L2-resident columns, register-blocked sub-panels with 256 / 512 threads) against the
+    oracle on a tiny LIZ, a ragged random matrix (w and sub-panel tails) and a mid LIZ (several row chunks)."""
+    try:
+        lt.lsms_set_panel_variant(variant)
+        batch = sl.make_batch("T").select([0, 17, 31])
+        ref, _ = oracle.tau00_batched(batch, "long double")
+        tau, info, _ = lt.tau00_from_liz_batch(batch)
+        assert not info.any()
+        assert max(relF(tau[b], ref[b]) for b in range(3)) < 1e-12
+        for n_sites, kmax in ((23, 9), (41, 4), (150, 9)):
+            n = n_sites * kmax
+            A = sl.random_dense_matrices(2, n, seed=700 + n)             # column-major storage: [b, col, row]
+            tau, info = lt.lsms_tau00_batched(torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
+            torch.cuda.synchronize()
+            assert not info.cpu().numpy().any()
+            tau = tau.cpu().numpy().transpose(0, 2, 1)
+            for b in range(2):
+                assert relF(tau[b], np.linalg.inv(A[b].T)[n - kmax:, n - kmax:]) < 1e-10
+        mid = sl.make_batch("M").select([5, 400])
+        refm, _ = oracle.tau00_batched(mid, "long double")
+        taum, infom, _ = lt.tau00_from_liz_batch(mid)
+        assert not infom.any()
+        assert max(relF(taum[b], refm[b]) for b in range(2)) < 1e-10
+    finally:
+        lt.lsms_set_panel_variant(0)
+
+
+def test_batch_groups_give_identical_results(lt):
+    """Batch groups run the same per-item elimination on separate streams: bitwise equal tau00 for every
+    group count, including counts that do not divide the batch and exceed it."""
+    batch = sl.make_batch("T").select(list(range(11)))
+    ref, _ = oracle.tau00_batched(batch, "long double")
+    out = []
+    try:
+        for g in (1, 2, 3, 8):
+            lt.lsms_set_groups(g)
+            tau, info, _ = lt.tau00_from_liz_batch(batch)
+            assert not info.any()
+            out.append(tau)
+        lt.lsms_set_groups(8)
+        small = sl.make_batch("T").select([0, 5, 9])
+        tau_s, info_s, _ = lt.tau00_from_liz_batch(small)
+        assert not info_s.any()
+    finally:
+        lt.lsms_set_groups(0)
+    for tau in out[1:]:
+        assert np.array_equal(out[0], tau)
+    assert max(relF(out[0][b], ref[b]) for b in range(11)) < 1e-10
+    assert np.array_equal(tau_s, out[0][[0, 5, 9]])
+
+
 def test_schur_update_alone_matches_numpy(lt):
     """K4 in isolation: C -= A B on ragged shapes (several tiles + tails in M, N and K)."""
     for n, c0, kk in ((333, 10, 64), (200, 0, 37), (130, 3, 16), (97, 40, 5)):
