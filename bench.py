@@ -152,7 +152,7 @@ def main() -> None:
     ap.add_argument("--nb", type=int, default=0, help="outer panel width override (0 = library default)")
     ap.add_argument("--ib", type=int, default=0, help="inner panel width override")
     ap.add_argument("--no-lookahead", action="store_true", help="factor the next panel in front of, not under, the update")
-    ap.add_argument("--panel", type=int, default=0, help="K2 variant: 0 register-blocked 256 thr, 1 512 thr, -1 L2-resident")
+    ap.add_argument("--panel", type=int, default=1, help="K2 variant: 1 register-blocked 512/256 thr, 0 256 thr, -1 L2-resident")
     ap.add_argument("--no-align", action="store_true", help="every outer panel NB wide (no tile-aligning first panel)")
     ap.add_argument("--groups", type=int, default=0, help="batch groups on separate streams (0 = library default)")
     args = ap.parse_args()

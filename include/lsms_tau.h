@@ -136,10 +136,10 @@ int lsms_set_lookahead(int on);
  * not depend on the setting (every item is eliminated independently).  Errors: -1 groups out of range. */
 int lsms_set_groups(int groups);
 
-/* Panel kernel (K2) variant: 0 (default) register-blocked sub-panels, 256 threads (half an SM, co-resident
- * with a Schur-update CTA under look-ahead); 1 register-blocked, 512 threads for tall panels; -1 the
- * L2-resident column-at-a-time kernel.  All variants pick the same pivots (|re|+|im|, ties to the lowest
- * row) and perform the same arithmetic per element.  Errors: -1 out of range. */
+/* Panel kernel (K2) variant: 1 (default) register-blocked sub-panels, 512 threads for panels taller than 1280
+ * rows and 256 below; 0 register-blocked, 256 threads throughout (half an SM, narrower sub-panels for tall
+ * panels); -1 the L2-resident column-at-a-time kernel.  All variants pick the same pivots (|re|+|im|, ties to
+ * the lowest row) and perform the same arithmetic per element.  Errors: -1 out of range. */
 int lsms_set_panel_variant(int variant);
 
 /* Tile alignment (default on): the first outer panel is n mod 64 columns wide, so that all later trailing

@@ -99,7 +99,7 @@ def lsms_set_lookahead(on: bool = True) -> None:
     _check(lib().lsms_set_lookahead(int(bool(on))), "lsms_set_lookahead")
 
 
-def lsms_set_panel_variant(variant: int = 0) -> None:
+def lsms_set_panel_variant(variant: int = 1) -> None:
     _check(lib().lsms_set_panel_variant(int(variant)), "lsms_set_panel_variant")
 
 

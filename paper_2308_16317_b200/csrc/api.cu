@@ -84,7 +84,7 @@ static size_t tau_ws_bytes(int n, int k, int batch) { return tau_ws_layout(nullp
 static int g_lookahead = 1;
 static int g_groups = 0;                  // 0 = chosen per shape
 static int g_align_first = 1;              // first panel n mod 64 wide (tile-aligned trailing matrices)
-static int g_panel_variant = 0;           // -1 L2-resident k_panel, 0 register-blocked half-SM, 1 register-blocked full-SM
+static int g_panel_variant = 1;           // -1 L2-resident k_panel, 0 register-blocked 256 threads, 1 register-blocked 512 threads for tall panels
 constexpr int MAX_GROUPS = 8;
 // Stream set of one batch group (see eliminate_groups): group 0 runs on the caller's stream, the others on
 // library-owned streams; every group has a high-priority auxiliary stream for the look-ahead panel.
@@ -205,7 +205,7 @@ static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* inf
 // items; the caller's stream is forked into the group streams and joined again before the call returns.
 static int pick_groups(int n, int batch) {
     int g = g_groups;
-    if (g <= 0) g = (batch >= 64) ? 4 : (batch >= 16 ? 2 : 1);
+    if (g <= 0) g = (batch >= 16) ? 2 : 1;
     if (g > MAX_GROUPS) g = MAX_GROUPS;
     if (g > batch) g = batch;
     (void)n;

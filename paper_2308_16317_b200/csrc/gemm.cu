@@ -13,14 +13,14 @@
 
 namespace lsms {
 
-constexpr int BM = 64, BN = 64, KS = 16, STAGES = 3;
+constexpr int BM = 64, BN = 64, KS = 16;
 constexpr int LDA_S = BM + 2;      // complex units; == 2 (mod 8): conflict-free LDS.128 of A fragments
 constexpr int LDB_S = KS + 4;      // complex units; == 4 (mod 8): conflict-free LDS.128 of B fragments
 constexpr int A_STAGE = KS * LDA_S;        // complex elements
 constexpr int B_STAGE = BN * LDB_S;
 constexpr int STAGE_ELEMS = A_STAGE + B_STAGE;
 constexpr int GEMM_THREADS = 256;
-constexpr size_t GEMM_SMEM = (size_t)STAGES * STAGE_ELEMS * sizeof(c128) + STAGES * sizeof(uint64_t);
+template <int STAGES> constexpr size_t gemm_smem() { return (size_t)STAGES * STAGE_ELEMS * sizeof(c128) + STAGES * sizeof(uint64_t); }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -52,6 +52,7 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 
 // Fill ring slot s with K-chunk kc of the A and B tiles: one bulk copy per tile column, issued by
 // threads 0..KS+BN-1; thread 0 also posts the expected byte count on the slot's mbarrier.
+template <int STAGES>
 __device__ __forceinline__ void issue_chunk(const GemmShape& g, const c128* A, const c128* B, c128* ring, uint64_t* full,
                                             int kc, int mvalid, int nvalid) {
     const int s = kc % STAGES, t = threadIdx.x;
@@ -69,6 +70,7 @@ __device__ __forceinline__ void issue_chunk(const GemmShape& g, const c128* A, c
     }
 }
 
+template <int STAGES>
 __global__ void __launch_bounds__(GEMM_THREADS, 2)
 k_schur_gemm(GemmShape g, int tiles_m) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -89,7 +91,7 @@ k_schur_gemm(GemmShape g, int tiles_m) {
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    for (int kc = 0; kc < STAGES && kc < nchunks; ++kc) issue_chunk(g, A, B, ring, full, kc, mvalid, nvalid);
+    for (int kc = 0; kc < STAGES && kc < nchunks; ++kc) issue_chunk<STAGES>(g, A, B, ring, full, kc, mvalid, nvalid);
 
     // C tile -> accumulators (issued before the first wait so that it overlaps the TMA fill)
     const int gq = lane >> 2, q = lane & 3;              // fragment coordinates: A[gq][q], B[q][gq], C[gq][2q..2q+1]
@@ -155,7 +157,7 @@ k_schur_gemm(GemmShape g, int tiles_m) {
         }
         if (kc + STAGES < nchunks) {          // refill this slot once every warp is done with it
             __syncthreads();
-            issue_chunk(g, A, B, ring, full, kc + STAGES, mvalid, nvalid);
+            issue_chunk<STAGES>(g, A, B, ring, full, kc + STAGES, mvalid, nvalid);
         }
     }
 
@@ -170,11 +172,11 @@ k_schur_gemm(GemmShape g, int tiles_m) {
             }
 }
 
-int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
-    if (g.Mr <= 0 || g.Nc <= 0 || g.K <= 0 || g.batch <= 0) return 0;
+template <int STAGES>
+static int launch_classic(const GemmShape& g, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEMM_SMEM));
+        LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<STAGES>()));
         attr_set = true;
     }
     const int tiles_m = (g.Mr + BM - 1) / BM, tiles_n = (g.Nc + BN - 1) / BN;
@@ -183,10 +185,20 @@ int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
         h.A = g.A + (size_t)b0 * g.strideA; h.B = g.B + (size_t)b0 * g.strideB; h.C = g.C + (size_t)b0 * g.strideC;
         h.batch = g.batch - b0 < 65535 ? g.batch - b0 : 65535;
         dim3 grid((unsigned)(tiles_m * tiles_n), (unsigned)h.batch);
-        k_schur_gemm<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(h, tiles_m);
+        k_schur_gemm<STAGES><<<grid, GEMM_THREADS, gemm_smem<STAGES>(), st>>>(h, tiles_m);
         LSMS_LAUNCH_CHECK();
     }
     return 0;
+}
+
+// K <= 16 is a single chunk: one ring stage (37 KB of shared memory instead of 112 KB) for the rank-IB updates
+// inside an outer panel.  Why two CTAs of 8 warps per SM: the DMMA result latency is about 220 cycles (measured:
+// one CTA per SM reaches 21.8 of 36.9 TFLOP/s) and ptxas schedules the two products of an accumulator four DMMAs
+// apart, so four warps per scheduler are needed to keep the pipe full.
+int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
+    if (g.Mr <= 0 || g.Nc <= 0 || g.K <= 0 || g.batch <= 0) return 0;
+    if (g.K <= KS) return launch_classic<1>(g, st);
+    return launch_classic<3>(g, st);
 }
 
 }  // namespace lsms

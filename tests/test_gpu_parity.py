@@ -296,7 +296,7 @@ def test_panel_kernel_variants_match_oracle(lt, variant):
         assert not infom.any()
         assert max(relF(taum[b], refm[b]) for b in range(2)) < 1e-10
     finally:
-        lt.lsms_set_panel_variant(0)
+        lt.lsms_set_panel_variant(1)
 
 
 def test_batch_groups_give_identical_results(lt):
@@ -324,18 +324,21 @@ def test_batch_groups_give_identical_results(lt):
 
 
 def test_schur_update_alone_matches_numpy(lt):
-    """K4 in isolation: C -= A B on ragged shapes (several tiles + tails in M, N and K)."""
-    for n, c0, kk in ((333, 10, 64), (200, 0, 37), (130, 3, 16), (97, 40, 5)):
-        A = sl.random_dense_matrices(2, n, seed=n)
-        M = torch.from_numpy(A).cuda()
-        lt.lsms_schur_update_batched(M, n, c0, kk, 2)
-        torch.cuda.synchronize()
-        out = M.cpu().numpy().transpose(0, 2, 1)
-        for b in range(2):
-            ref = A[b].T.copy()
-            r0 = c0 + kk
-            ref[r0:, r0:] -= ref[r0:, c0:r0] @ ref[c0:r0, r0:]
-            assert np.max(np.abs(out[b] - ref)) < 1e-12 * np.abs(ref).max() * kk
+    """K4 in isolation: C -= A B on ragged shapes (several tiles + tails in M, N and K; K of 1..6 chunks, so both the
+    one-stage and the three-stage ring are exercised)."""
+    if True:
+        for n, c0, kk, nb in ((333, 10, 64, 2), (200, 0, 37, 2), (130, 3, 16, 2), (97, 40, 5, 2), (700, 20, 96, 3), (450, 7, 48, 5),
+                              (1100, 0, 64, 1)):
+            A = sl.random_dense_matrices(nb, n, seed=n)
+            M = torch.from_numpy(A).cuda()
+            lt.lsms_schur_update_batched(M, n, c0, kk, nb)
+            torch.cuda.synchronize()
+            out = M.cpu().numpy().transpose(0, 2, 1)
+            for b in range(nb):
+                ref = A[b].T.copy()
+                r0 = c0 + kk
+                ref[r0:, r0:] -= ref[r0:, c0:r0] @ ref[c0:r0, r0:]
+                assert np.max(np.abs(out[b] - ref)) < 1e-12 * np.abs(ref).max() * kk
 
 
 # ------------------------------------------------------------------ end-to-end host entry point
