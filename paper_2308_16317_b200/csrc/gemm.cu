@@ -192,9 +192,12 @@ static int launch_classic(const GemmShape& g, cudaStream_t st) {
 }
 
 // K <= 16 is a single chunk: one ring stage (37 KB of shared memory instead of 112 KB) for the rank-IB updates
-// inside an outer panel.  Why two CTAs of 8 warps per SM: the DMMA result latency is about 220 cycles (measured:
-// one CTA per SM reaches 21.8 of 36.9 TFLOP/s) and ptxas schedules the two products of an accumulator four DMMAs
-// apart, so four warps per scheduler are needed to keep the pipe full.
+// inside an outer panel.  Why two CTAs of 8 warps per SM: measured, one such CTA per SM reaches 21.8 of 36.9 TFLOP/s
+// (ptxas keeps the two products of an accumulator four DMMAs apart whatever the source order, and a warp then waits
+// on the DMMA result), two reach 34.2; the remaining 8 % is the time one of the two CTAs spends loading or storing
+// its C tile.  Tried and dropped: a one-DMMA-per-accumulator loop body with operands picked by 64-bit loads
+// (31.7 TFLOP/s, bank-conflicted LDS.64) and a persistent one-CTA-per-SM variant with the next C tile prefetched
+// into shared memory (23.3 TFLOP/s).
 int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
     if (g.Mr <= 0 || g.Nc <= 0 || g.K <= 0 || g.batch <= 0) return 0;
     if (g.K <= KS) return launch_classic<1>(g, st);
