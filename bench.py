@@ -337,7 +337,7 @@ def main() -> None:
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "c128 (f64)", "data": "synthetic",
-            "config": {"workload": f"{cfg.name} LIZ (BASELINE.json configs[{cfg.index}]): {cfg.n_sites} sites, lmax={cfg.lmax}, "
+            "config": {"workload": f"{cfg.name} LIZ ({'BASELINE.json configs[%d]' % cfg.index if cfg.index < 5 else 'SURVEY 8(f) f1, paper shape PAPER.md:104'}): {cfg.n_sites} sites, lmax={cfg.lmax}, "
                                    f"spin_canted={cfg.spin_canted}, n={n}, k={k}, batch={B} per GPU",
                        "l2_policy": f"inputs larger than L2: {16.0 * n * n * B / 1e9:.2f} GB of M re-assembled and streamed per step",
                        "parallelism": f"batch sharded over {world} GPU(s), no data-path collective"},

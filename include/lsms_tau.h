@@ -118,6 +118,16 @@ int lsms_tau00_from_host(const lsms_c128* delta_host, const int* species_host, c
                          void* device_scratch, size_t scratch_bytes, void* cuda_stream,
                          size_t* h2d_bytes, size_t* d2h_bytes);
 
+/* the tau part of the energy-contour integral of eq. (2)/(3): for every
+ * central atom a,  out_a = sum_q weights_q * tau00_{a,q},  with the batch index = a * n_energies + q of
+ * lsms_tau00_batched (reading A19).  The caller supplies the complex quadrature weights (rule weight x dz/dq).
+ *   tau00   [n_atoms][n_energies][k*k]  device (the tau00_out of lsms_tau00_batched)
+ *   weights [n_energies]                device
+ *   out     [n_atoms][k*k]              device (out), column-major k x k like tau00
+ * Errors: -1 tau00, -2 weights, -3 n_atoms, -4 n_energies (1..2048), -5 k, -6 out.               */
+int lsms_contour_sum_batched(const lsms_c128* tau00, const lsms_c128* weights, int n_atoms, int n_energies, int k,
+                             lsms_c128* out, void* cuda_stream);
+
 /* Tuning knobs (process-wide, not thread-safe; defaults chosen per shape when 0):
  *   outer panel width NB (multiple of 4, <= 96; the workspace size depends on it: query
  *   lsms_workspace_bytes after setting it) and inner panel width IB (<= 16).             */

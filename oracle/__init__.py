@@ -182,3 +182,16 @@ def tau00_batched(batch, mode: str = "double") -> tuple[np.ndarray, np.ndarray]:
 
 def max_threads() -> int:
     return int(lib().orc_max_threads())
+
+
+def contour_sum(tau: np.ndarray, w: np.ndarray) -> np.ndarray:
+    """out[a] = sum_q w[q] tau[a, q]  (the tau part of eq. (2)/(3)).
+    tau complex128 [n_atoms, n_e, ...], w complex128 [n_e]."""
+    tau = np.ascontiguousarray(tau, dtype=np.complex128)
+    w = np.ascontiguousarray(w, dtype=np.complex128)
+    na, ne = tau.shape[0], tau.shape[1]
+    kk = int(np.prod(tau.shape[2:]))
+    out = np.zeros((na,) + tau.shape[2:], dtype=np.complex128)
+    lib().orc_contour_sum(na, ne, kk, _dp(tau.view(np.float64)), _dp(w.view(np.float64)), _dp(out.view(np.float64)))
+    return out
+

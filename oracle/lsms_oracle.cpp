@@ -475,4 +475,17 @@ int orc_max_threads(void) {
 #endif
 }
 
+// the tau part of the contour integral of eq. (2)/(3): for every central atom a,
+//   out_a = sum_q w_q tau00_{a,q},   q over the n_e contour points, w_q = quadrature weight * dz/dq (complex).
+// tau [n_atoms][n_e][kk], w [n_e], out [n_atoms][kk]; plain loops in the order of the definition.
+void orc_contour_sum(int n_atoms, int n_e, int kk, const double* tau, const double* w, double* out) {
+    const cd* T = reinterpret_cast<const cd*>(tau); const cd* W = reinterpret_cast<const cd*>(w); cd* O = reinterpret_cast<cd*>(out);
+    for (int a = 0; a < n_atoms; ++a)
+        for (int e = 0; e < kk; ++e) {
+            cd s(0.0, 0.0);
+            for (int q = 0; q < n_e; ++q) s += W[q] * T[((size_t)a * n_e + q) * kk + e];
+            O[(size_t)a * kk + e] = s;
+        }
+}
+
 }  // extern "C"

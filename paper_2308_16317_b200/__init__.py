@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "lsms_version", "lsms_workspace_bytes", "lsms_solve_workspace_bytes", "lsms_host_call_scratch_bytes",
     "lsms_tinv_from_phase_shifts", "lsms_build_M_batched", "lsms_tau00_batched",
-    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_set_blocking", "lsms_set_lookahead", "lsms_set_groups", "lsms_set_panel_variant", "lsms_set_align_first",
+    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_contour_sum_batched", "lsms_set_blocking", "lsms_set_lookahead", "lsms_set_groups", "lsms_set_panel_variant", "lsms_set_align_first",
     "lsms_last_launch_count", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe", "lsms_schur_update_batched",
     "lsms_debug_gaunt_closed_form",
 )
@@ -50,6 +50,7 @@ def lib() -> ctypes.CDLL:
         L.lsms_solve_central_column_batched.argtypes = [vp, ci, ci, ci, ci, vp, vp, vp, sz, vp]
         L.lsms_tau00_from_host.argtypes = [vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, vp, vp, vp, sz, vp,
                                            ctypes.POINTER(sz), ctypes.POINTER(sz)]
+        L.lsms_contour_sum_batched.argtypes = [vp, vp, ci, ci, ci, vp, vp]
         L.lsms_set_blocking.argtypes = [ci, ci]
         L.lsms_fp64_peak_probe.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double), vp]
         L.lsms_schur_update_batched.argtypes = [vp, ci, ci, ci, ci, vp]
@@ -211,6 +212,15 @@ def lsms_solve_central_column_batched(M, n_sites, kmax, spin_canted, batch, X_ou
                                                    _ptr(info), _ptr(workspace), workspace.numel(), _stream(stream)),
            "lsms_solve_central_column_batched")
     return X_out, info
+
+
+def lsms_contour_sum_batched(tau00, weights, n_atoms, n_energies, k, out=None, stream=None):
+    import torch
+    if out is None:
+        out = torch.empty((n_atoms, k, k), dtype=torch.complex128, device=tau00.device)
+    _check(lib().lsms_contour_sum_batched(_ptr(tau00), _ptr(weights), n_atoms, n_energies, k, _ptr(out), _stream(stream)),
+           "lsms_contour_sum_batched")
+    return out
 
 
 def lsms_schur_update_batched(M, n, c0, kk, batch, stream=None):

@@ -423,6 +423,18 @@ int lsms_tau00_from_host(const lsms_c128* delta_host, const int* species_host, c
     return 0;
 }
 
+int lsms_contour_sum_batched(const lsms_c128* tau00, const lsms_c128* weights, int n_atoms, int n_energies, int k,
+                             lsms_c128* out, void* cuda_stream) {
+    if (!tau00 || !aligned16(tau00)) return -1;
+    if (!weights || !aligned16(weights)) return -2;
+    if (n_atoms < 1) return -3;
+    if (n_energies < 1 || n_energies > 2048) return -4;
+    if (k < 1 || k > 4096) return -5;
+    if (!out || !aligned16(out)) return -6;
+    g_launches.n = 0;
+    return launch_contour_sum((const c128*)tau00, (const c128*)weights, n_atoms, n_energies, k * k, (c128*)out, (cudaStream_t)cuda_stream);
+}
+
 int lsms_set_blocking(int nb_outer, int ib_inner) {
     if (nb_outer < 0 || nb_outer > 96 || (nb_outer % 4) != 0) return -1;
     if (ib_inner < 0 || ib_inner > 16) return -2;

@@ -40,6 +40,9 @@ int launch_final_inverse(c128* base, size_t stride, int n, int k, int batch, c12
 int launch_backsolve_central(const c128* LU, size_t stride, int n, int k, int batch, const c128* tau, c128* X, cudaStream_t st);
 size_t final_inverse_ws_bytes(int k, int batch);
 
+// reduce.cu
+int launch_contour_sum(const c128* tau, const c128* w, int n_atoms, int n_e, int kk, c128* out, cudaStream_t st);
+
 // probe.cu
 int run_peak_probe(int which, int iters, double* tflops, cudaStream_t st);
 

@@ -59,6 +59,7 @@ class LizConfig:
     n_atoms: int
     n_energies: int
     contour: str        # "semicircle" (A6) or "arc" (A7)
+    ni_fraction: float = 0.5   # P(site is Ni): 1/2 for BASELINE.json's configs (A9), 0.3 for the paper's NiAu
 
     @property
     def kmax(self) -> int:
@@ -87,6 +88,10 @@ CONFIGS = {
     "P": LizConfig("production", 2, 135, 3, False, 4, 32, "semicircle"),
     "C": LizConfig("spin-canted", 3, 135, 3, True, 2, 32, "semicircle"),
     "H": LizConfig("high-l", 4, 135, 4, True, 1, 24, "arc"),
+    # the paper's own NiAu shapes (30 % Ni / 70 % Au, N_LIZ = 249, l_max = 4):
+    # rank 6225 and, spin-canted, 12450.  Not in BASELINE.json's configs; batch sizes chosen to fit one GPU.
+    "N": LizConfig("NiAu-249", 5, 249, 4, False, 1, 24, "semicircle", 0.3),
+    "NC": LizConfig("NiAu-249-canted", 6, 249, 4, True, 1, 12, "semicircle", 0.3),
 }
 
 FCC_SHELL_CLOSURES = (1, 13, 19, 43, 55, 79, 87, 135, 141, 177, 201, 225, 249, 321)
@@ -139,6 +144,19 @@ def contour_energies(kind: str, n_points: int) -> np.ndarray:
     return 0.1 + 0.6 * np.exp(1j * theta)
 
 
+def contour_weights(kind: str, n_points: int) -> np.ndarray:
+    """Complex quadrature weights w_q with  int_{-0.5}^{0.7} f(z) dz ~= sum_q w_q f(z_q)  along the contour of
+    `contour_energies` (same node order): z = 0.1 + 0.6 e^{i theta}, theta = theta_max (1 - x)/2, so
+    w_q = omega_q * dz/dx = -i * 0.6 e^{i theta_q} * (theta_max / 2) * omega_q  with omega_q the Gauss-Legendre
+    weights.  Like the nodes, the rule is input data for the reduction of SURVEY 8(f) f4, not method arithmetic."""
+    x, om = np.polynomial.legendre.leggauss(n_points)
+    order = np.argsort(x)
+    x, om = x[order], om[order]
+    tmax = {"semicircle": np.pi, "arc": np.pi / 4.0}[kind]
+    theta = tmax * (1.0 - x) / 2.0
+    return (-1j * 0.6 * np.exp(1j * theta) * (tmax / 2.0) * om).astype(np.complex128)
+
+
 def phase_shift_table(cfg: LizConfig) -> np.ndarray:
     """delta[species(0=Ni,1=Au)][spin][l], complex128 (A10, A11).
 
@@ -159,12 +177,12 @@ def phase_shift_table(cfg: LizConfig) -> np.ndarray:
 
 
 def atom_occupancy_and_moments(cfg: LizConfig, atom: int) -> tuple[np.ndarray, np.ndarray]:
-    """Per central atom: species int32 [n_sites] ~ Bernoulli(1/2) (A9) and unit
+    """Per central atom: species int32 [n_sites], Ni with probability cfg.ni_fraction (1/2: A9) and unit
     moment directions float64 [n_sites,3] (A12, isotropic).  Stream 1+atom."""
     rng = SplitMix64(BASE_SEED + 1000 * cfg.index + 1 + atom)
     species = np.zeros(cfg.n_sites, dtype=np.int32)
     for i in range(cfg.n_sites):
-        species[i] = 1 if rng.uniform() >= 0.5 else 0
+        species[i] = 1 if rng.uniform() >= cfg.ni_fraction else 0
     mom = np.zeros((cfg.n_sites, 3), dtype=np.float64)
     for i in range(cfg.n_sites):
         a, b = rng.normal_pair()

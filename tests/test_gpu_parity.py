@@ -205,6 +205,28 @@ def test_tau00_high_l_full_size_properties(lt):
         assert residual(Mo, X[i].cpu().numpy().T, cfg.k) < RES_TOL
 
 
+@pytest.mark.parametrize("key,item", [("N", 23), ("NC", 0)])
+def test_tau00_paper_niau_shapes_properties(lt, key, item):
+    """the paper's own NiAu ranks 6225 and 12450 (N_LIZ = 249, l_max = 4).  Same
+    property checks as the high-l case: assembled M equals the oracle's M block by block, the central block column
+    solves M X = E to <= 1e-12, and tau00 is the central block of X (checked against lsms_tau00_batched itself)."""
+    batch = sl.make_batch(key).select([item])
+    cfg = batch.cfg
+    assert cfg.n == {"N": 6225, "NC": 12450}[key]
+    M, _, _ = gpu_M(lt, batch)
+    X, info = lt.lsms_solve_central_column_batched(M, cfg.n_sites, cfg.kmax, cfg.spin_canted, 1)
+    torch.cuda.synchronize()
+    assert not info.cpu().numpy().any()
+    Mo = oracle_M(batch, 0)
+    assert block_rel_err(M[0].cpu().numpy().T, Mo, cfg.k) < ASM_TOL
+    Xh = X[0].cpu().numpy().T
+    assert residual(Mo, Xh, cfg.k) < RES_TOL
+    tau, info2 = lt.lsms_tau00_batched(M, cfg.n_sites, cfg.kmax, cfg.spin_canted, 1)      # overwrites M
+    torch.cuda.synchronize()
+    assert not info2.cpu().numpy().any()
+    assert relF(tau[0].cpu().numpy().T, Xh[cfg.n - cfg.k:, :]) < 1e-12
+
+
 # ------------------------------------------------------------------ direct input to lsms_tau00_batched
 
 @pytest.mark.parametrize("n_sites,kmax,canted", [(7, 9, False), (37, 1, False), (1, 16, False), (2, 4, True),
@@ -339,6 +361,31 @@ def test_schur_update_alone_matches_numpy(lt):
                 r0 = c0 + kk
                 ref[r0:, r0:] -= ref[r0:, c0:r0] @ ref[c0:r0, r0:]
                 assert np.max(np.abs(out[b] - ref)) < 1e-12 * np.abs(ref).max() * kk
+
+
+# ------------------------------------------------------------------ contour reduction
+
+def test_contour_sum_matches_oracle(lt):
+    """sum_q w_q tau00_{a,q} on the device vs the oracle's loop: the real tau00 of two tiny-LIZ atoms on the full
+    32-point contour, plus ragged shapes (k*k not a multiple of the block, one energy, many atoms)."""
+    cfg = sl.custom_config(13, 3, False, n_atoms=2, n_energies=32, index=0)
+    batch = sl.make_batch(cfg)
+    tau, info, _ = lt.tau00_from_liz_batch(batch)
+    assert not info.any()
+    w = sl.contour_weights("semicircle", 32)
+    ref = oracle.contour_sum(tau.reshape(2, 32, cfg.k, cfg.k), w)
+    tau_d = torch.from_numpy(np.ascontiguousarray(tau)).cuda()
+    out = lt.lsms_contour_sum_batched(tau_d, torch.from_numpy(w).cuda(), 2, 32, cfg.k)
+    torch.cuda.synchronize()
+    assert relF(out.cpu().numpy(), ref) < 1e-14
+    rng = np.random.default_rng(11)
+    for na, ne, k in ((1, 1, 1), (5, 24, 50), (300, 3, 7), (2, 33, 13)):
+        t = rng.standard_normal((na, ne, k, k)) + 1j * rng.standard_normal((na, ne, k, k))
+        ww = rng.standard_normal(ne) + 1j * rng.standard_normal(ne)
+        out = lt.lsms_contour_sum_batched(torch.from_numpy(t).cuda(), torch.from_numpy(ww).cuda(), na, ne, k)
+        torch.cuda.synchronize()
+        ref = oracle.contour_sum(t, ww)
+        assert np.max(np.abs(out.cpu().numpy() - ref)) < 1e-13 * np.sqrt(ne) * np.abs(t).max() * np.abs(ww).max()
 
 
 # ------------------------------------------------------------------ end-to-end host entry point

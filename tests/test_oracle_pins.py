@@ -360,3 +360,41 @@ def test_generator_recipe():
     assert np.all((d.real > 0) & (d.real < 1.5) & (d.imag > 0) & (d.imag < 0.05))
     bc = sl.make_batch("C", n_atoms=1, n_energies=2)
     assert np.allclose(np.linalg.norm(bc.moment_dir, axis=-1), 1.0)
+
+
+# ------------------------------------------------------------------ contour reduction
+
+def test_contour_sum_closed_forms():
+    """sum_q w_q tau(z_q) against integrals known in closed form (eq. (2): an energy integral up to E_F
+    taken along the contour): polynomials int_{-0.5}^{0.7} z^m dz = (0.7^{m+1} - (-0.5)^{m+1})/(m+1), and a simple
+    pole, where the arc over the pole differs from the straight path by -2 pi i (clockwise closed contour), while a
+    pole outside the half disc gives the principal-branch logarithm.  Fixes weights, node order and the reduction."""
+    for kind, npts, z_end in (("semicircle", 32, -0.5 + 0j), ("arc", 24, 0.1 + 0.6 * np.exp(1j * np.pi / 4))):
+        z = sl.contour_energies(kind, npts)
+        w = sl.contour_weights(kind, npts)
+        # a 3 x 2 "matrix" of monomials per atom, two atoms with different prefactors
+        tau = np.zeros((2, npts, 3, 2), dtype=np.complex128)
+        for a in range(2):
+            for i in range(3):
+                for j in range(2):
+                    tau[a, :, i, j] = (a + 1.5) * z ** (2 * i + j)
+        out = oracle.contour_sum(tau, w)
+        for a in range(2):
+            for i in range(3):
+                for j in range(2):
+                    m = 2 * i + j
+                    exact = (a + 1.5) * (0.7 ** (m + 1) - z_end ** (m + 1)) / (m + 1)
+                    assert abs(out[a, i, j] - exact) < 2e-14
+    z = sl.contour_energies("semicircle", 32)
+    w = sl.contour_weights("semicircle", 32)
+    for z0, winding in ((0.1 + 0.3j, -2j * np.pi), (0.1 + 0.9j, 0.0), (0.2 - 0.4j, 0.0)):
+        val = oracle.contour_sum((1.0 / (z - z0))[None, :, None], w)[0, 0]
+        exact = np.log(0.7 - z0) - np.log(-0.5 - z0) + winding
+        assert abs(val - exact) < 2e-6          # truncation error of the 32-point rule for a pole 0.3 away (seen: 4e-7)
+    # linearity and the order of the energy axis: a weight vector with a single 1 picks that energy's tau
+    rng = np.random.default_rng(5)
+    tau = rng.standard_normal((3, 7, 4, 4)) + 1j * rng.standard_normal((3, 7, 4, 4))
+    for q in (0, 3, 6):
+        e = np.zeros(7, dtype=np.complex128); e[q] = 1.0
+        assert np.array_equal(oracle.contour_sum(tau, e), tau[:, q])
+
