@@ -117,9 +117,9 @@ static int factor_panel(c128* M, int n, int batch, int J, int W, int ne, int IB,
         const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
         int rc;
         if (g_panel_variant >= 0 && n - c0 <= 16384) {
-            // register-blocked K2: factors the inner panel and applies its interchanges to the whole outer panel
+            // register-blocked K2: factors the inner panel, applies its interchanges to the whole outer panel and
+            // solves the w x w triangle for the outer panel's columns to the right
             { ProfScope ps(1, st); rc = launch_panel_reg(M, stride, n, J, W, c0, w, ne, batch, piv, info, g_panel_variant, st); } if (rc) return rc;
-            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, c0 + w, Jend, 2, batch, piv, st); } if (rc) return rc;
         } else {
             { ProfScope ps(1, st); rc = launch_panel(M, stride, n, c0, w, ne, batch, piv, info, st); } if (rc) return rc;
             { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, J, c0, 1, batch, piv, st); } if (rc) return rc;

@@ -16,9 +16,11 @@
 //        solve, whose result (rows of U) is published in shared memory
 //     5  rank-S update of the inner panel's remaining columns, L from registers, U from shared memory
 //
-// The row interchanges of the whole outer panel are thus done here (K3's interchange launches are
-// gone); the columns to the right of the inner panel still need the w x w triangular solve and the
-// rank-w update (k_swap_trsm mode 2 and K4).
+//   after the last sub-panel:
+//     6  the w x w unit-lower solve for the outer panel's columns to the right of the inner panel
+//
+// The row interchanges and triangular solves inside an outer panel are thus all done here (K3's launches
+// inside the outer panel are gone); what remains per inner panel is the rank-w update of those columns (K4).
 #include "common.cuh"
 #include "internal.h"
 
@@ -240,6 +242,28 @@ k_panel_reg(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
             }
         }
         __syncthreads();
+    }
+    // ---- 6: U12 of the outer panel's columns to the RIGHT of this inner panel: solve the w x w unit-lower L11
+    // against rows [c0, c0+w) of each such column (their interchanges were applied in step 4).  One thread per
+    // column; L11 is read back from the panel this CTA has just stored.
+    const int nr = (J + Wout) - (c0 + w);
+    if (nr > 0) {
+        __shared__ c128 Lw[P2_MAXW * P2_MAXW];
+        for (int e = tid; e < w * w; e += THREADS) { const int r = e % w, c = e / w; Lw[r + P2_MAXW * c] = A[(c0 + r) + (size_t)(c0 + c) * n]; }
+        __syncthreads();
+        if (tid < nr) {
+            c128* col = A + (size_t)(c0 + w + tid) * n + c0;
+            c128 x[P2_MAXW];
+#pragma unroll
+            for (int i = 0; i < P2_MAXW; ++i) x[i] = (i < w) ? col[i] : zero;
+#pragma unroll
+            for (int jq = 0; jq < P2_MAXW; ++jq)
+#pragma unroll
+                for (int i = jq + 1; i < P2_MAXW; ++i)
+                    if (i < w) cfms(x[i], Lw[i + P2_MAXW * jq], x[jq]);
+#pragma unroll
+            for (int i = 0; i < P2_MAXW; ++i) if (i < w) col[i] = x[i];
+        }
     }
 }
 
