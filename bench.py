@@ -240,6 +240,7 @@ def main() -> None:
     clocks = sampler.stop() if rank == 0 else None
     assert not info.cpu().numpy().any()
     ms_step = ms_total / args.steps
+    launches_timed = launches[0] * args.steps          # counted during the timed region (the breakdown step below runs another schedule)
     value = world * B / (ms_step * 1e-3)
     tflops = value * flops_per_matrix(n) / 1e12
 
@@ -345,7 +346,7 @@ def main() -> None:
             "frac_fp64_peak": tflops / peak_fp64 if peak_fp64 else None,
             "schedule": {"groups": args.groups or "auto (2)", "lookahead": not args.no_lookahead, "panel_variant": args.panel,
                          "nb": args.nb or 64, "ib": args.ib or 16, "align_first_panel": not args.no_align},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches[0] * args.steps,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches_timed,
             "roofline": roofline, "cpu_baseline": cpu_baseline,
         }))
     if world > 1:
