@@ -36,6 +36,12 @@ NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0
 FALLBACK_BF16_TFLOPS = 1590.0          # B200_PROFILING.md fallback (burst); sustained ~1400
 
 
+def workload_label(cfg) -> str:
+    src = "BASELINE.json configs[%d]" % cfg.index if cfg.index < 5 else "SURVEY 8(f) f1, paper shape PAPER.md:104"
+    return (f"{cfg.name} LIZ ({src}): {cfg.n_sites} sites, lmax={cfg.lmax}, spin_canted={cfg.spin_canted}, "
+            f"n={cfg.n}, k={cfg.k}, batch={cfg.batch} per GPU")
+
+
 def flops_per_matrix(n: int) -> float:
     return 8.0 / 3.0 * float(n) ** 3
 
@@ -133,7 +139,7 @@ def run_reference(args, cfg) -> None:
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "c128 (f64)", "data": "synthetic",
-        "config": {"workload": f"{cfg.name} LIZ: {cfg.n_sites} sites, lmax={cfg.lmax}, n={cfg.n}, batch={cfg.batch}"},
+        "config": {"workload": workload_label(cfg)},
         "tflops": value * flops_per_matrix(cfg.n) / 1e12,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -338,8 +344,7 @@ def main() -> None:
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "c128 (f64)", "data": "synthetic",
-            "config": {"workload": f"{cfg.name} LIZ ({'BASELINE.json configs[%d]' % cfg.index if cfg.index < 5 else 'SURVEY 8(f) f1, paper shape PAPER.md:104'}): {cfg.n_sites} sites, lmax={cfg.lmax}, "
-                                   f"spin_canted={cfg.spin_canted}, n={n}, k={k}, batch={B} per GPU",
+            "config": {"workload": workload_label(cfg),
                        "l2_policy": f"inputs larger than L2: {16.0 * n * n * B / 1e9:.2f} GB of M re-assembled and streamed per step",
                        "parallelism": f"batch sharded over {world} GPU(s), no data-path collective"},
             "tflops": tflops, "tflops_convention": "8/3 n^3 per matrix",
