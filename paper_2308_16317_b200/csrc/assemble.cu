@@ -127,11 +127,12 @@ __global__ void k_legendre_table(int l2, double* __restrict__ leg) {
 // One CTA per (column site sj, item b): it writes the k full columns of M that belong to site sj,
 // i.e. n*16 B contiguous per column (HBM-write-bound).
 //   phase 1 (a1): one thread per row site si != sj builds hY[si][L''] = h_{l''}(kappa R) Y_{L''}(R^) in smem
-//   phase 2 (a2): one thread per matrix row (si, s, L) walks the k columns (s', L') of the strip:
-//                 -g0 = -kappa sum_t coef_t hY[idx_t]   (s == s'),  0 (s != s'),  t^{-1} on the site diagonal.
+//   phase 2 (a2): one thread per (L, L') pair of the site block walks the row sites of the chunk:
+//                 -g0 = sum_t (-kappa coef_t) hY[idx_t]   (s == s'),  0 (s != s'),  t^{-1} on the site diagonal.
 // Row sites are processed in chunks that fit shared memory.
 constexpr int ASM_THREADS = 256;
 
+template <int MAXNT>       // >= l_max + 1: length of the per-thread Gaunt term arrays
 __global__ void __launch_bounds__(ASM_THREADS)
 k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, const double* __restrict__ moment,
            const c128* __restrict__ kappa, const c128* __restrict__ coef, const int* __restrict__ idx,
@@ -194,42 +195,57 @@ k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, c
             }
         }
         __syncthreads();
-        // ---- phase 2: rows of this chunk, all k columns of the strip
-        const int nrows = ns * k;
-        for (int rr = tid; rr < nrows; rr += ASM_THREADS) {
-            const int q = rr / k, w = rr % k, sr = w / kmax, L = w % kmax;
-            const int si = s0 + q;
-            const size_t row = (size_t)(si == 0 ? n_sites - 1 : si - 1) * k + w;
-            c128* dst = M + row + n * c0;
-            if (si == sj) {
-                // site-diagonal block: t^{-1} (g0^{ii} = 0, "between two different atom sites")
-                const c128* ti = tinv + ((size_t)b * n_sites + si) * nspin * nt;
-                int l = 0; while ((l + 1) * (l + 1) <= L) ++l;
-                c128 vd = ti[l], vo = zero;                      // same-spin and other-spin entry at column L
-                if (canted) {
-                    const double* mv = moment + ((size_t)b * n_sites + si) * 3;
-                    const c128 a = ti[l], bb = ti[nt + l];
-                    const c128 hsum = cscale(0.5, cadd(a, bb)), hdif = cscale(0.5, csub(a, bb));
-                    vd = (sr == 0) ? cadd(hsum, cscale(mv[2], hdif)) : csub(hsum, cscale(mv[2], hdif));
-                    vo = cmul(hdif, (sr == 0) ? cmake(mv[0], -mv[1]) : cmake(mv[0], mv[1]));   // (up,down): ex - i ey
-                }
-                for (int c = 0; c < k; ++c) {
-                    const int sc = c / kmax, Lc = c % kmax;
-                    dst[n * c] = (Lc == L) ? ((sc == sr) ? vd : vo) : zero;
-                }
-            } else {
-                const c128* hy = hY + (size_t)q * nl2;
-                for (int sc = 0; sc < nspin; ++sc)
-                    for (int Lp = 0; Lp < kmax; ++Lp) {
-                        c128 g = zero;
-                        if (sc == sr) {
-                            c128 s = zero;
-                            const int e = Lp * kmax + L;
-                            for (int t = 0; t < nt; ++t) cfma(s, coef[t * kk2 + e], hy[idx[t * kk2 + e]]);
-                            g = cneg(cmul(kap, s));
-                        }
-                        dst[n * (sc * kmax + Lp)] = g;
+        // ---- phase 2: one thread per (L, L') pair of the site block; its Gaunt terms (pre-multiplied by -kappa) stay
+        // in registers while it walks the row sites of the chunk: per element <= l_max+1 LDS.128 + complex FMAs and
+        // one (canted: four) coalesced store -- consecutive threads hold consecutive L = consecutive rows.
+        for (int p0 = 0; p0 < kk2; p0 += ASM_THREADS) {
+            const int p = p0 + tid;
+            if (p < kk2) {
+                const int L = p % kmax, Lp = p / kmax;
+                c128 cf[MAXNT]; int ix[MAXNT]; bool nz[MAXNT];
+#pragma unroll
+                for (int t = 0; t < MAXNT; ++t) {
+                    nz[t] = false; cf[t] = zero; ix[t] = 0;
+                    if (t < nt) {
+                        const c128 c = coef[t * kk2 + Lp * kmax + L];
+                        nz[t] = (c.x != 0.0 || c.y != 0.0);
+                        cf[t] = cneg(cmul(kap, c));
+                        ix[t] = idx[t * kk2 + Lp * kmax + L];
                     }
+                }
+                int lL = 0; while ((lL + 1) * (lL + 1) <= L) ++lL;
+                c128* colp = M + n * (c0 + Lp) + L;                    // column (sj, spin 0, L'), row offset L
+                for (int q = 0; q < ns; ++q) {
+                    const int si = s0 + q;
+                    const size_t rowb = (size_t)(si == 0 ? n_sites - 1 : si - 1) * k;
+                    if (si != sj) {
+                        const c128* hy = hY + (size_t)q * nl2;
+                        c128 g = zero;
+#pragma unroll
+                        for (int t = 0; t < MAXNT; ++t) if (nz[t]) cfma(g, cf[t], hy[ix[t]]);
+                        colp[rowb] = g;
+                        if (canted) {
+                            colp[rowb + kmax] = zero;                                   // (down, up)
+                            colp[rowb + n * kmax] = zero;                               // (up, down)
+                            colp[rowb + n * kmax + kmax] = g;                           // (down, down): g0 (x) 1_2
+                        }
+                    } else {
+                        // site-diagonal block: t^{-1} (g0^{ii} = 0, "between two different atom sites")
+                        const c128* ti = tinv + ((size_t)b * n_sites + si) * nspin * nt;
+                        const bool dg = (L == Lp);
+                        if (!canted) {
+                            colp[rowb] = dg ? ti[lL] : zero;
+                        } else {
+                            const double* mv = moment + ((size_t)b * n_sites + si) * 3;
+                            const c128 a = ti[lL], bb = ti[nt + lL];
+                            const c128 hsum = cscale(0.5, cadd(a, bb)), hdif = cscale(0.5, csub(a, bb));
+                            colp[rowb] = dg ? cadd(hsum, cscale(mv[2], hdif)) : zero;                         // (up, up)
+                            colp[rowb + kmax] = dg ? cmul(hdif, cmake(mv[0], mv[1])) : zero;                  // (down, up): ex + i ey
+                            colp[rowb + n * kmax] = dg ? cmul(hdif, cmake(mv[0], -mv[1])) : zero;             // (up, down): ex - i ey
+                            colp[rowb + n * kmax + kmax] = dg ? csub(hsum, cscale(mv[2], hdif)) : zero;       // (down, down)
+                        }
+                    }
+                }
             }
         }
     }
@@ -273,19 +289,23 @@ int launch_assemble(const c128* tinv, const double* site_pos, const double* mome
     const int nchunks = (n_sites + maxchunk - 1) / maxchunk;
     const int chunk = (n_sites + nchunks - 1) / nchunks;      // balanced chunks
     const size_t smem = (size_t)chunk * nl2 * sizeof(c128);
-    static size_t attr = 0;
-    if (smem > attr) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_assemble, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     const size_t k = kmax * (canted ? 2 : 1), n = (size_t)n_sites * k;
-    for (int b0 = 0; b0 < batch; b0 += 65535) {
-        int nb = batch - b0 < 65535 ? batch - b0 : 65535;
-        dim3 grid(n_sites, nb);
-        k_assemble<<<grid, ASM_THREADS, smem, st>>>(tinv + (size_t)b0 * n_sites * (canted ? 2 : 1) * nt,
-                                                    site_pos + (size_t)b0 * n_sites * 3,
-                                                    moment ? moment + (size_t)b0 * n_sites * 3 : nullptr, kappa + b0, coef, idx, leg,
-                                                    lmax, n_sites, canted, chunk, M + (size_t)b0 * n * n);
-        LSMS_LAUNCH_CHECK();
-    }
-    return 0;
+    auto run = [&](auto kern) -> int {
+        LSMS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(56 * 1024)));
+        for (int b0 = 0; b0 < batch; b0 += 65535) {
+            int nb = batch - b0 < 65535 ? batch - b0 : 65535;
+            dim3 grid(n_sites, nb);
+            kern<<<grid, ASM_THREADS, smem, st>>>(tinv + (size_t)b0 * n_sites * (canted ? 2 : 1) * nt,
+                                                  site_pos + (size_t)b0 * n_sites * 3,
+                                                  moment ? moment + (size_t)b0 * n_sites * 3 : nullptr, kappa + b0, coef, idx, leg,
+                                                  lmax, n_sites, canted, chunk, M + (size_t)b0 * n * n);
+            LSMS_LAUNCH_CHECK();
+        }
+        return 0;
+    };
+    if (lmax <= 3) return run(k_assemble<4>);
+    if (lmax == 4) return run(k_assemble<5>);
+    return run(k_assemble<9>);
 }
 
 }  // namespace lsms
