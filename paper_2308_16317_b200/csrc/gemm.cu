@@ -5,7 +5,7 @@
 // no f64 kind, so the warp-level DMMA is the FP64 tensor instruction on sm_100a).  One complex MAC =
 // 4 real MMAs:  Cr += Ar*(-Br) + Ai*Bi ;  Ci += Ar*(-Bi) + Ai*(-Br)   (so that C -= A*B).
 // Operand tiles are staged into shared memory by the TMA engine (cp.async.bulk, one bulk copy per
-// tile column, completion on an mbarrier) in a 3-stage ring.
+// tile column, completion on an mbarrier) in a 2- or 1-stage ring (see launch_schur_gemm).
 // A and B are read where the LU left them (column-major, interleaved complex), C lives in the
 // accumulators: it is loaded once, updated over the whole inner dimension, stored once.
 #include "common.cuh"
@@ -13,14 +13,13 @@
 
 namespace lsms {
 
-constexpr int BM = 64, BN = 64, KS = 16;
+constexpr int BM = 64, KS = 16;
 constexpr int LDA_S = BM + 2;      // complex units; == 2 (mod 8): conflict-free LDS.128 of A fragments
 constexpr int LDB_S = KS + 4;      // complex units; == 4 (mod 8): conflict-free LDS.128 of B fragments
 constexpr int A_STAGE = KS * LDA_S;        // complex elements
-constexpr int B_STAGE = BN * LDB_S;
-constexpr int STAGE_ELEMS = A_STAGE + B_STAGE;
-constexpr int GEMM_THREADS = 256;
-template <int STAGES> constexpr size_t gemm_smem() { return (size_t)STAGES * STAGE_ELEMS * sizeof(c128) + STAGES * sizeof(uint64_t); }
+// tile width BN = 64 with 256 threads (8 warps as 2 x 4) or BN = 32 with 128 threads (4 warps as 2 x 2); warp tile 32 x 16
+template <int BN> __host__ __device__ constexpr int stage_elems() { return A_STAGE + BN * LDB_S; }
+template <int STAGES, int BN> constexpr size_t gemm_smem() { return (size_t)STAGES * stage_elems<BN>() * sizeof(c128) + STAGES * sizeof(uint64_t); }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -52,12 +51,12 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 
 // Fill ring slot s with K-chunk kc of the A and B tiles: one bulk copy per tile column, issued by
 // threads 0..KS+BN-1; thread 0 also posts the expected byte count on the slot's mbarrier.
-template <int STAGES>
+template <int STAGES, int BN>
 __device__ __forceinline__ void issue_chunk(const GemmShape& g, const c128* A, const c128* B, c128* ring, uint64_t* full,
                                             int kc, int mvalid, int nvalid) {
     const int s = kc % STAGES, t = threadIdx.x;
     const int k0 = kc * KS, kvalid = min(KS, g.K - k0);
-    c128* As = ring + (size_t)s * STAGE_ELEMS;
+    c128* As = ring + (size_t)s * stage_elems<BN>();
     c128* Bs = As + A_STAGE;
     if (t == 0) mbar_expect_tx(&full[s], (uint32_t)((kvalid * mvalid + nvalid * kvalid) * sizeof(c128)));
     if (t < KS) {
@@ -70,12 +69,12 @@ __device__ __forceinline__ void issue_chunk(const GemmShape& g, const c128* A, c
     }
 }
 
-template <int STAGES>
-__global__ void __launch_bounds__(GEMM_THREADS, 2)
+template <int STAGES, int BN>
+__global__ void __launch_bounds__(BN * 4, 512 / (BN * 4))
 k_schur_gemm(GemmShape g, int tiles_m) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c128* ring = reinterpret_cast<c128*>(smem_raw);
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)STAGES * STAGE_ELEMS * sizeof(c128));
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)STAGES * stage_elems<BN>() * sizeof(c128));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tm = blockIdx.x % tiles_m, tn = blockIdx.x / tiles_m;
@@ -91,7 +90,7 @@ k_schur_gemm(GemmShape g, int tiles_m) {
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    for (int kc = 0; kc < STAGES && kc < nchunks; ++kc) issue_chunk<STAGES>(g, A, B, ring, full, kc, mvalid, nvalid);
+    for (int kc = 0; kc < STAGES && kc < nchunks; ++kc) issue_chunk<STAGES, BN>(g, A, B, ring, full, kc, mvalid, nvalid);
 
     // C tile -> accumulators (issued before the first wait so that it overlaps the TMA fill)
     const int gq = lane >> 2, q = lane & 3;              // fragment coordinates: A[gq][q], B[q][gq], C[gq][2q..2q+1]
@@ -113,7 +112,7 @@ k_schur_gemm(GemmShape g, int tiles_m) {
         const int s = kc % STAGES;
         mbar_wait(&full[s], (kc / STAGES) & 1);
         const int kvalid = min(KS, g.K - kc * KS);
-        const c128* As = ring + (size_t)s * STAGE_ELEMS;
+        const c128* As = ring + (size_t)s * stage_elems<BN>();
         const c128* Bs = As + A_STAGE;
         const int nfull = kvalid >> 2;
 #pragma unroll 1
@@ -157,7 +156,7 @@ k_schur_gemm(GemmShape g, int tiles_m) {
         }
         if (kc + STAGES < nchunks) {          // refill this slot once every warp is done with it
             __syncthreads();
-            issue_chunk<STAGES>(g, A, B, ring, full, kc + STAGES, mvalid, nvalid);
+            issue_chunk<STAGES, BN>(g, A, B, ring, full, kc + STAGES, mvalid, nvalid);
         }
     }
 
@@ -172,11 +171,11 @@ k_schur_gemm(GemmShape g, int tiles_m) {
             }
 }
 
-template <int STAGES>
+template <int STAGES, int BN>
 static int launch_classic(const GemmShape& g, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<STAGES>()));
+        LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<STAGES, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<STAGES, BN>()));
         attr_set = true;
     }
     const int tiles_m = (g.Mr + BM - 1) / BM, tiles_n = (g.Nc + BN - 1) / BN;
@@ -185,23 +184,25 @@ static int launch_classic(const GemmShape& g, cudaStream_t st) {
         h.A = g.A + (size_t)b0 * g.strideA; h.B = g.B + (size_t)b0 * g.strideB; h.C = g.C + (size_t)b0 * g.strideC;
         h.batch = g.batch - b0 < 65535 ? g.batch - b0 : 65535;
         dim3 grid((unsigned)(tiles_m * tiles_n), (unsigned)h.batch);
-        k_schur_gemm<STAGES><<<grid, GEMM_THREADS, gemm_smem<STAGES>(), st>>>(h, tiles_m);
+        k_schur_gemm<STAGES, BN><<<grid, BN * 4, gemm_smem<STAGES, BN>(), st>>>(h, tiles_m);
         LSMS_LAUNCH_CHECK();
     }
     return 0;
 }
 
-// K <= 16 is a single chunk: one ring stage (37 KB of shared memory instead of 112 KB) for the rank-IB updates
-// inside an outer panel.  Why two CTAs of 8 warps per SM: measured, one such CTA per SM reaches 21.8 of 36.9 TFLOP/s
-// (ptxas keeps the two products of an accumulator four DMMAs apart whatever the source order, and a warp then waits
-// on the DMMA result), two reach 34.2; the remaining 8 % is the time one of the two CTAs spends loading or storing
-// its C tile.  Tried and dropped: a one-DMMA-per-accumulator loop body with operands picked by 64-bit loads
+// Tile shapes.  K > 16 (Schur updates, triangular solve as GEMM): 64 x 32 tiles, 4 warps, 2-stage ring (54 KB), FOUR
+// CTAs per SM.  Why four small CTAs: ptxas keeps the two products of an accumulator four DMMAs apart whatever the
+// source order, and a warp then waits on the DMMA result, so the pipe needs about 3.4 warps per scheduler to stay
+// full (measured: 8 warps per SM reach 21.8 of 36.9 TFLOP/s, 16 warps 34.1).  With two 8-warp CTAs per SM the pipe
+// therefore starves whenever one of them loads or stores its C tile (92 % DMMA-active); with four 4-warp CTAs three
+// are still in their main loop: 34.6 TFLOP/s.  K <= 16 (rank-IB updates inside an outer panel): 64 x 64 tiles, one
+// ring stage.  Tried and dropped: a one-DMMA-per-accumulator loop body with operands picked by 64-bit loads
 // (31.7 TFLOP/s, bank-conflicted LDS.64) and a persistent one-CTA-per-SM variant with the next C tile prefetched
 // into shared memory (23.3 TFLOP/s).
 int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
     if (g.Mr <= 0 || g.Nc <= 0 || g.K <= 0 || g.batch <= 0) return 0;
-    if (g.K <= KS) return launch_classic<1>(g, st);
-    return launch_classic<3>(g, st);
+    if (g.K <= KS) return launch_classic<1, 64>(g, st);
+    return launch_classic<2, 32>(g, st);
 }
 
 }  // namespace lsms
