@@ -195,13 +195,13 @@ static int launch_classic(const GemmShape& g, cudaStream_t st) {
 // source order, and a warp then waits on the DMMA result, so the pipe needs about 3.4 warps per scheduler to stay
 // full (measured: 8 warps per SM reach 21.8 of 36.9 TFLOP/s, 16 warps 34.1).  With two 8-warp CTAs per SM the pipe
 // therefore starves whenever one of them loads or stores its C tile (92 % DMMA-active); with four 4-warp CTAs three
-// are still in their main loop: 34.6 TFLOP/s.  K <= 16 (rank-IB updates inside an outer panel): 64 x 64 tiles, one
-// ring stage.  Tried and dropped: a one-DMMA-per-accumulator loop body with operands picked by 64-bit loads
+// are still in their main loop: 34.6 TFLOP/s.  K <= 16 (rank-IB updates inside an outer panel, bound by the C-tile
+// traffic): the same 64 x 32 tiles with one ring stage (6.2 -> 4.9 ms per P step against 64 x 64 tiles).  Tried and dropped: a one-DMMA-per-accumulator loop body with operands picked by 64-bit loads
 // (31.7 TFLOP/s, bank-conflicted LDS.64) and a persistent one-CTA-per-SM variant with the next C tile prefetched
 // into shared memory (23.3 TFLOP/s).
 int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
     if (g.Mr <= 0 || g.Nc <= 0 || g.K <= 0 || g.batch <= 0) return 0;
-    if (g.K <= KS) return launch_classic<1, 64>(g, st);
+    if (g.K <= KS) return launch_classic<1, 32>(g, st);
     return launch_classic<2, 32>(g, st);
 }
 
