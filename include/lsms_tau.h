@@ -19,10 +19,15 @@
  *   - Rydberg atomic units: kappa = sqrt(z), Im kappa >= 0, lengths in Bohr
  *
  * Pointers are DEVICE pointers unless the name ends in _host.  The caller owns every
- * buffer, including the workspace; the library allocates nothing and keeps no state.
- * All device work is enqueued on `cuda_stream` (a cudaStream_t passed as void*) and the
+ * buffer, including the workspace; the library allocates no device memory.  Its only
+ * persistent objects are the internal streams and events of lsms_tau00_batched's scheduler
+ * (look-ahead and batch-group streams, created on first use) and the process-wide tuning
+ * knobs below.  All device work is ordered after what is already enqueued on `cuda_stream`
+ * (a cudaStream_t passed as void*), later work on `cuda_stream` is ordered after it, and the
  * calls return without synchronising (the *_host entry point synchronises the stream
- * before returning because it hands results back in host memory).
+ * before returning because it hands results back in host memory).  Because the internal
+ * streams are shared, calls from several host threads must be serialised by the caller;
+ * successive calls on different caller streams are correct and run one after the other.
  *
  * Return value (LAPACK-like): 0 = enqueued; -i = i-th argument invalid (null pointer,
  * out-of-range size, workspace too small, pointer not 16-byte aligned); >0 = CUDA runtime
