@@ -160,6 +160,7 @@ def main() -> None:
     ap.add_argument("--no-lookahead", action="store_true", help="factor the next panel in front of, not under, the update")
     ap.add_argument("--panel", type=int, default=1, help="K2 variant: 1 register-blocked 512/256 thr, 0 256 thr, -1 L2-resident")
     ap.add_argument("--no-align", action="store_true", help="every outer panel NB wide (no tile-aligning first panel)")
+    ap.add_argument("--shared-g0", action="store_true", help="SURVEY 8(f) f3: assemble with one g0 per energy shared by all atoms")
     ap.add_argument("--groups", type=int, default=0, help="batch groups on separate streams (0 = library default)")
     args = ap.parse_args()
     cfg = sl.CONFIGS[args.workload]
@@ -208,8 +209,12 @@ def main() -> None:
     def step():
         lt.lsms_tinv_from_phase_shifts(delta, species, z, cfg.lmax, cfg.n_sites, cfg.spin_canted, 2, B, tinv, kappa, stream)
         c = lt.lsms_last_launch_count()
-        lt.lsms_build_M_batched(tinv, pos, mom if cfg.spin_canted else None, kappa, cfg.lmax, cfg.n_sites, cfg.spin_canted,
-                                B, M, ws, stream)
+        if args.shared_g0:
+            lt.lsms_build_M_shared_g0_batched(tinv, pos, mom if cfg.spin_canted else None, kappa, cfg.lmax, cfg.n_sites,
+                                              cfg.spin_canted, cfg.n_atoms, cfg.n_energies, M, ws, stream)
+        else:
+            lt.lsms_build_M_batched(tinv, pos, mom if cfg.spin_canted else None, kappa, cfg.lmax, cfg.n_sites, cfg.spin_canted,
+                                    B, M, ws, stream)
         c += lt.lsms_last_launch_count()
         lt.lsms_tau00_batched(M, cfg.n_sites, cfg.kmax, cfg.spin_canted, B, tau, info, ws, stream)
         launches[0] = c + lt.lsms_last_launch_count()
@@ -350,7 +355,8 @@ def main() -> None:
             "tflops": tflops, "tflops_convention": "8/3 n^3 per matrix",
             "frac_fp64_peak": tflops / peak_fp64 if peak_fp64 else None,
             "schedule": {"groups": args.groups or "auto (2)", "lookahead": not args.no_lookahead, "panel_variant": args.panel,
-                         "nb": args.nb or 64, "ib": args.ib or 16, "align_first_panel": not args.no_align},
+                         "nb": args.nb or 64, "ib": args.ib or 16, "align_first_panel": not args.no_align,
+                         "assembly": "one g0 per energy shared by all atoms (f3)" if args.shared_g0 else "every item assembled independently"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_timed,
             "roofline": roofline, "cpu_baseline": cpu_baseline,
         }))

@@ -87,6 +87,19 @@ int lsms_build_M_batched(const lsms_c128* tinv_diag, const double* site_pos, con
                          const lsms_c128* kappa, int lmax, int n_sites, int spin_canted, int batch,
                          lsms_c128* M_out, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* de-duplicated assembly.  g0 depends on the LIZ geometry and on kappa only, so when the batch
+ * is (central atoms) x (energies) on one lattice (reading A19: item = atom * n_energies + energy) and every atom's
+ * LIZ has the same site positions, each g0 block is evaluated once per energy and stored into the matrices of all
+ * n_atoms atoms; only the site-diagonal t^{-1} blocks (and moments) are per item.  Arguments as for
+ * lsms_build_M_batched with batch = n_atoms * n_energies, except that site_pos and kappa are READ FOR ATOM 0 ONLY
+ * (items 0 .. n_energies-1): the caller guarantees site_pos[a][e] == site_pos[0][e] and kappa[a][e] == kappa[0][e].
+ * The result is bit-identical to lsms_build_M_batched on such input.
+ * Errors: -1..-4 null inputs, -5 lmax, -6 n_sites, -8 n_atoms, -9 n_energies, -10 M_out, -11/-12 workspace.        */
+int lsms_build_M_shared_g0_batched(const lsms_c128* tinv_diag, const double* site_pos, const double* moment_dir,
+                                   const lsms_c128* kappa, int lmax, int n_sites, int spin_canted,
+                                   int n_atoms, int n_energies,
+                                   lsms_c128* M_out, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* tau^{00}_b = central-site k x k block of M_b^{-1} by a blocked right-looking
  * LU with panel partial pivoting restricted to the non-central rows; the trailing k x k block after
  * n-k columns is the Schur complement of the central site and tau^{00} is its inverse (no

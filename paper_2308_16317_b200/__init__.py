@@ -17,7 +17,7 @@ _lib = None
 
 EXPORTS = (
     "lsms_version", "lsms_workspace_bytes", "lsms_solve_workspace_bytes", "lsms_host_call_scratch_bytes",
-    "lsms_tinv_from_phase_shifts", "lsms_build_M_batched", "lsms_tau00_batched",
+    "lsms_tinv_from_phase_shifts", "lsms_build_M_batched", "lsms_build_M_shared_g0_batched", "lsms_tau00_batched",
     "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_contour_sum_batched", "lsms_set_blocking", "lsms_set_lookahead", "lsms_set_groups", "lsms_set_panel_variant", "lsms_set_align_first",
     "lsms_last_launch_count", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe", "lsms_schur_update_batched",
     "lsms_debug_gaunt_closed_form",
@@ -46,6 +46,7 @@ def lib() -> ctypes.CDLL:
         L.lsms_host_call_scratch_bytes.argtypes = [ci, ci, ci, ci, ci]
         L.lsms_tinv_from_phase_shifts.argtypes = [vp, vp, vp, ci, ci, ci, ci, ci, vp, vp, vp]
         L.lsms_build_M_batched.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, vp, vp, sz, vp]
+        L.lsms_build_M_shared_g0_batched.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ci, vp, vp, sz, vp]
         L.lsms_tau00_batched.argtypes = [vp, ci, ci, ci, ci, vp, vp, vp, sz, vp]
         L.lsms_solve_central_column_batched.argtypes = [vp, ci, ci, ci, ci, vp, vp, vp, sz, vp]
         L.lsms_tau00_from_host.argtypes = [vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, vp, vp, vp, sz, vp,
@@ -176,6 +177,23 @@ def lsms_build_M_batched(tinv_diag, site_pos, moment_dir, kappa, lmax, n_sites, 
     _check(lib().lsms_build_M_batched(_ptr(tinv_diag), _ptr(site_pos), _ptr(moment_dir), _ptr(kappa), lmax, n_sites,
                                       int(bool(spin_canted)), batch, _ptr(M_out), _ptr(workspace), workspace.numel(),
                                       _stream(stream)), "lsms_build_M_batched")
+    return M_out
+
+
+def lsms_build_M_shared_g0_batched(tinv_diag, site_pos, moment_dir, kappa, lmax, n_sites, spin_canted, n_atoms, n_energies,
+                                   M_out=None, workspace=None, stream=None):
+    """De-duplicated assembly (one g0 per energy for all atoms); same outputs as lsms_build_M_batched."""
+    import torch
+    k = (lmax + 1) ** 2 * (2 if spin_canted else 1)
+    n = n_sites * k
+    batch = n_atoms * n_energies
+    if M_out is None:
+        M_out = torch.empty((batch, n, n), dtype=torch.complex128, device=kappa.device)
+    if workspace is None:
+        workspace = _workspace(lsms_workspace_bytes(n_sites, lmax, spin_canted, batch), kappa.device)
+    _check(lib().lsms_build_M_shared_g0_batched(_ptr(tinv_diag), _ptr(site_pos), _ptr(moment_dir), _ptr(kappa), lmax, n_sites,
+                                                int(bool(spin_canted)), n_atoms, n_energies, _ptr(M_out), _ptr(workspace),
+                                                workspace.numel(), _stream(stream)), "lsms_build_M_shared_g0_batched")
     return M_out
 
 

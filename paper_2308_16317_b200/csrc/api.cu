@@ -299,7 +299,27 @@ int lsms_build_M_batched(const lsms_c128* tinv_diag, const double* site_pos, con
     g_launches.n = 0;
     ProfScope ps(0, (cudaStream_t)cuda_stream);
     return launch_assemble((const c128*)tinv_diag, site_pos, moment_dir, (const c128*)kappa, lmax, n_sites,
-                           spin_canted ? 1 : 0, batch, (c128*)M_out, workspace, (cudaStream_t)cuda_stream);
+                           spin_canted ? 1 : 0, batch, 1, (c128*)M_out, workspace, (cudaStream_t)cuda_stream);
+}
+
+int lsms_build_M_shared_g0_batched(const lsms_c128* tinv_diag, const double* site_pos, const double* moment_dir,
+                                   const lsms_c128* kappa, int lmax, int n_sites, int spin_canted, int n_atoms, int n_energies,
+                                   lsms_c128* M_out, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!tinv_diag || !aligned16(tinv_diag)) return -1;
+    if (!site_pos) return -2;
+    if (spin_canted && !moment_dir) return -3;
+    if (!kappa || !aligned16(kappa)) return -4;
+    if (lmax < 0 || lmax > 8) return -5;
+    if (n_sites < 1) return -6;
+    if (n_atoms < 1) return -8;
+    if (n_energies < 1) return -9;
+    if (!M_out || !aligned16(M_out)) return -10;
+    if (!workspace || !aligned16(workspace)) return -11;
+    if (workspace_bytes < align256(gaunt_table_bytes(lmax))) return -12;
+    g_launches.n = 0;
+    ProfScope ps(0, (cudaStream_t)cuda_stream);
+    return launch_assemble((const c128*)tinv_diag, site_pos, moment_dir, (const c128*)kappa, lmax, n_sites,
+                           spin_canted ? 1 : 0, n_energies, n_atoms, (c128*)M_out, workspace, (cudaStream_t)cuda_stream);
 }
 
 int lsms_tau00_batched(lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,

@@ -132,18 +132,21 @@ __global__ void k_legendre_table(int l2, double* __restrict__ leg) {
 // Row sites are processed in chunks that fit shared memory.
 constexpr int ASM_THREADS = 256;
 
-template <int MAXNT>       // >= l_max + 1: length of the per-thread Gaunt term arrays
+template <int MAXNT, bool REP>   // MAXNT >= l_max + 1: length of the per-thread Gaunt term arrays; REP: shared-g0 mode (n_rep >= 1 items per CTA)
 __global__ void __launch_bounds__(ASM_THREADS)
 k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, const double* __restrict__ moment,
            const c128* __restrict__ kappa, const c128* __restrict__ coef, const int* __restrict__ idx,
-           const double* __restrict__ leg, int lmax, int n_sites, int canted, int chunk, c128* __restrict__ Mout) {
+           const double* __restrict__ leg, int lmax, int n_sites, int canted, int chunk, int n_rep, int rep_stride,
+           c128* __restrict__ Mout) {
     extern __shared__ __align__(16) unsigned char asm_smem[];
     const int kmax = (lmax + 1) * (lmax + 1), nt = lmax + 1, l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
     const int nspin = canted ? 2 : 1, k = kmax * nspin, kk2 = kmax * kmax, S = nl2;
     const size_t n = (size_t)n_sites * k;
     const int b = blockIdx.y, sj = blockIdx.x, tid = threadIdx.x;
     c128* hY = reinterpret_cast<c128*>(asm_smem);                 // [chunk][nl2]
-    c128* M = Mout + (size_t)b * n * n;
+    c128* M = Mout + (size_t)b * n * n;          // item b; items b + a*rep_stride, a < n_rep, share its geometry and kappa
+    const size_t rep_elems = (size_t)rep_stride * n * n;
+    const int nrep = REP ? n_rep : 1;
     const size_t c0 = (size_t)(sj == 0 ? n_sites - 1 : sj - 1) * k;
     const c128 kap = kappa[b];
     const c128 zero = cmake(0.0, 0.0);
@@ -223,26 +226,34 @@ k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, c
                         c128 g = zero;
 #pragma unroll
                         for (int t = 0; t < MAXNT; ++t) if (nz[t]) cfma(g, cf[t], hy[ix[t]]);
-                        colp[rowb] = g;
-                        if (canted) {
-                            colp[rowb + kmax] = zero;                                   // (down, up)
-                            colp[rowb + n * kmax] = zero;                               // (up, down)
-                            colp[rowb + n * kmax + kmax] = g;                           // (down, down): g0 (x) 1_2
+                        // g0 depends on the geometry and kappa only: one evaluation serves every item that shares them
+                        for (int a = 0; a < nrep; ++a) {
+                            c128* cp = colp + (size_t)a * rep_elems;
+                            cp[rowb] = g;
+                            if (canted) {
+                                cp[rowb + kmax] = zero;                                   // (down, up)
+                                cp[rowb + n * kmax] = zero;                               // (up, down)
+                                cp[rowb + n * kmax + kmax] = g;                           // (down, down): g0 (x) 1_2
+                            }
                         }
                     } else {
                         // site-diagonal block: t^{-1} (g0^{ii} = 0, "between two different atom sites")
-                        const c128* ti = tinv + ((size_t)b * n_sites + si) * nspin * nt;
                         const bool dg = (L == Lp);
-                        if (!canted) {
-                            colp[rowb] = dg ? ti[lL] : zero;
-                        } else {
-                            const double* mv = moment + ((size_t)b * n_sites + si) * 3;
-                            const c128 a = ti[lL], bb = ti[nt + lL];
-                            const c128 hsum = cscale(0.5, cadd(a, bb)), hdif = cscale(0.5, csub(a, bb));
-                            colp[rowb] = dg ? cadd(hsum, cscale(mv[2], hdif)) : zero;                         // (up, up)
-                            colp[rowb + kmax] = dg ? cmul(hdif, cmake(mv[0], mv[1])) : zero;                  // (down, up): ex + i ey
-                            colp[rowb + n * kmax] = dg ? cmul(hdif, cmake(mv[0], -mv[1])) : zero;             // (up, down): ex - i ey
-                            colp[rowb + n * kmax + kmax] = dg ? csub(hsum, cscale(mv[2], hdif)) : zero;       // (down, down)
+                        for (int a = 0; a < nrep; ++a) {
+                            const size_t item = (size_t)b + (size_t)a * rep_stride;
+                            const c128* ti = tinv + (item * n_sites + si) * nspin * nt;
+                            c128* cp = colp + (size_t)a * rep_elems;
+                            if (!canted) {
+                                cp[rowb] = dg ? ti[lL] : zero;
+                            } else {
+                                const double* mv = moment + (item * n_sites + si) * 3;
+                                const c128 ta = ti[lL], tb = ti[nt + lL];
+                                const c128 hsum = cscale(0.5, cadd(ta, tb)), hdif = cscale(0.5, csub(ta, tb));
+                                cp[rowb] = dg ? cadd(hsum, cscale(mv[2], hdif)) : zero;                         // (up, up)
+                                cp[rowb + kmax] = dg ? cmul(hdif, cmake(mv[0], mv[1])) : zero;                  // (down, up): ex + i ey
+                                cp[rowb + n * kmax] = dg ? cmul(hdif, cmake(mv[0], -mv[1])) : zero;             // (up, down): ex - i ey
+                                cp[rowb + n * kmax + kmax] = dg ? csub(hsum, cscale(mv[2], hdif)) : zero;       // (down, down)
+                            }
                         }
                     }
                 }
@@ -271,8 +282,10 @@ int launch_tinv(const c128* delta, const int* species, const c128* z, int lmax, 
     return 0;
 }
 
+// n_rep > 1: de-duplicated assembly -- `batch` then counts the DISTINCT (geometry, kappa) items (the energies); item
+// e + a*batch, a < n_rep, shares the geometry and kappa of item e and differs in tinv / moments only.
 int launch_assemble(const c128* tinv, const double* site_pos, const double* moment, const c128* kappa, int lmax,
-                    int n_sites, int canted, int batch, c128* M, void* ws, cudaStream_t st) {
+                    int n_sites, int canted, int batch, int n_rep, c128* M, void* ws, cudaStream_t st) {
     size_t kmax = (size_t)(lmax + 1) * (lmax + 1), nt = lmax + 1, e = kmax * kmax * nt;
     const int l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
     c128* coef = (c128*)ws;
@@ -298,14 +311,19 @@ int launch_assemble(const c128* tinv, const double* site_pos, const double* mome
             kern<<<grid, ASM_THREADS, smem, st>>>(tinv + (size_t)b0 * n_sites * (canted ? 2 : 1) * nt,
                                                   site_pos + (size_t)b0 * n_sites * 3,
                                                   moment ? moment + (size_t)b0 * n_sites * 3 : nullptr, kappa + b0, coef, idx, leg,
-                                                  lmax, n_sites, canted, chunk, M + (size_t)b0 * n * n);
+                                                  lmax, n_sites, canted, chunk, n_rep, batch, M + (size_t)b0 * n * n);
             LSMS_LAUNCH_CHECK();
         }
         return 0;
     };
-    if (lmax <= 3) return run(k_assemble<4>);
-    if (lmax == 4) return run(k_assemble<5>);
-    return run(k_assemble<9>);
+    if (n_rep > 1) {
+        if (lmax <= 3) return run(k_assemble<4, true>);
+        if (lmax == 4) return run(k_assemble<5, true>);
+        return run(k_assemble<9, true>);
+    }
+    if (lmax <= 3) return run(k_assemble<4, false>);
+    if (lmax == 4) return run(k_assemble<5, false>);
+    return run(k_assemble<9, false>);
 }
 
 }  // namespace lsms

@@ -12,7 +12,7 @@ double gaunt_closed_form_host(int l, int m, int lp, int mp, int lpp);
 int launch_tinv(const c128* delta, const int* species, const c128* z, int lmax, int n_sites, int nspin, int batch,
                 c128* tinv, c128* kappa, cudaStream_t st);
 int launch_assemble(const c128* tinv, const double* site_pos, const double* moment, const c128* kappa, int lmax,
-                    int n_sites, int canted, int batch, c128* M, void* ws, cudaStream_t st);
+                    int n_sites, int canted, int batch, int n_rep, c128* M, void* ws, cudaStream_t st);
 
 // gemm.cu -- K4: C[Mr x Nc] -= A[Mr x K] * B[K x Nc] inside the same column-major matrices (ld = n)
 struct GemmShape {

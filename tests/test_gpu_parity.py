@@ -108,6 +108,25 @@ def test_assembly_small_lmax_range(lt):
             assert block_rel_err(Mg[i], oracle_M(batch, i), cfg.k) < ASM_TOL
 
 
+def test_shared_g0_assembly_is_identical_to_per_item_assembly(lt):
+    """one g0 evaluation per energy shared by all central atoms of a lattice.  Same arithmetic per
+    element, so the matrices must be bit-identical to the per-item assembly (which is itself checked against the
+    oracle above); plain and spin-canted (per-item moments and t^-1 on the site diagonal), and one oracle block check."""
+    for cfg in (sl.custom_config(19, 3, False, n_atoms=3, n_energies=5), sl.custom_config(13, 2, True, n_atoms=4, n_energies=3),
+                sl.custom_config(13, 4, False, n_atoms=2, n_energies=2)):
+        batch = sl.make_batch(cfg)
+        delta, species, z, pos, mom = lt.device_inputs(batch)
+        tinv, kappa = lt.lsms_tinv_from_phase_shifts(delta, species, z, cfg.lmax, cfg.n_sites, cfg.spin_canted, 2, batch.batch)
+        momd = mom if cfg.spin_canted else None
+        M_item = lt.lsms_build_M_batched(tinv, pos, momd, kappa, cfg.lmax, cfg.n_sites, cfg.spin_canted, batch.batch)
+        M_shared = lt.lsms_build_M_shared_g0_batched(tinv, pos, momd, kappa, cfg.lmax, cfg.n_sites, cfg.spin_canted,
+                                                     cfg.n_atoms, cfg.n_energies)
+        torch.cuda.synchronize()
+        assert torch.equal(torch.view_as_real(M_item), torch.view_as_real(M_shared))
+        b = batch.batch - 1                                         # last atom, last energy
+        assert block_rel_err(M_shared[b].cpu().numpy().T, oracle_M(batch, b), cfg.k) < ASM_TOL
+
+
 # ------------------------------------------------------------------ whole path, element-wise
 
 def test_tau00_tiny_full_batch(lt):
