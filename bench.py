@@ -161,6 +161,7 @@ def main() -> None:
     ap.add_argument("--panel", type=int, default=1, help="K2 variant: 1 register-blocked 512/256 thr, 0 256 thr, -1 L2-resident")
     ap.add_argument("--no-align", action="store_true", help="every outer panel NB wide (no tile-aligning first panel)")
     ap.add_argument("--shared-g0", action="store_true", help="SURVEY 8(f) f3: assemble with one g0 per energy shared by all atoms")
+    ap.add_argument("--panel-cluster", type=int, default=0, help="CTAs per matrix in the panel kernel: 0 auto, 1 never, 2/4/8")
     ap.add_argument("--groups", type=int, default=0, help="batch groups on separate streams (0 = library default)")
     args = ap.parse_args()
     cfg = sl.CONFIGS[args.workload]
@@ -190,6 +191,7 @@ def main() -> None:
     lt.lsms_set_lookahead(not args.no_lookahead)
     lt.lsms_set_groups(args.groups)
     lt.lsms_set_panel_variant(args.panel)
+    lt.lsms_set_panel_cluster(args.panel_cluster)
     lt.lsms_set_align_first(not args.no_align)
 
     # ---- inputs: every rank gets its own central atoms (weak scaling: per-GPU work fixed)

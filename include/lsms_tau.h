@@ -170,6 +170,12 @@ int lsms_set_groups(int groups);
  * the lowest row) and perform the same arithmetic per element.  Errors: -1 out of range. */
 int lsms_set_panel_variant(int variant);
 
+/* CTAs per matrix in the panel kernel (thread-block cluster, rows dealt round-robin, exchange through distributed
+ * shared memory): 0 (default) chosen per shape -- 8 (4) CTAs for batches of one or two matrices while the panel is
+ * taller than 4096 (2048) rows, else one: under look-ahead a cluster has to wait for co-scheduled SMs and larger
+ * batches lose --, 1 never, 2 / 4 / 8 forced.  Same pivots and arithmetic as the one-CTA kernel.  Errors: -1. */
+int lsms_set_panel_cluster(int cl);
+
 /* Tile alignment (default on): the first outer panel is n mod 64 columns wide, so that all later trailing
  * matrices are whole multiples of the 64 x 64 Schur-update tile.  Off: every panel is NB wide. */
 int lsms_set_align_first(int on);

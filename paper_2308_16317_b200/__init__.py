@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "lsms_version", "lsms_workspace_bytes", "lsms_solve_workspace_bytes", "lsms_host_call_scratch_bytes",
     "lsms_tinv_from_phase_shifts", "lsms_build_M_batched", "lsms_build_M_shared_g0_batched", "lsms_tau00_batched",
-    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_contour_sum_batched", "lsms_set_blocking", "lsms_set_lookahead", "lsms_set_groups", "lsms_set_panel_variant", "lsms_set_align_first",
+    "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_contour_sum_batched", "lsms_set_blocking", "lsms_set_lookahead", "lsms_set_groups", "lsms_set_panel_variant", "lsms_set_panel_cluster", "lsms_set_align_first",
     "lsms_last_launch_count", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe", "lsms_schur_update_batched",
     "lsms_debug_gaunt_closed_form",
 )
@@ -103,6 +103,10 @@ def lsms_set_lookahead(on: bool = True) -> None:
 
 def lsms_set_panel_variant(variant: int = 1) -> None:
     _check(lib().lsms_set_panel_variant(int(variant)), "lsms_set_panel_variant")
+
+
+def lsms_set_panel_cluster(cl: int = 0) -> None:
+    _check(lib().lsms_set_panel_cluster(int(cl)), "lsms_set_panel_cluster")
 
 
 def lsms_set_align_first(on: bool = True) -> None:

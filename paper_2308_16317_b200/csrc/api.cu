@@ -108,6 +108,23 @@ static int ensure_streams(int groups) {
     return 0;
 }
 
+static int g_panel_cluster = 0;            // 0 = chosen per shape, 1 = never, 2/4/8 = forced
+// CTAs per matrix for the panel kernel.  A cluster shortens the panel factorisation of a tall panel several times
+// (rank 12450, 12 matrices: 303 -> 117 ms per step when timed alone), but its CTAs must be co-scheduled on free SMs, so
+// under look-ahead it waits for the Schur update to drain instead of running beneath it and whole steps of batches
+// >= 4 got SLOWER (NC 1897 -> 1928 ms, H 629 -> 654, C 440 -> 465, P 121 -> 129).  It pays when there is next to
+// nothing to overlap with: one or two tall matrices (rank 12450, batch 1: 369 -> 223 ms; rank 4320: 36.9 -> 32.5 ms).
+static int panel_cluster_size(int m, int batch) {
+    if (g_panel_variant < 1) return 1;
+    if (g_panel_cluster == 1) return 1;
+    int cl = 1;
+    if (g_panel_cluster > 1) cl = g_panel_cluster;
+    else if (batch <= 2 && m >= 4096) cl = 8;
+    else if (batch <= 2 && m >= 2048) cl = 4;
+    if (cl > 1 && (m + cl - 1) / cl > 5120) cl = 1;         // taller than the cluster instances cover: one-CTA kernel
+    return cl;
+}
+
 // factor the outer panel [J, J+W) on stream st: inner panels of width <= IB
 static int factor_panel(c128* M, int n, int batch, int J, int W, int ne, int IB, int* piv, int* info, cudaStream_t st) {
     const size_t stride = (size_t)n * n;
@@ -119,7 +136,11 @@ static int factor_panel(c128* M, int n, int batch, int J, int W, int ne, int IB,
         if (g_panel_variant >= 0 && n - c0 <= 16384) {
             // register-blocked K2: factors the inner panel, applies its interchanges to the whole outer panel and
             // solves the w x w triangle for the outer panel's columns to the right
-            { ProfScope ps(1, st); rc = launch_panel_reg(M, stride, n, J, W, c0, w, ne, batch, piv, info, g_panel_variant, st); } if (rc) return rc;
+            // small batches of tall panels: a cluster of CTAs per matrix, so that the panel phase spans the chip too
+            const int cl = panel_cluster_size(n - c0, batch);
+            if (cl > 1) { ProfScope ps(1, st); rc = launch_panel_cluster(M, stride, n, J, W, c0, w, ne, batch, piv, info, cl, st); }
+            else { ProfScope ps(1, st); rc = launch_panel_reg(M, stride, n, J, W, c0, w, ne, batch, piv, info, g_panel_variant, st); }
+            if (rc) return rc;
         } else {
             { ProfScope ps(1, st); rc = launch_panel(M, stride, n, c0, w, ne, batch, piv, info, st); } if (rc) return rc;
             { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, J, c0, 1, batch, piv, st); } if (rc) return rc;
@@ -465,6 +486,12 @@ int lsms_set_blocking(int nb_outer, int ib_inner) {
 int lsms_set_lookahead(int on) { g_lookahead = on ? 1 : 0; return 0; }
 
 int lsms_set_align_first(int on) { g_align_first = on ? 1 : 0; return 0; }
+
+int lsms_set_panel_cluster(int cl) {
+    if (cl != 0 && cl != 1 && cl != 2 && cl != 4 && cl != 8) return -1;
+    g_panel_cluster = cl;
+    return 0;
+}
 
 int lsms_set_panel_variant(int variant) {
     if (variant < -1 || variant > 1) return -1;

@@ -32,6 +32,9 @@ int launch_swap_trsm(c128* base, size_t stride, int n, int c0, int w, int col_lo
 // panel.cu -- K2 with the sub-panel in registers; also applies the interchanges to the whole outer panel [J, J+Wout)
 int launch_panel_reg(c128* base, size_t stride, int n, int J, int Wout, int c0, int w, int ne, int batch, int* piv, int* info,
                      int variant, cudaStream_t st);
+// panel_cluster.cu -- the same with a cluster of cl CTAs per matrix (small batches of tall panels)
+int launch_panel_cluster(c128* base, size_t stride, int n, int J, int Wout, int c0, int w, int ne, int batch, int* piv, int* info,
+                         int cl, cudaStream_t st);
 int launch_panel_post(const c128* base, size_t stride, int n, int J, int W, int batch, const int* piv, int* perm, c128* ninv,
                       int nbmax, cudaStream_t st);
 int launch_row_permute(c128* base, size_t stride, int n, int J, int W, int col_lo, int col_hi, int batch, const int* perm,

@@ -1,0 +1,325 @@
+// panel_cluster.cu -- K2 for tall panels of SMALL batches: one thread-block CLUSTER per matrix
+// ("lets large ones span the whole chip"; PAPER.md:92 LU; pivot rule: reading A14).
+//
+// With one CTA per matrix (panel.cu) a batch of 12 rank-12450 matrices keeps 12 of the 148 SMs busy during the
+// panel factorisation, and each CTA's rows-per-thread count forces 1-column sub-panels.  Here the rows of a panel
+// are dealt round-robin to the CL CTAs of a cluster (CL = 2, 4 or 8; global thread g = rank*THREADS + tid owns
+// rows c0 + g + r*CL*THREADS), so the sub-panel stays 4 columns wide and CL times as many SMs pull the panel
+// through their load/store units.  Same algorithm and arithmetic as k_panel_reg; what crosses CTAs goes through
+// distributed shared memory, every CTA keeping a full copy of the small shared state:
+//   * arg-max: each warp writes its candidate into slot [rank][warp] of EVERY CTA, one cluster barrier, then every
+//     thread reduces the CL*NW candidates itself (same result everywhere, no broadcast step);
+//   * pivot row / row j, L11, the rows of U: written by their owner into every CTA's copy;
+//   * the interchanges of the outer panel's other columns and the final w x w solve are done by rank 0.
+// Barriers per column step: two cluster barriers (arrive.release / wait.acquire, which also order the global-memory
+// traffic between the CTAs of the cluster).
+#include "common.cuh"
+#include "internal.h"
+
+namespace lsms {
+
+constexpr int PC_MAXW = 16;       // inner panel width limit
+constexpr int PC_MAXOUT = 128;    // outer panel width limit
+constexpr int PC_MAXCL = 8;       // portable cluster size limit
+
+__device__ __forceinline__ uint32_t pc_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t pc_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t pc_nranks() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void pc_sync() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// address of the same shared variable in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t pc_map(const void* p, uint32_t rank) {
+    uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(pc_smem_u32(p)), "r"(rank)); return r;
+}
+__device__ __forceinline__ void pc_st_c128(uint32_t addr, c128 v) {
+    asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void pc_st_f64(uint32_t addr, double v) { asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
+__device__ __forceinline__ void pc_st_s32(uint32_t addr, int v) { asm volatile("st.shared::cluster.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
+// store v into the copy of *p held by every CTA of the cluster (including this one)
+__device__ __forceinline__ void pc_bcast_c128(c128* p, c128 v, uint32_t ncl) { for (uint32_t k = 0; k < ncl; ++k) pc_st_c128(pc_map(p, k), v); }
+
+template <int THREADS, int R, int S>
+__global__ void __launch_bounds__(THREADS, (THREADS <= 256) ? 2 : 1)
+k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int c0, int w, int ne,
+            int* __restrict__ piv, int* __restrict__ info) {
+    constexpr int NW = THREADS / 32;
+    const uint32_t rank = pc_rank(), ncl = pc_nranks();
+    const int item = blockIdx.x / ncl;
+    c128* A = base + (size_t)item * stride;
+    int* pv = piv + (size_t)item * n;
+    __shared__ double red_v[PC_MAXCL * NW];
+    __shared__ int red_i[PC_MAXCL * NW];
+    __shared__ c128 prow[S], jrow[S];
+    __shared__ c128 L11[S * S];                 // L11[i*S + q] = multiplier of row cs+i, column cs+q (q < i)
+    __shared__ c128 Us[S * PC_MAXW];            // Us[q*PC_MAXW + c] = U(cs+q, cs+sw+c)
+    __shared__ int spiv[S], canon[S];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int TT = THREADS * (int)ncl;          // threads per matrix
+    const int g0 = (int)rank * THREADS + tid;   // global thread index inside the cluster
+    const int ncand = NW * (int)ncl;
+    const c128 zero = cmake(0.0, 0.0);
+
+    for (int s0 = 0; s0 < w; s0 += S) {
+        const int cs = c0 + s0, sw = min(S, w - s0);
+        // ---- 1: sub-panel -> registers
+        c128 v[R][S];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int row = c0 + g0 + r * TT;
+#pragma unroll
+            for (int q = 0; q < S; ++q) v[r][q] = (row < n && q < sw) ? A[row + (size_t)(cs + q) * n] : zero;
+        }
+        // ---- 2: column steps
+#pragma unroll
+        for (int q = 0; q < S; ++q) {
+            if (q < sw) {
+                const int j = cs + q;
+                double bv = -1.0; int bi = 0x7fffffff;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int row = c0 + g0 + r * TT;
+                    const double a = cabs1(v[r][q]);
+                    if (row >= j && row < ne && a > bv) { bv = a; bi = row; }
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    const double ov = __shfl_xor_sync(0xffffffffu, bv, o); const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+                }
+                // every warp publishes its candidate in every CTA's table: lane k < ncl writes to CTA k
+                if (lane < (int)ncl) {
+                    pc_st_f64(pc_map(&red_v[rank * NW + warp], lane), bv);
+                    pc_st_s32(pc_map(&red_i[rank * NW + warp], lane), bi);
+                }
+                pc_sync();
+                bv = -1.0; bi = 0x7fffffff;
+                for (int e = lane; e < ncand; e += 32) {
+                    const double ov = red_v[e]; const int oi = red_i[e];
+                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    const double ov = __shfl_xor_sync(0xffffffffu, bv, o); const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+                }
+                const bool bad = !(bv > 0.0) || !(bv < 1.0e300 * 1.0e300);     // zero, NaN or Inf pivot
+                const int p = bad ? j : bi;
+                if (tid == 0) {
+                    spiv[q] = p;
+                    if (rank == 0) { pv[j] = p; if (bad) atomicCAS(&info[item], 0, j + 1); }
+                }
+                // ---- pivot row and row j into every CTA's copy
+                const int gj = (j - c0) % TT, rj = (j - c0) / TT;
+                const int gp = (p - c0) % TT, rp_ = (p - c0) / TT;
+                if (g0 == gp) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) if (r == rp_) {
+#pragma unroll
+                        for (int t = 0; t < S; ++t) pc_bcast_c128(&prow[t], v[r][t], ncl);
+                    }
+                }
+                if (p != j && g0 == gj) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) if (r == rj) {
+#pragma unroll
+                        for (int t = 0; t < S; ++t) pc_bcast_c128(&jrow[t], v[r][t], ncl);
+                    }
+                }
+                pc_sync();
+                if (p != j) {
+                    if (g0 == gj) {
+#pragma unroll
+                        for (int r = 0; r < R; ++r) if (r == rj) {
+#pragma unroll
+                            for (int t = 0; t < S; ++t) v[r][t] = prow[t];
+                        }
+                    }
+                    if (g0 == gp) {
+#pragma unroll
+                        for (int r = 0; r < R; ++r) if (r == rp_) {
+#pragma unroll
+                            for (int t = 0; t < S; ++t) v[r][t] = jrow[t];
+                        }
+                    }
+                }
+                // ---- scale column j and rank-1 update of the sub-panel's remaining columns
+                if (!bad) {
+                    const c128 rp = crecip(prow[q]);
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const int row = c0 + g0 + r * TT;
+                        if (row > j && row < n) {
+                            const c128 l = cmul(v[r][q], rp);
+                            v[r][q] = l;
+#pragma unroll
+                            for (int t = q + 1; t < S; ++t) if (t < sw) cfms(v[r][t], l, prow[t]);
+                        }
+                    }
+                }
+            }
+        }
+        // ---- 3: store the sub-panel (rows above cs hold finished U entries and are unchanged); L11 to every CTA
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int row = c0 + g0 + r * TT;
+            if (row >= cs && row < n) {
+#pragma unroll
+                for (int q = 0; q < S; ++q) if (q < sw) A[row + (size_t)(cs + q) * n] = v[r][q];
+                if (row < cs + sw) {
+#pragma unroll
+                    for (int q = 0; q < S; ++q) pc_bcast_c128(&L11[(row - cs) * S + q], v[r][q], ncl);
+                }
+            }
+        }
+        if (tid == 0) {
+            // canon[i] = first step whose pivot row equals that of step i (rows below the sub-panel only)
+            for (int i = 0; i < sw; ++i) {
+                int c = -1;
+                if (spiv[i] >= cs + sw) { c = i; for (int t = 0; t < i; ++t) if (spiv[t] == spiv[i]) { c = t; break; } }
+                canon[i] = c;
+            }
+        }
+        pc_sync();           // sub-panel stores (global) and L11 (shared) visible to the whole cluster
+        // ---- 4 (rank 0): the other columns of the outer panel: interchanges (+ S x S solve for the inner panel's right part)
+        const int nright = (c0 + w) - (cs + sw);          // inner-panel columns still to be updated
+        if (rank == 0 && tid < Wout) {
+            const int cu = J + tid;
+            if (cu < cs || cu >= cs + sw) {
+                c128* col = A + (size_t)cu * n;
+                c128 x[S], y[S];
+#pragma unroll
+                for (int i = 0; i < S; ++i) {
+                    x[i] = (i < sw) ? col[cs + i] : zero;
+                    y[i] = (i < sw && canon[i] == i) ? col[spiv[i]] : zero;
+                }
+#pragma unroll
+                for (int i = 0; i < S; ++i) {
+                    if (i < sw) {
+                        const int p = spiv[i];
+                        if (p != cs + i) {
+                            const int k = (p < cs + sw) ? (p - cs) : canon[i];
+                            const bool top = p < cs + sw;
+                            const c128 xi = x[i];
+                            c128 other = xi;
+#pragma unroll
+                            for (int t = 0; t < S; ++t) if (t == k) other = top ? x[t] : y[t];
+#pragma unroll
+                            for (int t = 0; t < S; ++t) if (t == k) { if (top) x[t] = xi; else y[t] = xi; }
+                            x[i] = other;
+                        }
+                    }
+                }
+                const bool right = cu >= cs + sw && cu < c0 + w;
+                if (right) {
+#pragma unroll
+                    for (int jq = 0; jq < S; ++jq)
+#pragma unroll
+                        for (int i = jq + 1; i < S; ++i)
+                            if (i < sw) cfms(x[i], L11[i * S + jq], x[jq]);
+#pragma unroll
+                    for (int i = 0; i < S; ++i) if (i < sw) pc_bcast_c128(&Us[i * PC_MAXW + (cu - cs - sw)], x[i], ncl);
+                }
+#pragma unroll
+                for (int i = 0; i < S; ++i) {
+                    if (i < sw) {
+                        col[cs + i] = x[i];
+                        if (canon[i] == i) col[spiv[i]] = y[i];
+                    }
+                }
+            }
+        }
+        pc_sync();           // interchanged columns (global) and the rows of U (shared) visible to the whole cluster
+        // ---- 5: rank-sw update of the inner panel's remaining columns (rows below the sub-panel), software-pipelined
+        if (nright > 0) {
+            constexpr int RC = (R % 5 == 0) ? 5 : ((R % 4 == 0) ? 4 : R);      // rows per chunk
+            constexpr int NCH = R / RC;
+            c128 cur[RC], nxt[RC];
+#pragma unroll
+            for (int i = 0; i < RC; ++i) {
+                const int row = c0 + g0 + i * TT;
+                cur[i] = (row >= cs + sw && row < n) ? A[row + (size_t)(cs + sw) * n] : zero;
+            }
+            for (int c = 0; c < nright; ++c) {
+#pragma unroll
+                for (int ch = 0; ch < NCH; ++ch) {
+                    const int nch = (ch + 1 == NCH) ? 0 : ch + 1;
+                    const int nc = c + ((ch + 1 == NCH) ? 1 : 0);
+#pragma unroll
+                    for (int i = 0; i < RC; ++i) {
+                        const int row = c0 + g0 + (nch * RC + i) * TT;
+                        nxt[i] = (nc < nright && row >= cs + sw && row < n) ? A[row + (size_t)(cs + sw + nc) * n] : zero;
+                    }
+#pragma unroll
+                    for (int i = 0; i < RC; ++i) {
+                        const int r = ch * RC + i;
+                        const int row = c0 + g0 + r * TT;
+                        if (row >= cs + sw && row < n) {
+#pragma unroll
+                            for (int q = 0; q < S; ++q) if (q < sw) cfms(cur[i], v[r][q], Us[q * PC_MAXW + c]);
+                            A[row + (size_t)(cs + sw + c) * n] = cur[i];
+                        }
+                    }
+#pragma unroll
+                    for (int i = 0; i < RC; ++i) cur[i] = nxt[i];
+                }
+            }
+        }
+        pc_sync();           // updated columns visible before the next sub-panel is loaded by other owners' neighbours
+    }
+    // ---- 6 (rank 0): U12 of the outer panel's columns to the RIGHT of this inner panel: the w x w unit-lower solve
+    const int nr = (J + Wout) - (c0 + w);
+    if (nr > 0 && rank == 0) {
+        __shared__ c128 Lw[PC_MAXW * PC_MAXW];
+        for (int e = tid; e < w * w; e += THREADS) { const int r = e % w, c = e / w; Lw[r + PC_MAXW * c] = A[(c0 + r) + (size_t)(c0 + c) * n]; }
+        __syncthreads();
+        if (tid < nr) {
+            c128* col = A + (size_t)(c0 + w + tid) * n + c0;
+            c128 x[PC_MAXW];
+#pragma unroll
+            for (int i = 0; i < PC_MAXW; ++i) x[i] = (i < w) ? col[i] : zero;
+#pragma unroll
+            for (int jq = 0; jq < PC_MAXW; ++jq)
+#pragma unroll
+                for (int i = jq + 1; i < PC_MAXW; ++i)
+                    if (i < w) cfms(x[i], Lw[i + PC_MAXW * jq], x[jq]);
+#pragma unroll
+            for (int i = 0; i < PC_MAXW; ++i) if (i < w) col[i] = x[i];
+        }
+    }
+}
+
+template <int THREADS, int R, int S>
+static int launch_clu(c128* base, size_t stride, int n, int J, int Wout, int c0, int w, int ne, int batch, int* piv, int* info,
+                      int cl, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(batch * cl), 1, 1);
+    cfg.blockDim = dim3(THREADS, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    LSMS_CUDA_OK(cudaLaunchKernelEx(&cfg, k_panel_clu<THREADS, R, S>, base, stride, n, J, Wout, c0, w, ne, piv, info));
+    LSMS_LAUNCH_CHECK();
+    return 0;
+}
+
+// cl = CTAs per matrix (2, 4 or 8); rows per CTA = ceil((n - c0) / cl) picks the instance
+int launch_panel_cluster(c128* base, size_t stride, int n, int J, int Wout, int c0, int w, int ne, int batch, int* piv, int* info,
+                         int cl, cudaStream_t st) {
+    if (w < 1 || w > PC_MAXW || Wout > PC_MAXOUT || cl < 2 || cl > PC_MAXCL) return -1;
+    const int m = (n - c0 + cl - 1) / cl;
+#define LSMS_PC(T, R, S) return launch_clu<T, R, S>(base, stride, n, J, Wout, c0, w, ne, batch, piv, info, cl, st)
+    if (m <= 256) LSMS_PC(256, 1, 4);
+    if (m <= 512) LSMS_PC(256, 2, 4);
+    if (m <= 1024) LSMS_PC(512, 2, 4);
+    if (m <= 2560) LSMS_PC(512, 5, 4);
+    if (m <= 5120) LSMS_PC(512, 10, 2);
+#undef LSMS_PC
+    return -1;
+}
+
+}  // namespace lsms

@@ -340,6 +340,43 @@ def test_panel_kernel_variants_match_oracle(lt, variant):
         lt.lsms_set_panel_variant(1)
 
 
+@pytest.mark.parametrize("cl", [2, 4, 8])
+def test_panel_cluster_kernel_matches_one_cta_kernel_and_oracle(lt, cl):
+    """K2 with a cluster of cl CTAs per matrix: same pivots and arithmetic as the one-CTA kernel, so tau00 must be
+    bit-identical to it; also against the oracle / LAPACK on a tiny LIZ, ragged random matrices (rows not a multiple
+    of the cluster's thread count, sub-panel tails) and a singular matrix (info)."""
+    try:
+        batch = sl.make_batch("T").select([0, 31])
+        ref, _ = oracle.tau00_batched(batch, "long double")
+        lt.lsms_set_panel_cluster(1)
+        tau1, info1, _ = lt.tau00_from_liz_batch(batch)
+        lt.lsms_set_panel_cluster(cl)
+        tau, info, _ = lt.tau00_from_liz_batch(batch)
+        assert not info.any() and not info1.any()
+        assert np.array_equal(tau, tau1)
+        assert max(relF(tau[b], ref[b]) for b in range(2)) < 1e-12
+        for n_sites, kmax in ((23, 9), (150, 9), (131, 16)):
+            n = n_sites * kmax
+            A = sl.random_dense_matrices(2, n, seed=900 + n)             # column-major storage: [b, col, row]
+            lt.lsms_set_panel_cluster(1)
+            t1, i1 = lt.lsms_tau00_batched(torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
+            lt.lsms_set_panel_cluster(cl)
+            t2, i2 = lt.lsms_tau00_batched(torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
+            torch.cuda.synchronize()
+            assert not i1.cpu().numpy().any() and not i2.cpu().numpy().any()
+            assert torch.equal(torch.view_as_real(t1), torch.view_as_real(t2))
+            t2 = t2.cpu().numpy().transpose(0, 2, 1)
+            for b in range(2):
+                assert relF(t2[b], np.linalg.inv(A[b].T)[n - kmax:, n - kmax:]) < 1e-10
+        A = sl.random_dense_matrices(1, 24, seed=3)
+        A[0, 5, :] = 0.0                           # column 5 identically zero -> exact zero pivot at step 6
+        _, i3 = lt.lsms_tau00_batched(torch.from_numpy(A).cuda(), 6, 4, False, 1)
+        torch.cuda.synchronize()
+        assert int(i3.cpu().numpy()[0]) == 6
+    finally:
+        lt.lsms_set_panel_cluster(0)
+
+
 def test_batch_groups_give_identical_results(lt):
     """Batch groups run the same per-item elimination on separate streams: bitwise equal tau00 for every
     group count, including counts that do not divide the batch and exceed it."""
