@@ -185,10 +185,11 @@ def test_tau00_full_size_mid_batch_residual_every_item(lt):
 
 
 @pytest.mark.parametrize("key,items,mode", [("P", [0, 24, 31, 56, 64, 88, 120, 127], "double"),
-                                             ("C", [16, 63], "double")])
+                                             ("C", [0, 16, 24, 31, 32, 47, 56, 63], "double")])
 def test_tau00_production_sizes_sampled(lt, key, items, mode):
-    """2160^2 and 4320^2 (the north-star sizes): sampled items against the oracle's textbook route,
-    plus the residual of the central block column for the same items on the host."""
+    """2160^2 and 4320^2 (the north-star sizes): eight sampled items each (first and last energy of every atom, the
+    worst-conditioned contour point q = 24) against the oracle's textbook route, which runs one item per host
+    thread, plus the residual of the central block column for the same items on the host."""
     batch = sl.make_batch(key).select(items)
     cfg = batch.cfg
     M, _, _ = gpu_M(lt, batch)
