@@ -2,6 +2,8 @@
 on the same seeded inputs.  Bars (BASELINE.json north_star):
 relative Frobenius error <= 1e-10 on tau00, normwise residual <= 1e-12, assembled M within
 1e-13 of the oracle's M relative to the largest entry of its site block."""
+import os
+
 import numpy as np
 import pytest
 
@@ -223,6 +225,28 @@ def test_tau00_high_l_full_size_properties(lt):
         Mo = oracle_M(batch, i)
         assert block_rel_err(M[i].cpu().numpy().T, Mo, cfg.k) < ASM_TOL
         assert residual(Mo, X[i].cpu().numpy().T, cfg.k) < RES_TOL
+
+
+@pytest.mark.parametrize("key,item", [("H", 0), ("H", 23), ("N", 23), ("C", 24)])
+def test_tau00_full_size_against_stored_oracle_values(lt, key, item):
+    """Element-wise parity at full size where the oracle needs minutes per item: tau00 of single items of the
+    largest workloads (H item 0 is the worst-conditioned matrix of all configs, cond_1 ~ 1.6e6) against values the
+    oracle wrote into tests/golden/ (tests/golden/make_golden_full_size.py: oracle.assemble_M + FP64 LU with
+    long-double iterative refinement; nothing there comes from the CUDA path)."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"tau00_full_size_{key}_{item}.txt")
+    with open(path) as f:
+        head = f.readline().split()
+        assert head[1] == key and int(head[2]) == item
+        n, k = int(head[3]), int(head[4])
+        ref = np.zeros((k, k), dtype=np.complex128)
+        for line in f:
+            r, c, re, im = line.split()
+            ref[int(r), int(c)] = complex(float(re), float(im))
+    batch = sl.make_batch(key).select([item])
+    assert batch.cfg.n == n and batch.cfg.k == k
+    tau, info, _ = lt.tau00_from_liz_batch(batch)
+    assert not info.any()
+    assert relF(tau[0], ref) < TAU_TOL, relF(tau[0], ref)
 
 
 @pytest.mark.parametrize("key,item", [("N", 23), ("NC", 0)])

@@ -398,3 +398,27 @@ def test_contour_sum_closed_forms():
         e = np.zeros(7, dtype=np.complex128); e[q] = 1.0
         assert np.array_equal(oracle.contour_sum(tau, e), tau[:, q])
 
+
+def test_stored_full_size_values_are_well_formed():
+    """tests/golden/tau00_full_size_*.txt (written by make_golden_full_size.py from oracle/ alone): header matches the
+    workload's shape, every (row, col) present once, finite; and the route that wrote them (FP64 LU + long-double
+    refinement) agrees with the long-double textbook route on a case small enough to run here."""
+    import glob
+    files = sorted(glob.glob(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "tau00_full_size_*.txt")))
+    assert files, "run tests/golden/make_golden_full_size.py"
+    for path in files:
+        with open(path) as f:
+            head = f.readline().split()
+            cfg = sl.CONFIGS[head[1]]
+            assert int(head[3]) == cfg.n and int(head[4]) == cfg.k and 0 <= int(head[2]) < cfg.batch
+            seen = set()
+            for line in f:
+                r, c, re, im = line.split()
+                seen.add((int(r), int(c)))
+                assert np.isfinite(float(re)) and np.isfinite(float(im))
+            assert len(seen) == cfg.k * cfg.k
+    cfg = sl.custom_config(19, 2, True, n_energies=2)
+    b = sl.make_batch(cfg)
+    M = oracle.assemble_M(cfg.n_sites, cfg.lmax, cfg.spin_canted, b.site_pos[1], b.species[1], b.delta, b.moment_dir[1], b.z[1])
+    assert relF(oracle.tau00_refined(M, cfg.k, 3), oracle.tau00_full(M, cfg.k, "long double")) < 1e-14
+
