@@ -157,7 +157,7 @@ int lsms_set_blocking(int nb_outer, int ib_inner);
  * and their events are created on first use and are the library's only persistent objects. */
 int lsms_set_lookahead(int on);
 
-/* Batch groups (default 0 = chosen per shape): the batch is cut into `groups` (<= 8) contiguous groups that
+/* Batch groups (default 0 = chosen per shape: two groups for batches of 16 or more, else one): the batch is cut into `groups` (<= 8) contiguous groups that
  * run the elimination on separate library-owned streams, forked from and joined back into the caller's
  * stream inside lsms_tau00_batched, so that the poorly parallel phases of one group (net permutation,
  * triangular solve, look-ahead slice, last panels) run under another group's Schur updates.  Results do
@@ -177,7 +177,7 @@ int lsms_set_panel_variant(int variant);
 int lsms_set_panel_cluster(int cl);
 
 /* Tile alignment (default on): the first outer panel is n mod 64 columns wide, so that all later trailing
- * matrices are whole multiples of the 64 x 64 Schur-update tile.  Off: every panel is NB wide. */
+ * matrices are whole multiples of 64 rows and columns (the Schur-update tile is 64 x 32).  Off: every panel is NB wide. */
 int lsms_set_align_first(int on);
 
 /* How many kernels the last lsms_tau00_batched / lsms_build_M_batched call on this thread enqueued. */

@@ -181,7 +181,7 @@ static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* inf
     if (ne <= 0) return 0;
     // Tile alignment: the first panel is n mod 64 wide (when that is non-zero), so that every trailing matrix
     // the Schur update sees has a multiple of the 64 x 64 DMMA tile in both dimensions; only the last,
-    // smallest updates carry a ragged tile (n = 2160: 34 x 34 tiles of which one row and column 3/4 full -> 33 x 33 full).
+    // smallest updates carry a ragged tile (n = 2160, 64-row tiles: 34 tile rows of which one 3/4 full -> 33 full).
     int W0 = ne < NB ? ne : NB;
     if (g_align_first && NB % 64 == 0 && n % 64 != 0 && n % 64 < W0) W0 = n % 64;
     int rc = factor_panel(M, n, batch, 0, W0, ne, IB, piv, info, st); if (rc) return rc;
