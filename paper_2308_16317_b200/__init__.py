@@ -33,8 +33,13 @@ def lib() -> ctypes.CDLL:
     global _lib
     if _lib is None:
         if not os.path.exists(LIB_PATH):
-            raise LsmsError(f"{LIB_PATH} is missing: run `python paper_2308_16317_b200/build.py` "
-                            "(there is no CPU fallback)")
+            # a fresh checkout has no built artefact: compile it (nvcc cross-compiles without a GPU); never a fallback
+            try:
+                from . import build as _build
+                _build.build()
+            except Exception as exc:          # noqa: BLE001 - reported below
+                raise LsmsError(f"{LIB_PATH} is missing and `python paper_2308_16317_b200/build.py` failed: {exc} "
+                                "(there is no CPU fallback)") from exc
         L = ctypes.CDLL(LIB_PATH)
         vp, ci, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
         L.lsms_version.restype = ctypes.c_char_p
