@@ -1,56 +1,83 @@
-// api.cu -- the C ABI of include/lsms_tau.h: argument checks, workspace layout and the batch
-// scheduler that walks the blocked right-looking elimination.
+// api.cu -- the C ABI of include/lsms_tau.h and include/lsms_tau_diag.h: argument checks, the per-handle context,
+// workspace layout and the batch scheduler that walks the blocked right-looking elimination.
 #include <math.h>
 #include <stdint.h>
+#include <string.h>
+#include <new>
 #include <vector>
 #include "../../include/lsms_tau.h"
+#include "../../include/lsms_tau_diag.h"
 #include "common.cuh"
 #include "internal.h"
 
 namespace lsms {
 thread_local LaunchCounter g_launches = {0};
-static int g_nb_outer = 0, g_ib_inner = 0;
+thread_local Ctx* t_ctx = nullptr;
 
 // ---- optional per-kernel-class timing (lsms_profile_begin / lsms_profile_end): CUDA events recorded on
-// the caller's stream around each launch, so bench.py can report the Schur update's duration and share
-// measured inside the step.  Classes: 0 K1 assembly, 1 K2 panel, 2 K3 swap/trsm, 3 K4 inner (K <= IB),
-// 4 K4 Schur update (K = NB), 5 K5 final inverse, 6 K3a/K3b net permutation + Ninv, 7 K4 as TRSM (U12 = -Ninv*A12).
-struct Prof {
-    bool on = false;
-    std::vector<cudaEvent_t> ev;     // pairs
-    std::vector<int> cls;
-    size_t used = 0;
-    double flops[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-};
-static Prof g_prof;
-struct ProfScope {
-    cudaStream_t st; bool live;
-    ProfScope(int cls, cudaStream_t s, double flops = 0.0) : st(s), live(g_prof.on) {
-        if (!live) return;
-        if (g_prof.ev.size() < 2 * (g_prof.used + 1)) {
-            cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
-            g_prof.ev.push_back(a); g_prof.ev.push_back(b); g_prof.cls.push_back(cls);
-        }
-        g_prof.cls[g_prof.used] = cls;
-        g_prof.flops[cls] += flops;
-        cudaEventRecord(g_prof.ev[2 * g_prof.used], st);
+// the launch stream around each launch, so bench.py can report the Schur update's duration and share
+// measured inside the step.  Classes: lsms_tau_diag.h.
+ProfScope::ProfScope(int cls, cudaStream_t s, double flops) : st(s), live(t_ctx && t_ctx->prof.on) {
+    if (!live) return;
+    Prof& p = t_ctx->prof;
+    if (p.ev.size() < 2 * (p.used + 1)) {
+        cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+        p.ev.push_back(a); p.ev.push_back(b); p.cls.push_back(cls);
     }
-    ~ProfScope() { if (live) { cudaEventRecord(g_prof.ev[2 * g_prof.used + 1], st); ++g_prof.used; } }
-};
+    p.cls[p.used] = cls;
+    p.flops[cls] += flops;
+    cudaEventRecord(p.ev[2 * p.used], st);
+}
+ProfScope::~ProfScope() { if (live) { Prof& p = t_ctx->prof; cudaEventRecord(p.ev[2 * p.used + 1], st); ++p.used; } }
 
 static inline size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 static int isqrt_exact(int v) { int r = (int)lround(sqrt((double)v)); return (r * r == v) ? r : -1; }
 
-static inline int eff_nb() { return g_nb_outer > 0 ? g_nb_outer : 64; }
-static inline int eff_ib() { return g_ib_inner > 0 ? g_ib_inner : 16; }
+static inline int eff_nb(const Ctx* c) { return c->opt[LSMS_OPT_NB_OUTER] > 0 ? c->opt[LSMS_OPT_NB_OUTER] : 64; }
+static inline int eff_ib(const Ctx* c) { return c->opt[LSMS_OPT_IB_INNER] > 0 ? c->opt[LSMS_OPT_IB_INNER] : 16; }
+
+// First enqueueing call through a handle: bind it to the current device -- opt the kernels into their shared-memory
+// sizes there and create the scheduler's streams and events.
+static int bind_device(Ctx* c, int dev) {
+    LSMS_CUDA_OK(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
+    int rc;
+    if ((rc = init_attrs_gemm()) || (rc = init_attrs_lu()) || (rc = init_attrs_assemble()) || (rc = init_attrs_fused())) return rc;
+    int lo = 0, hi = 0;
+    LSMS_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    LSMS_CUDA_OK(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
+    for (int g = 0; g < MAX_GROUPS; ++g) {
+        GroupStreams& s = c->gs[g];
+        if (g > 0) LSMS_CUDA_OK(cudaStreamCreateWithFlags(&s.main, cudaStreamNonBlocking));
+        LSMS_CUDA_OK(cudaStreamCreateWithPriority(&s.aux, cudaStreamNonBlocking, hi));
+        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming));
+        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming));
+        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+    }
+    c->device = dev;
+    return 0;
+}
+
+// Entry of every extern "C" call that enqueues work (after its argument checks): the handle is bound to the current
+// device on first use and must be used on that device afterwards.
+struct CallScope {
+    int rc = 0;
+    explicit CallScope(Ctx* c) {
+        int dev = -1;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) { rc = (int)e; return; }
+        if (c->device < 0) { rc = bind_device(c, dev); if (rc) return; }
+        if (dev != c->device) { rc = (int)cudaErrorInvalidDevice; return; }
+        t_ctx = c; g_launches.n = 0;
+    }
+    ~CallScope() { if (!rc && t_ctx) t_ctx->last_launches = g_launches.n; }
+};
 
 // Workspace layout for lsms_tau00_batched:
 //   [pivots int32 batch*n][perm int32 batch*(4+3NB)][Ninv c128 batch*NB*NB][Tperm c128 batch*NB*n][K5 scratch]
 struct TauWs { int* piv; int* perm; c128* ninv; c128* tperm; void* k5; size_t total; };
-static TauWs tau_ws_layout(void* base, int n, int k, int batch) {
-    const int NB = eff_nb();
+static TauWs tau_ws_layout(void* base, int NB, int n, int k, int batch) {
     TauWs w; char* p = (char*)base;
     w.piv = (int*)p; p += align256((size_t)batch * n * sizeof(int));
     w.perm = (int*)p; p += align256((size_t)batch * (4 + 3 * NB) * sizeof(int));
@@ -60,15 +87,15 @@ static TauWs tau_ws_layout(void* base, int n, int k, int batch) {
     w.total = (size_t)(p - (char*)base);
     return w;
 }
-static size_t tau_ws_bytes(int n, int k, int batch) { return tau_ws_layout(nullptr, n, k, batch).total; }
+static size_t tau_ws_bytes(const Ctx* c, int n, int k, int batch) { return tau_ws_layout(nullptr, eff_nb(c), n, k, batch).total; }
 
 // Blocked right-looking elimination of the first ne = n-k columns of every item, in lock-step over
 // the batch: each launch covers all items, so the latency-bound panel kernels (one CTA per item)
 // fill the chip through the batch dimension while the update kernels tile every trailing matrix.
 //   outer panel [J, J+W), W <= NB:
 //     for each inner panel [c0, c0+w), w <= IB:                       (inside the outer panel only)
-//        K2  factor the (n-c0) x w panel, pivots restricted to rows < ne
-//        K3  interchanges on the outer panel's other columns; TRSM on those to the right
+//        K2  factor the (n-c0) x w panel, pivots restricted to rows < ne; interchanges and triangular solves
+//            inside the outer panel
 //        K4  rank-w update of the outer panel's remaining columns
 //     K3a fold the W interchanges into one row permutation; Ninv = -(L11^{-1})
 //     K3b permute the trailing columns [J+W, n): new top block -> Tperm, displaced rows scattered
@@ -80,45 +107,19 @@ static size_t tau_ws_bytes(int n, int k, int batch) { return tau_ws_layout(nullp
 // factored on a high-priority auxiliary stream while the main stream updates the remaining columns.  The
 // latency/L2-bound panel kernels thus run underneath the DMMA-bound update instead of in front of it.
 // The two streams touch disjoint columns (the panel's interchanges reach the trailing columns only in K3b,
-// after the join).  The auxiliary stream and two events are the library's only persistent objects.
-static int g_lookahead = 1;
-static int g_groups = 0;                  // 0 = chosen per shape
-static int g_align_first = 1;              // first panel n mod 64 wide (tile-aligned trailing matrices)
-static int g_panel_variant = 1;           // -1 L2-resident k_panel, 0 register-blocked 256 threads, 1 register-blocked 512 threads for tall panels
-constexpr int MAX_GROUPS = 8;
-// Stream set of one batch group (see eliminate_groups): group 0 runs on the caller's stream, the others on
-// library-owned streams; every group has a high-priority auxiliary stream for the look-ahead panel.
-struct GroupStreams { cudaStream_t main = nullptr, aux = nullptr; cudaEvent_t fork = nullptr, join = nullptr, done = nullptr; };
-static GroupStreams g_gs[MAX_GROUPS];
-static cudaEvent_t g_ev_start = nullptr;
+// after the join).  The streams and events belong to the handle.
 
-static int ensure_streams(int groups) {
-    int lo = 0, hi = 0;
-    LSMS_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
-    if (!g_ev_start) LSMS_CUDA_OK(cudaEventCreateWithFlags(&g_ev_start, cudaEventDisableTiming));
-    for (int g = 0; g < groups; ++g) {
-        GroupStreams& s = g_gs[g];
-        if (s.aux) continue;
-        if (g > 0) LSMS_CUDA_OK(cudaStreamCreateWithFlags(&s.main, cudaStreamNonBlocking));
-        LSMS_CUDA_OK(cudaStreamCreateWithPriority(&s.aux, cudaStreamNonBlocking, hi));
-        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming));
-        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming));
-        LSMS_CUDA_OK(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
-    }
-    return 0;
-}
-
-static int g_panel_cluster = 0;            // 0 = chosen per shape, 1 = never, 2/4/8 = forced
 // CTAs per matrix for the panel kernel.  A cluster shortens the panel factorisation of a tall panel several times
 // (rank 12450, 12 matrices: 303 -> 117 ms per step when timed alone), but its CTAs must be co-scheduled on free SMs, so
 // under look-ahead it waits for the Schur update to drain instead of running beneath it and whole steps of batches
 // >= 4 got SLOWER (NC 1897 -> 1928 ms, H 629 -> 654, C 440 -> 465, P 121 -> 129).  It pays when there is next to
 // nothing to overlap with: one or two tall matrices (rank 12450, batch 1: 369 -> 223 ms; rank 4320: 36.9 -> 32.5 ms).
-static int panel_cluster_size(int m, int batch) {
-    if (g_panel_variant < 1) return 1;
-    if (g_panel_cluster == 1) return 1;
+static int panel_cluster_size(const Ctx* c, int m, int batch) {
+    const int pc = c->opt[LSMS_OPT_PANEL_CLUSTER];
+    if (c->opt[LSMS_OPT_PANEL_THREADS] < 1) return 1;
+    if (pc == 1) return 1;
     int cl = 1;
-    if (g_panel_cluster > 1) cl = g_panel_cluster;
+    if (pc > 1) cl = pc;
     else if (batch <= 2 && m >= 4096) cl = 8;
     else if (batch <= 2 && m >= 2048) cl = 4;
     if (cl > 1 && (m + cl - 1) / cl > 5120) cl = 1;         // taller than the cluster instances cover: one-CTA kernel
@@ -126,26 +127,20 @@ static int panel_cluster_size(int m, int batch) {
 }
 
 // factor the outer panel [J, J+W) on stream st: inner panels of width <= IB
-static int factor_panel(c128* M, int n, int batch, int J, int W, int ne, int IB, int* piv, int* info, cudaStream_t st) {
+static int factor_panel(const Ctx* c, c128* M, int n, int batch, int J, int W, int ne, int IB, int* piv, int* info, cudaStream_t st) {
     const size_t stride = (size_t)n * n;
     const int Jend = J + W;
     GemmShape g; g.strideA = g.strideB = g.strideC = stride; g.ldA = g.ldB = g.ldC = n; g.batch = batch; g.beta0 = 0;
     for (int jj = 0; jj < W; jj += IB) {
         const int c0 = J + jj, w = (W - jj < IB) ? W - jj : IB;
         int rc;
-        if (g_panel_variant >= 0 && n - c0 <= 16384) {
-            // register-blocked K2: factors the inner panel, applies its interchanges to the whole outer panel and
-            // solves the w x w triangle for the outer panel's columns to the right
-            // small batches of tall panels: a cluster of CTAs per matrix, so that the panel phase spans the chip too
-            const int cl = panel_cluster_size(n - c0, batch);
-            if (cl > 1) { ProfScope ps(1, st); rc = launch_panel_cluster(M, stride, n, J, W, c0, w, ne, batch, piv, info, cl, st); }
-            else { ProfScope ps(1, st); rc = launch_panel_reg(M, stride, n, J, W, c0, w, ne, batch, piv, info, g_panel_variant, st); }
-            if (rc) return rc;
-        } else {
-            { ProfScope ps(1, st); rc = launch_panel(M, stride, n, c0, w, ne, batch, piv, info, st); } if (rc) return rc;
-            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, J, c0, 1, batch, piv, st); } if (rc) return rc;
-            { ProfScope ps(2, st); rc = launch_swap_trsm(M, stride, n, c0, w, c0 + w, Jend, 3, batch, piv, st); } if (rc) return rc;
-        }
+        // register-blocked K2: factors the inner panel, applies its interchanges to the whole outer panel and
+        // solves the w x w triangle for the outer panel's columns to the right;
+        // small batches of tall panels: a cluster of CTAs per matrix, so that the panel phase spans the chip too
+        const int cl = panel_cluster_size(c, n - c0, batch);
+        if (cl > 1) { ProfScope ps(1, st); rc = launch_panel_cluster(M, stride, n, J, W, c0, w, ne, batch, piv, info, cl, st); }
+        else { ProfScope ps(1, st); rc = launch_panel_reg(M, stride, n, J, W, c0, w, ne, batch, piv, info, c->opt[LSMS_OPT_PANEL_THREADS], st); }
+        if (rc) return rc;
         const int rem = Jend - (c0 + w);
         if (rem > 0) {
             g.Mr = n - (c0 + w); g.Nc = rem; g.K = w;
@@ -172,19 +167,19 @@ static int schur_update(c128* M, int n, int batch, int J, int W, int c_lo, int c
 }
 
 // one batch group [0, batch) of items (pointers already offset to the group's first item)
-static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* info, cudaStream_t st, const GroupStreams& gs) {
+static int eliminate(const Ctx* c, c128* M, int n, int k, int batch, const TauWs& ws, int* info, cudaStream_t st, const GroupStreams& gs) {
     const int ne = n - k;
-    const int NB = eff_nb(), IB = eff_ib();
+    const int NB = eff_nb(c), IB = eff_ib(c);
     const size_t stride = (size_t)n * n;
     int* piv = ws.piv;
-    const bool la = g_lookahead != 0;
+    const bool la = c->opt[LSMS_OPT_LOOKAHEAD] != 0;
     if (ne <= 0) return 0;
     // Tile alignment: the first panel is n mod 64 wide (when that is non-zero), so that every trailing matrix
-    // the Schur update sees has a multiple of the 64 x 64 DMMA tile in both dimensions; only the last,
+    // the Schur update sees has a multiple of the 64-row DMMA tile in both dimensions; only the last,
     // smallest updates carry a ragged tile (n = 2160, 64-row tiles: 34 tile rows of which one 3/4 full -> 33 full).
     int W0 = ne < NB ? ne : NB;
-    if (g_align_first && NB % 64 == 0 && n % 64 != 0 && n % 64 < W0) W0 = n % 64;
-    int rc = factor_panel(M, n, batch, 0, W0, ne, IB, piv, info, st); if (rc) return rc;
+    if (c->opt[LSMS_OPT_ALIGN_FIRST] && NB % 64 == 0 && n % 64 != 0 && n % 64 < W0) W0 = n % 64;
+    int rc = factor_panel(c, M, n, batch, 0, W0, ne, IB, piv, info, st); if (rc) return rc;
     { ProfScope ps(6, st); rc = launch_panel_post(M, stride, n, 0, W0, batch, piv, ws.perm, ws.ninv, NB, st); } if (rc) return rc;
     for (int J = 0, W = W0; J < ne; J += W, W = (ne - J < NB) ? ne - J : NB) {
         const int Jend = J + W;                               // Jend <= ne < n
@@ -200,17 +195,21 @@ static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* inf
             rc = schur_update(M, n, batch, J, W, Jend, Jend + W2, st); if (rc) return rc;
             LSMS_CUDA_OK(cudaEventRecord(gs.fork, st));
             LSMS_CUDA_OK(cudaStreamWaitEvent(gs.aux, gs.fork, 0));
-            rc = factor_panel(M, n, batch, Jend, W2, ne, IB, piv, info, gs.aux); if (rc) return rc;
+            rc = factor_panel(c, M, n, batch, Jend, W2, ne, IB, piv, info, gs.aux);
             // the next panel's net permutation and -(L11^-1) are also built under the update: perm/Ninv of
             // panel J were last read by the permutation / triangular solve above, before the fork
-            { ProfScope ps(6, gs.aux); rc = launch_panel_post(M, stride, n, Jend, W2, batch, piv, ws.perm, ws.ninv, NB, gs.aux); } if (rc) return rc;
-            LSMS_CUDA_OK(cudaEventRecord(gs.join, gs.aux));
-            rc = schur_update(M, n, batch, J, W, Jend + W2, n, st); if (rc) return rc;
-            LSMS_CUDA_OK(cudaStreamWaitEvent(st, gs.join, 0));
+            if (!rc) { ProfScope ps(6, gs.aux); rc = launch_panel_post(M, stride, n, Jend, W2, batch, piv, ws.perm, ws.ninv, NB, gs.aux); }
+            // the auxiliary stream is joined back even when a launch failed, so that the caller's stream stays ordered
+            cudaError_t e1 = cudaEventRecord(gs.join, gs.aux);
+            int rc2 = rc ? 0 : schur_update(M, n, batch, J, W, Jend + W2, n, st);
+            cudaError_t e2 = cudaStreamWaitEvent(st, gs.join, 0);
+            if (rc) return rc;
+            if (rc2) return rc2;
+            LSMS_CUDA_OK(e1); LSMS_CUDA_OK(e2);
         } else {
             rc = schur_update(M, n, batch, J, W, Jend, n, st); if (rc) return rc;
             if (W2 > 0) {
-                rc = factor_panel(M, n, batch, Jend, W2, ne, IB, piv, info, st); if (rc) return rc;
+                rc = factor_panel(c, M, n, batch, Jend, W2, ne, IB, piv, info, st); if (rc) return rc;
                 { ProfScope ps(6, st); rc = launch_panel_post(M, stride, n, Jend, W2, batch, piv, ws.perm, ws.ninv, NB, st); } if (rc) return rc;
             }
         }
@@ -224,8 +223,8 @@ static int eliminate(c128* M, int n, int k, int batch, const TauWs& ws, int* inf
 // contiguous groups that run the same elimination on separate streams: while one group is in such a phase
 // the hardware scheduler fills the SMs with another group's Schur-update tiles.  The groups touch disjoint
 // items; the caller's stream is forked into the group streams and joined again before the call returns.
-static int pick_groups(int n, int batch) {
-    int g = g_groups;
+static int pick_groups(const Ctx* c, int n, int batch) {
+    int g = c->opt[LSMS_OPT_GROUPS];
     if (g <= 0) g = (batch >= 16) ? 2 : 1;
     if (g > MAX_GROUPS) g = MAX_GROUPS;
     if (g > batch) g = batch;
@@ -233,147 +232,257 @@ static int pick_groups(int n, int batch) {
     return g;
 }
 
-static int eliminate_groups(c128* M, int n, int k, int batch, const TauWs& ws, c128* tau, int* info, cudaStream_t st) {
-    const int NB = eff_nb();
-    const int groups = pick_groups(n, batch);
-    int rc = ensure_streams(groups); if (rc) return rc;
+static int eliminate_groups(Ctx* c, c128* M, int n, int k, int batch, const TauWs& ws, c128* tau, int* info, cudaStream_t st) {
+    const int NB = eff_nb(c);
+    const int groups = pick_groups(c, n, batch);
     const size_t stride = (size_t)n * n;
-    if (groups > 1) LSMS_CUDA_OK(cudaEventRecord(g_ev_start, st));
-    for (int g = 0; g < groups; ++g) {
+    if (groups > 1) LSMS_CUDA_OK(cudaEventRecord(c->ev_start, st));
+    int rc = 0, forked = 0;
+    for (int g = 0; g < groups && !rc; ++g) {
         const int b0 = (int)((long long)batch * g / groups), b1 = (int)((long long)batch * (g + 1) / groups);
         if (b1 <= b0) continue;
-        cudaStream_t gst = (g == 0) ? st : g_gs[g].main;
-        if (g > 0) LSMS_CUDA_OK(cudaStreamWaitEvent(gst, g_ev_start, 0));
+        cudaStream_t gst = (g == 0) ? st : c->gs[g].main;
+        if (g > 0) { rc = (int)cudaStreamWaitEvent(gst, c->ev_start, 0); if (rc) break; }
         TauWs w = ws;
         w.piv = ws.piv + (size_t)b0 * n;
         w.perm = ws.perm + (size_t)b0 * (4 + 3 * NB);
         w.ninv = ws.ninv + (size_t)b0 * NB * NB;
         w.tperm = ws.tperm + (size_t)b0 * NB * n;
         w.k5 = (char*)ws.k5 + (final_inverse_ws_bytes(k, 1) ? (size_t)b0 * k * k * sizeof(c128) : 0);
-        rc = eliminate(M + (size_t)b0 * stride, n, k, b1 - b0, w, info + b0, gst, g_gs[g]); if (rc) return rc;
-        { ProfScope ps(5, gst);
-          rc = launch_final_inverse(M + (size_t)b0 * stride, stride, n, k, b1 - b0, tau + (size_t)b0 * k * k, info + b0, w.k5, gst); }
-        if (rc) return rc;
-        if (g > 0) LSMS_CUDA_OK(cudaEventRecord(g_gs[g].done, gst));
+        rc = eliminate(c, M + (size_t)b0 * stride, n, k, b1 - b0, w, info + b0, gst, c->gs[g]);
+        if (!rc) {
+            ProfScope ps(5, gst);
+            rc = launch_final_inverse(M + (size_t)b0 * stride, stride, n, k, b1 - b0, tau + (size_t)b0 * k * k, info + b0, w.k5, gst);
+        }
+        // a group stream that was forked is always joined back, also after a failed launch
+        if (g > 0) { cudaEventRecord(c->gs[g].done, gst); forked = g; }
     }
-    for (int g = 1; g < groups; ++g) {
-        const int b0 = (int)((long long)batch * g / groups), b1 = (int)((long long)batch * (g + 1) / groups);
-        if (b1 > b0) LSMS_CUDA_OK(cudaStreamWaitEvent(st, g_gs[g].done, 0));
+    for (int g = 1; g <= forked; ++g) {
+        cudaError_t e = cudaStreamWaitEvent(st, c->gs[g].done, 0);
+        if (!rc && e != cudaSuccess) rc = (int)e;
     }
-    return 0;
+    return rc;
+}
+
+// ---- the batch scheduler's first decision (north_star: "packs small LIZ matrices several per SM and lets large
+// ones span the whole chip").  Small-matrix mode eliminates a matrix start to finish inside one launch, `cl` CTAs per
+// matrix; 0 = lock-step launches over the batch.  See fused.cu for the measurements behind the thresholds.
+static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
+    const int sm = c->opt[LSMS_OPT_SMALL_MODE];
+    if (sm == 1) return 0;
+    if (!fused_supported(n, k, eff_nb(c), eff_ib(c))) return 0;
+    if (sm >= 3) return 1 << (sm - 2);
+    // one CTA per matrix keeps a quarter of an SM busy: it needs about four matrices per SM to fill the chip, and
+    // the per-matrix latency (n sequential pivot steps) must not exceed what the lock-step path needs for the batch
+    const long long slots = 4LL * c->sms;
+    int cl = 1;
+    while (cl < 8 && (long long)batch * cl * 2 <= slots) cl *= 2;     // few matrices: several CTAs per matrix
+    if (sm == 2) return cl;
+    if (n > 1024) return 0;
+    return cl;
+}
+
+static int tau00_impl(Ctx* c, c128* M, int n, int k, int batch, c128* tau, int* info, void* workspace, cudaStream_t st) {
+    const TauWs ws = tau_ws_layout(workspace, eff_nb(c), n, k, batch);
+    const int cl = pick_small_mode(c, n, k, batch);
+    c->last_schedule = cl;
+    if (cl > 0) {
+        ProfScope ps(2, st, 8.0 / 3.0 * (double)n * n * n * batch);
+        return launch_lu_fused(M, (size_t)n * n, n, k, batch, eff_nb(c), eff_ib(c), c->opt[LSMS_OPT_ALIGN_FIRST], cl, ws.piv, tau, info, st);
+    }
+    return eliminate_groups(c, M, n, k, batch, ws, tau, info, st);
+}
+
+static size_t workspace_bytes_impl(const Ctx* c, int n_sites, int lmax, int spin_canted, int batch) {
+    if (n_sites < 1 || lmax < 0 || lmax > 8 || batch < 1) return 0;
+    int kmax = (lmax + 1) * (lmax + 1), k = kmax * (spin_canted ? 2 : 1);
+    size_t n = (size_t)n_sites * k;
+    if (n > 46340) return 0;
+    size_t a = align256(gaunt_table_bytes(lmax));
+    size_t t = tau_ws_bytes(c, (int)n, k, batch);
+    return a > t ? a : t;
 }
 
 }  // namespace lsms
 
 using namespace lsms;
 
+#define LSMS_ENTER(h) if (!(h)) return -1
+#define LSMS_BIND(h) CallScope scope__(h); if (scope__.rc) return scope__.rc
+
 extern "C" {
 
-const char* lsms_version(void) { return "lsms_tau 0.1 (sm_100a; DMMA.8x8x4 Schur update, TMA-staged)"; }
+const char* lsms_version(void) { return "lsms_tau 0.2 (sm_100a; DMMA.8x8x4 Schur update, TMA-staged; small-matrix mode)"; }
 
-size_t lsms_workspace_bytes(int n_sites, int lmax, int spin_canted, int batch) {
-    if (n_sites < 1 || lmax < 0 || lmax > 8 || batch < 1) return 0;
-    int kmax = (lmax + 1) * (lmax + 1), k = kmax * (spin_canted ? 2 : 1);
-    size_t n = (size_t)n_sites * k;
-    size_t a = align256(gaunt_table_bytes(lmax));
-    size_t t = tau_ws_bytes((int)n, k, batch);
-    return a > t ? a : t;
+int lsms_create(lsms_handle_t* handle_out) {
+    if (!handle_out) return -1;
+    lsms_context* c = new (std::nothrow) lsms_context();
+    *handle_out = c;
+    if (!c) return (int)cudaErrorMemoryAllocation;
+    for (int i = 0; i < LSMS_OPT_COUNT; ++i) c->opt[i] = 0;
+    c->opt[LSMS_OPT_LOOKAHEAD] = 1; c->opt[LSMS_OPT_PANEL_THREADS] = 1; c->opt[LSMS_OPT_ALIGN_FIRST] = 1;
+    c->device = -1;                      // bound by the first call that enqueues work
+    return 0;
 }
 
-size_t lsms_solve_workspace_bytes(int n_sites, int kmax, int spin_canted, int batch) {
-    if (n_sites < 1 || kmax < 1 || batch < 1) return 0;
+int lsms_destroy(lsms_handle_t c) {
+    if (!c) return -1;
+    if (t_ctx == c) t_ctx = nullptr;
+    for (int g = 0; g < MAX_GROUPS; ++g) {
+        GroupStreams& s = c->gs[g];
+        if (s.main) cudaStreamDestroy(s.main);
+        if (s.aux) cudaStreamDestroy(s.aux);
+        if (s.fork) cudaEventDestroy(s.fork);
+        if (s.join) cudaEventDestroy(s.join);
+        if (s.done) cudaEventDestroy(s.done);
+    }
+    if (c->ev_start) cudaEventDestroy(c->ev_start);
+    for (cudaEvent_t ev : c->prof.ev) cudaEventDestroy(ev);
+    delete c;
+    return 0;
+}
+
+int lsms_set_option(lsms_handle_t c, int option, int value) {
+    if (!c) return -1;
+    bool ok = false;
+    switch (option) {
+        case LSMS_OPT_NB_OUTER: ok = value >= 0 && value <= 96 && value % 4 == 0; break;
+        case LSMS_OPT_IB_INNER: ok = value >= 0 && value <= 16; break;
+        case LSMS_OPT_LOOKAHEAD: case LSMS_OPT_PANEL_THREADS: case LSMS_OPT_ALIGN_FIRST: ok = value == 0 || value == 1; break;
+        case LSMS_OPT_GROUPS: ok = value >= 0 && value <= MAX_GROUPS; break;
+        case LSMS_OPT_PANEL_CLUSTER: ok = value == 0 || value == 1 || value == 2 || value == 4 || value == 8; break;
+        case LSMS_OPT_SMALL_MODE: ok = value >= 0 && value <= 5; break;
+        default: return -2;
+    }
+    if (!ok) return -3;
+    c->opt[option] = value;
+    return 0;
+}
+
+int lsms_get_option(lsms_handle_t c, int option, int* value_host) {
+    if (!c) return -1;
+    if (option < 0 || option >= LSMS_OPT_COUNT) return -2;
+    if (!value_host) return -3;
+    *value_host = c->opt[option];
+    return 0;
+}
+
+size_t lsms_workspace_bytes(lsms_handle_t c, int n_sites, int lmax, int spin_canted, int batch) {
+    if (!c) return 0;
+    return workspace_bytes_impl(c, n_sites, lmax, spin_canted, batch);
+}
+
+size_t lsms_solve_workspace_bytes(lsms_handle_t c, int n_sites, int kmax, int spin_canted, int batch) {
+    if (!c || n_sites < 1 || kmax < 1 || batch < 1) return 0;
     int k = kmax * (spin_canted ? 2 : 1);
     size_t n = (size_t)n_sites * k;
-    return align256((size_t)batch * n * n * sizeof(c128)) + align256((size_t)batch * k * k * sizeof(c128)) + tau_ws_bytes((int)n, k, batch);
+    if (n > 46340) return 0;
+    return align256((size_t)batch * n * n * sizeof(c128)) + align256((size_t)batch * k * k * sizeof(c128)) + tau_ws_bytes(c, (int)n, k, batch);
 }
 
-int lsms_tinv_from_phase_shifts(const lsms_c128* delta, const int* species, const lsms_c128* z,
+int lsms_tinv_from_phase_shifts(lsms_handle_t h, const lsms_c128* delta, const int* species, const lsms_c128* z,
                                 int lmax, int n_sites, int spin_canted, int n_species, int batch,
-                                lsms_c128* tinv_diag, lsms_c128* kappa, void* cuda_stream) {
-    if (!delta || !aligned16(delta)) return -1;
-    if (!species) return -2;
-    if (!z || !aligned16(z)) return -3;
-    if (lmax < 0 || lmax > 8) return -4;
-    if (n_sites < 1) return -5;
-    if (n_species < 1) return -7;
-    if (batch < 1) return -8;
-    if (!tinv_diag || !aligned16(tinv_diag)) return -9;
-    if (!kappa || !aligned16(kappa)) return -10;
-    g_launches.n = 0;
-    return launch_tinv((const c128*)delta, species, (const c128*)z, lmax, n_sites, spin_canted ? 2 : 1, batch,
-                       (c128*)tinv_diag, (c128*)kappa, (cudaStream_t)cuda_stream);
+                                lsms_c128* tinv_diag, lsms_c128* kappa, int* info, void* cuda_stream) {
+    LSMS_ENTER(h);
+    if (!delta || !aligned16(delta)) return -2;
+    if (!species) return -3;
+    if (!z || !aligned16(z)) return -4;
+    if (lmax < 0 || lmax > 8) return -5;
+    if (n_sites < 1) return -6;
+    if (n_species < 1) return -8;
+    if (batch < 1) return -9;
+    if (!tinv_diag || !aligned16(tinv_diag)) return -10;
+    if (!kappa || !aligned16(kappa)) return -11;
+    if (!info) return -12;
+    LSMS_BIND(h);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    LSMS_CUDA_OK(cudaMemsetAsync(info, 0, (size_t)batch * sizeof(int), st));
+    return launch_tinv((const c128*)delta, species, (const c128*)z, lmax, n_sites, spin_canted ? 2 : 1, n_species, batch,
+                       (c128*)tinv_diag, (c128*)kappa, info, st);
 }
 
-int lsms_build_M_batched(const lsms_c128* tinv_diag, const double* site_pos, const double* moment_dir,
+int lsms_build_M_batched(lsms_handle_t h, const lsms_c128* tinv_diag, const double* site_pos, const double* moment_dir,
                          const lsms_c128* kappa, int lmax, int n_sites, int spin_canted, int batch,
-                         lsms_c128* M_out, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    if (!tinv_diag || !aligned16(tinv_diag)) return -1;
-    if (!site_pos) return -2;
-    if (spin_canted && !moment_dir) return -3;
-    if (!kappa || !aligned16(kappa)) return -4;
-    if (lmax < 0 || lmax > 8) return -5;
-    if (n_sites < 1) return -6;
-    if (batch < 1) return -8;
-    if (!M_out || !aligned16(M_out)) return -9;
-    if (!workspace || !aligned16(workspace)) return -10;
-    if (workspace_bytes < align256(gaunt_table_bytes(lmax))) return -11;
-    g_launches.n = 0;
-    ProfScope ps(0, (cudaStream_t)cuda_stream);
-    return launch_assemble((const c128*)tinv_diag, site_pos, moment_dir, (const c128*)kappa, lmax, n_sites,
-                           spin_canted ? 1 : 0, batch, 1, (c128*)M_out, workspace, (cudaStream_t)cuda_stream);
-}
-
-int lsms_build_M_shared_g0_batched(const lsms_c128* tinv_diag, const double* site_pos, const double* moment_dir,
-                                   const lsms_c128* kappa, int lmax, int n_sites, int spin_canted, int n_atoms, int n_energies,
-                                   lsms_c128* M_out, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    if (!tinv_diag || !aligned16(tinv_diag)) return -1;
-    if (!site_pos) return -2;
-    if (spin_canted && !moment_dir) return -3;
-    if (!kappa || !aligned16(kappa)) return -4;
-    if (lmax < 0 || lmax > 8) return -5;
-    if (n_sites < 1) return -6;
-    if (n_atoms < 1) return -8;
-    if (n_energies < 1) return -9;
+                         lsms_c128* M_out, int* info, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    LSMS_ENTER(h);
+    if (!tinv_diag || !aligned16(tinv_diag)) return -2;
+    if (!site_pos) return -3;
+    if (spin_canted && !moment_dir) return -4;
+    if (!kappa || !aligned16(kappa)) return -5;
+    if (lmax < 0 || lmax > 8) return -6;
+    if (n_sites < 1) return -7;
+    if (batch < 1) return -9;
     if (!M_out || !aligned16(M_out)) return -10;
-    if (!workspace || !aligned16(workspace)) return -11;
-    if (workspace_bytes < align256(gaunt_table_bytes(lmax))) return -12;
-    g_launches.n = 0;
-    ProfScope ps(0, (cudaStream_t)cuda_stream);
+    if (!info) return -11;
+    if (!workspace || !aligned16(workspace)) return -12;
+    if (workspace_bytes < align256(gaunt_table_bytes(lmax))) return -13;
+    LSMS_BIND(h);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    LSMS_CUDA_OK(cudaMemsetAsync(info, 0, (size_t)batch * sizeof(int), st));
+    ProfScope ps(0, st);
     return launch_assemble((const c128*)tinv_diag, site_pos, moment_dir, (const c128*)kappa, lmax, n_sites,
-                           spin_canted ? 1 : 0, n_energies, n_atoms, (c128*)M_out, workspace, (cudaStream_t)cuda_stream);
+                           spin_canted ? 1 : 0, batch, 1, (c128*)M_out, info, workspace, st);
 }
 
-int lsms_tau00_batched(lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
+int lsms_build_M_shared_g0_batched(lsms_handle_t h, const lsms_c128* tinv_diag, const double* site_pos, const double* moment_dir,
+                                   const lsms_c128* kappa, int lmax, int n_sites, int spin_canted, int n_atoms, int n_energies,
+                                   lsms_c128* M_out, int* info, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    LSMS_ENTER(h);
+    if (!tinv_diag || !aligned16(tinv_diag)) return -2;
+    if (!site_pos) return -3;
+    if (spin_canted && !moment_dir) return -4;
+    if (!kappa || !aligned16(kappa)) return -5;
+    if (lmax < 0 || lmax > 8) return -6;
+    if (n_sites < 1) return -7;
+    if (n_atoms < 1) return -9;
+    if (n_energies < 1) return -10;
+    if (!M_out || !aligned16(M_out)) return -11;
+    if (!info) return -12;
+    if (!workspace || !aligned16(workspace)) return -13;
+    if (workspace_bytes < align256(gaunt_table_bytes(lmax))) return -14;
+    LSMS_BIND(h);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    LSMS_CUDA_OK(cudaMemsetAsync(info, 0, (size_t)n_atoms * n_energies * sizeof(int), st));
+    ProfScope ps(0, st);
+    return launch_assemble((const c128*)tinv_diag, site_pos, moment_dir, (const c128*)kappa, lmax, n_sites,
+                           spin_canted ? 1 : 0, n_energies, n_atoms, (c128*)M_out, info, workspace, st);
+}
+
+int lsms_tau00_batched(lsms_handle_t h, lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
                        lsms_c128* tau00_out, int* info, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    if (!M || !aligned16(M)) return -1;
-    if (n_sites < 1) return -2;
-    if (kmax < 1 || isqrt_exact(kmax) < 0 || kmax > 81) return -3;
-    if (batch < 1) return -5;
-    if (!tau00_out || !aligned16(tau00_out)) return -6;
-    if (!info) return -7;
+    LSMS_ENTER(h);
+    if (!M || !aligned16(M)) return -2;
+    if (n_sites < 1) return -3;
+    if (kmax < 1 || isqrt_exact(kmax) < 0 || kmax > 81) return -4;
+    if (batch < 1) return -6;
+    if (!tau00_out || !aligned16(tau00_out)) return -7;
+    if (!info) return -8;
     const int k = kmax * (spin_canted ? 2 : 1);
     const long long nll = (long long)n_sites * k;
-    if (nll > 46340) return -2;
+    if (nll > 46340) return -3;
     const int n = (int)nll;
-    if (!workspace || !aligned16(workspace)) return -8;
-    if (workspace_bytes < tau_ws_bytes(n, k, batch)) return -9;
+    if (!workspace || !aligned16(workspace)) return -9;
+    if (workspace_bytes < tau_ws_bytes(h, n, k, batch)) return -10;
+    LSMS_BIND(h);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    g_launches.n = 0;
-    const TauWs ws = tau_ws_layout(workspace, n, k, batch);
     LSMS_CUDA_OK(cudaMemsetAsync(info, 0, (size_t)batch * sizeof(int), st));
-    return eliminate_groups((c128*)M, n, k, batch, ws, (c128*)tau00_out, info, st);
+    return tau00_impl(h, (c128*)M, n, k, batch, (c128*)tau00_out, info, workspace, st);
 }
 
-int lsms_solve_central_column_batched(const lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
+int lsms_solve_central_column_batched(lsms_handle_t h, const lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
                                       lsms_c128* X_out, int* info, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    if (!M || !aligned16(M)) return -1;
-    if (n_sites < 1) return -2;
-    if (kmax < 1 || isqrt_exact(kmax) < 0 || kmax > 81) return -3;
-    if (batch < 1) return -5;
-    if (!X_out || !aligned16(X_out)) return -6;
-    if (!info) return -7;
-    if (!workspace || !aligned16(workspace)) return -8;
-    if (workspace_bytes < lsms_solve_workspace_bytes(n_sites, kmax, spin_canted, batch)) return -9;
+    LSMS_ENTER(h);
+    if (!M || !aligned16(M)) return -2;
+    if (n_sites < 1) return -3;
+    if (kmax < 1 || isqrt_exact(kmax) < 0 || kmax > 81) return -4;
+    if (batch < 1) return -6;
+    if (!X_out || !aligned16(X_out)) return -7;
+    if (!info) return -8;
+    if (!workspace || !aligned16(workspace)) return -9;
+    const size_t need = lsms_solve_workspace_bytes(h, n_sites, kmax, spin_canted, batch);
+    if (need == 0) return -3;
+    if (workspace_bytes < need) return -10;
+    LSMS_BIND(h);
     const int k = kmax * (spin_canted ? 2 : 1);
     const int n = n_sites * k;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -381,16 +490,18 @@ int lsms_solve_central_column_batched(const lsms_c128* M, int n_sites, int kmax,
     c128* copy = (c128*)p; p += align256((size_t)batch * n * n * sizeof(c128));
     c128* tau = (c128*)p; p += align256((size_t)batch * k * k * sizeof(c128));
     LSMS_CUDA_OK(cudaMemcpyAsync(copy, M, (size_t)batch * n * n * sizeof(c128), cudaMemcpyDeviceToDevice, st));
-    int rc = lsms_tau00_batched((lsms_c128*)copy, n_sites, kmax, spin_canted, batch, (lsms_c128*)tau, info, p,
-                                tau_ws_bytes(n, k, batch), cuda_stream);
+    LSMS_CUDA_OK(cudaMemsetAsync(info, 0, (size_t)batch * sizeof(int), st));
+    int rc = tau00_impl(h, copy, n, k, batch, tau, info, p, st);
     if (rc) return rc;
     return launch_backsolve_central(copy, (size_t)n * n, n, k, batch, tau, (c128*)X_out, st);
 }
 
-size_t lsms_host_call_scratch_bytes(int n_sites, int lmax, int spin_canted, int n_species, int batch) {
-    if (n_sites < 1 || lmax < 0 || lmax > 8 || batch < 1 || n_species < 1) return 0;
+size_t lsms_host_call_scratch_bytes(lsms_handle_t c, int n_sites, int lmax, int spin_canted, int n_species, int batch) {
+    if (!c || n_sites < 1 || lmax < 0 || lmax > 8 || batch < 1 || n_species < 1) return 0;
     int nspin = spin_canted ? 2 : 1, nl = lmax + 1, kmax = nl * nl, k = kmax * nspin;
     size_t n = (size_t)n_sites * k;
+    const size_t wsb = workspace_bytes_impl(c, n_sites, lmax, spin_canted, batch);
+    if (wsb == 0) return 0;
     size_t s = 0;
     s += align256((size_t)n_species * nspin * nl * sizeof(c128));          // delta
     s += align256((size_t)batch * n_sites * sizeof(int));                 // species
@@ -401,29 +512,34 @@ size_t lsms_host_call_scratch_bytes(int n_sites, int lmax, int spin_canted, int 
     s += align256((size_t)batch * n * n * sizeof(c128));                  // M
     s += align256((size_t)batch * k * k * sizeof(c128));                  // tau00
     s += align256((size_t)batch * sizeof(int));                           // info
-    s += lsms_workspace_bytes(n_sites, lmax, spin_canted, batch);
+    s += wsb;
     return s;
 }
 
-int lsms_tau00_from_host(const lsms_c128* delta_host, const int* species_host, const lsms_c128* z_host,
+int lsms_tau00_from_host(lsms_handle_t h, const lsms_c128* delta_host, const int* species_host, const lsms_c128* z_host,
                          const double* site_pos_host, const double* moment_dir_host,
-                         int lmax, int n_sites, int spin_canted, int n_species, int batch,
+                         int lmax, int n_sites, int spin_canted, int n_species, int batch, int n_energies,
                          lsms_c128* tau00_out_host, int* info_host,
                          void* device_scratch, size_t scratch_bytes, void* cuda_stream,
                          size_t* h2d_bytes, size_t* d2h_bytes) {
-    if (!delta_host) return -1;
-    if (!species_host) return -2;
-    if (!z_host) return -3;
-    if (!site_pos_host) return -4;
-    if (spin_canted && !moment_dir_host) return -5;
-    if (lmax < 0 || lmax > 8) return -6;
-    if (n_sites < 1) return -7;
-    if (n_species < 1) return -9;
-    if (batch < 1) return -10;
-    if (!tau00_out_host) return -11;
-    if (!info_host) return -12;
-    if (!device_scratch || !aligned16(device_scratch)) return -13;
-    if (scratch_bytes < lsms_host_call_scratch_bytes(n_sites, lmax, spin_canted, n_species, batch)) return -14;
+    LSMS_ENTER(h);
+    if (!delta_host) return -2;
+    if (!species_host) return -3;
+    if (!z_host) return -4;
+    if (!site_pos_host) return -5;
+    if (spin_canted && !moment_dir_host) return -6;
+    if (lmax < 0 || lmax > 8) return -7;
+    if (n_sites < 1) return -8;
+    if (n_species < 1) return -10;
+    if (batch < 1) return -11;
+    if (n_energies < 0 || n_energies > batch) return -12;
+    if (!tau00_out_host) return -13;
+    if (!info_host) return -14;
+    if (!device_scratch || !aligned16(device_scratch)) return -15;
+    const size_t need = lsms_host_call_scratch_bytes(h, n_sites, lmax, spin_canted, n_species, batch);
+    if (need == 0) return -8;
+    if (scratch_bytes < need) return -16;
+    LSMS_BIND(h);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int nspin = spin_canted ? 2 : 1, nl = lmax + 1, kmax = nl * nl, k = kmax * nspin;
     const size_t n = (size_t)n_sites * k;
@@ -437,25 +553,33 @@ int lsms_tau00_from_host(const lsms_c128* delta_host, const int* species_host, c
     c128* d_tinv = (c128*)take((size_t)batch * n_sites * nspin * nl * sizeof(c128)); c128* d_kappa = (c128*)take(b_z);
     c128* d_M = (c128*)take((size_t)batch * n * n * sizeof(c128));
     c128* d_tau = (c128*)take(b_tau); int* d_info = (int*)take(b_info);
-    void* ws = p; const size_t ws_bytes = lsms_workspace_bytes(n_sites, lmax, spin_canted, batch);
+    void* ws = p;
+    // f3: one g0 per energy when the host inputs show that all atoms share geometry and energies
+    int n_atoms = 1, n_e = batch;
+    if (n_energies > 0 && n_energies < batch && batch % n_energies == 0) {
+        const size_t pos_e = (size_t)n_energies * n_sites * 3 * sizeof(double), z_e = (size_t)n_energies * sizeof(c128);
+        bool same = true;
+        for (int a = 1; a < batch / n_energies && same; ++a)
+            same = memcmp((const char*)site_pos_host + a * pos_e, site_pos_host, pos_e) == 0 &&
+                   memcmp((const char*)z_host + a * z_e, z_host, z_e) == 0;
+        if (same) { n_atoms = batch / n_energies; n_e = n_energies; }
+    }
     size_t h2d = 0;
     LSMS_CUDA_OK(cudaMemcpyAsync(d_delta, delta_host, b_delta, cudaMemcpyHostToDevice, st)); h2d += b_delta;
     LSMS_CUDA_OK(cudaMemcpyAsync(d_spec, species_host, b_spec, cudaMemcpyHostToDevice, st)); h2d += b_spec;
     LSMS_CUDA_OK(cudaMemcpyAsync(d_z, z_host, b_z, cudaMemcpyHostToDevice, st)); h2d += b_z;
     LSMS_CUDA_OK(cudaMemcpyAsync(d_pos, site_pos_host, b_pos, cudaMemcpyHostToDevice, st)); h2d += b_pos;
     if (spin_canted) { LSMS_CUDA_OK(cudaMemcpyAsync(d_mom, moment_dir_host, b_pos, cudaMemcpyHostToDevice, st)); h2d += b_pos; }
-    int rc = lsms_tinv_from_phase_shifts((lsms_c128*)d_delta, d_spec, (lsms_c128*)d_z, lmax, n_sites, spin_canted, n_species, batch,
-                                         (lsms_c128*)d_tinv, (lsms_c128*)d_kappa, cuda_stream);
+    // info is cleared once; every stage records only the FIRST non-zero code of an item
+    LSMS_CUDA_OK(cudaMemsetAsync(d_info, 0, b_info, st));
+    int rc = launch_tinv(d_delta, d_spec, d_z, lmax, n_sites, nspin, n_species, batch, d_tinv, d_kappa, d_info, st);
     if (rc) return rc;
-    int launches = g_launches.n;
-    rc = lsms_build_M_batched((lsms_c128*)d_tinv, d_pos, spin_canted ? d_mom : nullptr, (lsms_c128*)d_kappa, lmax, n_sites, spin_canted,
-                              batch, (lsms_c128*)d_M, ws, ws_bytes, cuda_stream);
+    { ProfScope ps(0, st);
+      rc = launch_assemble(d_tinv, d_pos, spin_canted ? d_mom : nullptr, d_kappa, lmax, n_sites, spin_canted ? 1 : 0, n_e, n_atoms,
+                           d_M, d_info, ws, st); }
     if (rc) return rc;
-    launches += g_launches.n;
-    rc = lsms_tau00_batched((lsms_c128*)d_M, n_sites, kmax, spin_canted, batch, (lsms_c128*)d_tau, d_info, ws, ws_bytes, cuda_stream);
+    rc = tau00_impl(h, d_M, (int)n, k, batch, d_tau, d_info, ws, st);
     if (rc) return rc;
-    launches += g_launches.n;
-    g_launches.n = launches;
     LSMS_CUDA_OK(cudaMemcpyAsync(tau00_out_host, d_tau, b_tau, cudaMemcpyDeviceToHost, st));
     LSMS_CUDA_OK(cudaMemcpyAsync(info_host, d_info, b_info, cudaMemcpyDeviceToHost, st));
     LSMS_CUDA_OK(cudaStreamSynchronize(st));
@@ -464,89 +588,71 @@ int lsms_tau00_from_host(const lsms_c128* delta_host, const int* species_host, c
     return 0;
 }
 
-int lsms_contour_sum_batched(const lsms_c128* tau00, const lsms_c128* weights, int n_atoms, int n_energies, int k,
+int lsms_contour_sum_batched(lsms_handle_t h, const lsms_c128* tau00, const lsms_c128* weights, int n_atoms, int n_energies, int k,
                              lsms_c128* out, void* cuda_stream) {
-    if (!tau00 || !aligned16(tau00)) return -1;
-    if (!weights || !aligned16(weights)) return -2;
-    if (n_atoms < 1) return -3;
-    if (n_energies < 1 || n_energies > 2048) return -4;
-    if (k < 1 || k > 4096) return -5;
-    if (!out || !aligned16(out)) return -6;
-    g_launches.n = 0;
+    LSMS_ENTER(h);
+    if (!tau00 || !aligned16(tau00)) return -2;
+    if (!weights || !aligned16(weights)) return -3;
+    if (n_atoms < 1) return -4;
+    if (n_energies < 1 || n_energies > 2048) return -5;
+    if (k < 1 || k > 4096) return -6;
+    if (!out || !aligned16(out)) return -7;
+    LSMS_BIND(h);
     return launch_contour_sum((const c128*)tau00, (const c128*)weights, n_atoms, n_energies, k * k, (c128*)out, (cudaStream_t)cuda_stream);
 }
 
-int lsms_set_blocking(int nb_outer, int ib_inner) {
-    if (nb_outer < 0 || nb_outer > 96 || (nb_outer % 4) != 0) return -1;
-    if (ib_inner < 0 || ib_inner > 16) return -2;
-    g_nb_outer = nb_outer; g_ib_inner = ib_inner;
+// ---------------------------------------------------------------- include/lsms_tau_diag.h
+
+int lsms_last_launch_count(lsms_handle_t h) { return h ? h->last_launches : -1; }
+int lsms_last_schedule(lsms_handle_t h) { return h ? h->last_schedule : -1; }
+
+int lsms_profile_begin(lsms_handle_t h) {
+    if (!h) return -1;
+    h->prof.on = true; h->prof.used = 0;
+    for (int i = 0; i < 8; ++i) h->prof.flops[i] = 0.0;
     return 0;
 }
 
-int lsms_set_lookahead(int on) { g_lookahead = on ? 1 : 0; return 0; }
-
-int lsms_set_align_first(int on) { g_align_first = on ? 1 : 0; return 0; }
-
-int lsms_set_panel_cluster(int cl) {
-    if (cl != 0 && cl != 1 && cl != 2 && cl != 4 && cl != 8) return -1;
-    g_panel_cluster = cl;
-    return 0;
-}
-
-int lsms_set_panel_variant(int variant) {
-    if (variant < -1 || variant > 1) return -1;
-    g_panel_variant = variant;
-    return 0;
-}
-
-int lsms_set_groups(int groups) {
-    if (groups < 0 || groups > MAX_GROUPS) return -1;
-    g_groups = groups;
-    return 0;
-}
-
-int lsms_last_launch_count(void) { return g_launches.n; }
-
-int lsms_profile_begin(void) {
-    g_prof.on = true; g_prof.used = 0;
-    for (int i = 0; i < 8; ++i) g_prof.flops[i] = 0.0;
-    return 0;
-}
-
-int lsms_profile_end(double* ms_by_class_host, int* launches_by_class_host, double* flops_by_class_host) {
-    if (!ms_by_class_host) return -1;
-    if (!launches_by_class_host) return -2;
-    if (!flops_by_class_host) return -3;
-    g_prof.on = false;
-    for (int i = 0; i < 8; ++i) { ms_by_class_host[i] = 0.0; launches_by_class_host[i] = 0; flops_by_class_host[i] = g_prof.flops[i]; }
-    for (size_t i = 0; i < g_prof.used; ++i) {
-        LSMS_CUDA_OK(cudaEventSynchronize(g_prof.ev[2 * i + 1]));
+int lsms_profile_end(lsms_handle_t h, double* ms_by_class_host, int* launches_by_class_host, double* flops_by_class_host) {
+    if (!h) return -1;
+    if (!ms_by_class_host) return -2;
+    if (!launches_by_class_host) return -3;
+    if (!flops_by_class_host) return -4;
+    Prof& p = h->prof;
+    p.on = false;
+    for (int i = 0; i < 8; ++i) { ms_by_class_host[i] = 0.0; launches_by_class_host[i] = 0; flops_by_class_host[i] = p.flops[i]; }
+    for (size_t i = 0; i < p.used; ++i) {
+        LSMS_CUDA_OK(cudaEventSynchronize(p.ev[2 * i + 1]));
         float ms = 0.f;
-        LSMS_CUDA_OK(cudaEventElapsedTime(&ms, g_prof.ev[2 * i], g_prof.ev[2 * i + 1]));
-        ms_by_class_host[g_prof.cls[i]] += ms; launches_by_class_host[g_prof.cls[i]] += 1;
+        LSMS_CUDA_OK(cudaEventElapsedTime(&ms, p.ev[2 * i], p.ev[2 * i + 1]));
+        ms_by_class_host[p.cls[i]] += ms; launches_by_class_host[p.cls[i]] += 1;
     }
-    g_prof.used = 0;
+    p.used = 0;
     return 0;
 }
 
-int lsms_fp64_peak_probe(int which, int iters, double* tflops_host, void* cuda_stream) {
-    if (which < 0 || which > 1) return -1;
-    if (iters < 1) return -2;
-    if (!tflops_host) return -3;
-    return run_peak_probe(which, iters, tflops_host, (cudaStream_t)cuda_stream);
+int lsms_fp64_peak_probe(lsms_handle_t h, int which, int iters, double* sink, double* tflops_host, void* cuda_stream) {
+    LSMS_ENTER(h);
+    if (which < 0 || which > 1) return -2;
+    if (iters < 1) return -3;
+    if (!sink) return -4;
+    if (!tflops_host) return -5;
+    LSMS_BIND(h);
+    return run_peak_probe(which, iters, sink, tflops_host, (cudaStream_t)cuda_stream);
 }
 
-int lsms_schur_update_batched(lsms_c128* M, int n, int c0, int kk, int batch, void* cuda_stream) {
-    if (!M || !aligned16(M)) return -1;
-    if (n < 2) return -2;
-    if (c0 < 0 || kk < 1 || c0 + kk >= n) return -3;
-    if (batch < 1) return -5;
+int lsms_schur_update_batched(lsms_handle_t h, lsms_c128* M, int n, int c0, int kk, int batch, void* cuda_stream) {
+    LSMS_ENTER(h);
+    if (!M || !aligned16(M)) return -2;
+    if (n < 2) return -3;
+    if (c0 < 0 || kk < 1 || c0 + kk >= n) return -4;
+    if (batch < 1) return -6;
+    LSMS_BIND(h);
     GemmShape g; g.strideA = g.strideB = g.strideC = (size_t)n * n; g.ldA = g.ldB = g.ldC = n; g.batch = batch; g.beta0 = 0;
     const int r0 = c0 + kk;
     c128* base = (c128*)M;
     g.Mr = n - r0; g.Nc = n - r0; g.K = kk;
     g.A = base + (size_t)r0 + (size_t)c0 * n; g.B = base + (size_t)c0 + (size_t)r0 * n; g.C = base + (size_t)r0 + (size_t)r0 * n;
-    g_launches.n = 0;
     return launch_schur_gemm(g, (cudaStream_t)cuda_stream);
 }
 

@@ -85,24 +85,41 @@ __device__ inline c128 csqrt_upper(c128 z) {       // principal root with Im >= 
     return k;
 }
 
+// Reading A4 / include/lsms_tau.h: illegal input VALUES are reported per item (first non-zero code wins, no sync):
+//   -4 z non-finite or Im z < 0,  -2 species index out of range,  -1 phase shift non-finite or sin(delta) = 0.
+__device__ __forceinline__ bool finite2(c128 a) { return isfinite(a.x) && isfinite(a.y); }
+
 __global__ void k_tinv(const c128* __restrict__ delta, const int* __restrict__ species, const c128* __restrict__ z,
-                       int lmax, int n_sites, int nspin, int batch, c128* __restrict__ tinv, c128* __restrict__ kappa) {
+                       int lmax, int n_sites, int nspin, int n_species, int batch, c128* __restrict__ tinv, c128* __restrict__ kappa,
+                       int* __restrict__ info) {
     int nl = lmax + 1;
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     long long total = (long long)batch * n_sites * nspin * nl;
-    if (e < batch) kappa[e] = csqrt_upper(z[e]);
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+    if (e < batch) {
+        const c128 zz = z[e];
+        const bool bad = !finite2(zz) || zz.y < 0.0;
+        kappa[e] = bad ? cmake(qnan, qnan) : csqrt_upper(zz);
+        if (bad) atomicCAS(&info[e], 0, -4);
+    }
     if (e >= total) return;
     int l = (int)(e % nl); long long r = e / nl;
     int s = (int)(r % nspin); r /= nspin;
     int site = (int)(r % n_sites); int b = (int)(r / n_sites);
-    c128 kap = csqrt_upper(z[b]);
-    c128 d = delta[((size_t)species[(size_t)b * n_sites + site] * nspin + s) * nl + l];
+    const c128 zz = z[b];
+    const bool zbad = !finite2(zz) || zz.y < 0.0;
+    const int sp = species[(size_t)b * n_sites + site];
+    if (sp < 0 || sp >= n_species) { atomicCAS(&info[b], 0, -2); tinv[e] = cmake(qnan, qnan); return; }
+    c128 kap = csqrt_upper(zz);
+    c128 d = delta[((size_t)sp * nspin + s) * nl + l];
     // sin(a+ib) = sin a cosh b + i cos a sinh b ;  e^{i(a+ib)} = e^{-b}(cos a + i sin a)
     double sa, ca; sincos(d.x, &sa, &ca);
     double eb = exp(-d.y);
     c128 sn = cmake(sa * cosh(d.y), ca * sinh(d.y));
     c128 ex = cmake(eb * ca, eb * sa);
-    tinv[e] = cneg(cdiv(kap, cmul(sn, ex)));       // -kappa / (sin d e^{i d})
+    c128 t = cneg(cdiv(kap, cmul(sn, ex)));       // -kappa / (sin d e^{i d})
+    if (!zbad && (!finite2(d) || !finite2(t))) atomicCAS(&info[b], 0, -1);
+    tinv[e] = zbad ? cmake(qnan, qnan) : t;
 }
 
 // ---------------------------------------------------------------- Legendre recurrence table
@@ -137,7 +154,7 @@ __global__ void __launch_bounds__(ASM_THREADS)
 k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, const double* __restrict__ moment,
            const c128* __restrict__ kappa, const c128* __restrict__ coef, const int* __restrict__ idx,
            const double* __restrict__ leg, int lmax, int n_sites, int canted, int chunk, int n_rep, int rep_stride,
-           c128* __restrict__ Mout) {
+           c128* __restrict__ Mout, int* __restrict__ info) {
     extern __shared__ __align__(16) unsigned char asm_smem[];
     const int kmax = (lmax + 1) * (lmax + 1), nt = lmax + 1, l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
     const int nspin = canted ? 2 : 1, k = kmax * nspin, kk2 = kmax * kmax, S = nl2;
@@ -148,8 +165,16 @@ k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, c
     const size_t rep_elems = (size_t)rep_stride * n * n;
     const int nrep = REP ? n_rep : 1;
     const size_t c0 = (size_t)(sj == 0 ? n_sites - 1 : sj - 1) * k;
-    const c128 kap = kappa[b];
-    const c128 zero = cmake(0.0, 0.0);
+    // reading A4: Im kappa < 0 (the wrong sheet: h_l would grow with R) or a non-finite kappa rejects the item:
+    // info = -5 and the whole matrix becomes NaN (kappa := NaN poisons every g0 and, below, every t^{-1} entry)
+    c128 kap = kappa[b];
+    const bool kbad = !(isfinite(kap.x) && isfinite(kap.y)) || kap.y < 0.0;
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+    if (kbad) {
+        kap = cmake(qnan, qnan);
+        if (sj == 0) for (int a = tid; a < nrep; a += ASM_THREADS) atomicCAS(&info[(size_t)b + (size_t)a * rep_stride], 0, -5);
+    }
+    const c128 zero = kbad ? cmake(qnan, qnan) : cmake(0.0, 0.0);     // also the "zero" entries of a rejected item
     const double* pj = site_pos + ((size_t)b * n_sites + sj) * 3;
     const double xj = pj[0], yj = pj[1], zj = pj[2];
 
@@ -244,10 +269,10 @@ k_assemble(const c128* __restrict__ tinv, const double* __restrict__ site_pos, c
                             const c128* ti = tinv + (item * n_sites + si) * nspin * nt;
                             c128* cp = colp + (size_t)a * rep_elems;
                             if (!canted) {
-                                cp[rowb] = dg ? ti[lL] : zero;
+                                cp[rowb] = (dg && !kbad) ? ti[lL] : zero;
                             } else {
                                 const double* mv = moment + (item * n_sites + si) * 3;
-                                const c128 ta = ti[lL], tb = ti[nt + lL];
+                                const c128 ta = kbad ? zero : ti[lL], tb = kbad ? zero : ti[nt + lL];
                                 const c128 hsum = cscale(0.5, cadd(ta, tb)), hdif = cscale(0.5, csub(ta, tb));
                                 cp[rowb] = dg ? cadd(hsum, cscale(mv[2], hdif)) : zero;                         // (up, up)
                                 cp[rowb + kmax] = dg ? cmul(hdif, cmake(mv[0], mv[1])) : zero;                  // (down, up): ex + i ey
@@ -272,20 +297,31 @@ size_t gaunt_table_bytes(int lmax) {
     return al256(e * sizeof(c128)) + al256(e * sizeof(int)) + al256(3 * S * sizeof(double));
 }
 
-int launch_tinv(const c128* delta, const int* species, const c128* z, int lmax, int n_sites, int nspin, int batch,
-                c128* tinv, c128* kappa, cudaStream_t st) {
+int launch_tinv(const c128* delta, const int* species, const c128* z, int lmax, int n_sites, int nspin, int n_species, int batch,
+                c128* tinv, c128* kappa, int* info, cudaStream_t st) {
     long long total = (long long)batch * n_sites * nspin * (lmax + 1);
     if (total < batch) total = batch;
     int thr = 256; long long blocks = (total + thr - 1) / thr;
-    k_tinv<<<(unsigned)blocks, thr, 0, st>>>(delta, species, z, lmax, n_sites, nspin, batch, tinv, kappa);
+    k_tinv<<<(unsigned)blocks, thr, 0, st>>>(delta, species, z, lmax, n_sites, nspin, n_species, batch, tinv, kappa, info);
     LSMS_LAUNCH_CHECK();
     return 0;
 }
 
 // n_rep > 1: de-duplicated assembly -- `batch` then counts the DISTINCT (geometry, kappa) items (the energies); item
 // e + a*batch, a < n_rep, shares the geometry and kappa of item e and differs in tinv / moments only.
+int init_attrs_assemble() {
+    const int smem = 56 * 1024;
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_assemble<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_assemble<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_assemble<9, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_assemble<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_assemble<5, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_assemble<9, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    return 0;
+}
+
 int launch_assemble(const c128* tinv, const double* site_pos, const double* moment, const c128* kappa, int lmax,
-                    int n_sites, int canted, int batch, int n_rep, c128* M, void* ws, cudaStream_t st) {
+                    int n_sites, int canted, int batch, int n_rep, c128* M, int* info, void* ws, cudaStream_t st) {
     size_t kmax = (size_t)(lmax + 1) * (lmax + 1), nt = lmax + 1, e = kmax * kmax * nt;
     const int l2 = 2 * lmax, nl2 = (l2 + 1) * (l2 + 1);
     c128* coef = (c128*)ws;
@@ -304,14 +340,13 @@ int launch_assemble(const c128* tinv, const double* site_pos, const double* mome
     const size_t smem = (size_t)chunk * nl2 * sizeof(c128);
     const size_t k = kmax * (canted ? 2 : 1), n = (size_t)n_sites * k;
     auto run = [&](auto kern) -> int {
-        LSMS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(56 * 1024)));
         for (int b0 = 0; b0 < batch; b0 += 65535) {
             int nb = batch - b0 < 65535 ? batch - b0 : 65535;
             dim3 grid(n_sites, nb);
             kern<<<grid, ASM_THREADS, smem, st>>>(tinv + (size_t)b0 * n_sites * (canted ? 2 : 1) * nt,
                                                   site_pos + (size_t)b0 * n_sites * 3,
                                                   moment ? moment + (size_t)b0 * n_sites * 3 : nullptr, kappa + b0, coef, idx, leg,
-                                                  lmax, n_sites, canted, chunk, n_rep, batch, M + (size_t)b0 * n * n);
+                                                  lmax, n_sites, canted, chunk, n_rep, batch, M + (size_t)b0 * n * n, info + b0);
             LSMS_LAUNCH_CHECK();
         }
         return 0;

@@ -173,11 +173,6 @@ k_schur_gemm(GemmShape g, int tiles_m) {
 
 template <int STAGES, int BN>
 static int launch_classic(const GemmShape& g, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<STAGES, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<STAGES, BN>()));
-        attr_set = true;
-    }
     const int tiles_m = (g.Mr + BM - 1) / BM, tiles_n = (g.Nc + BN - 1) / BN;
     for (int b0 = 0; b0 < g.batch; b0 += 65535) {
         GemmShape h = g;
@@ -199,6 +194,12 @@ static int launch_classic(const GemmShape& g, cudaStream_t st) {
 // traffic): the same 64 x 32 tiles with one ring stage (6.2 -> 4.9 ms per P step against 64 x 64 tiles).  Tried and dropped: a one-DMMA-per-accumulator loop body with operands picked by 64-bit loads
 // (31.7 TFLOP/s, bank-conflicted LDS.64) and a persistent one-CTA-per-SM variant with the next C tile prefetched
 // into shared memory (23.3 TFLOP/s).
+int init_attrs_gemm() {
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<1, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<1, 32>()));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<2, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<2, 32>()));
+    return 0;
+}
+
 int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
     if (g.Mr <= 0 || g.Nc <= 0 || g.K <= 0 || g.batch <= 0) return 0;
     if (g.K <= KS) return launch_classic<1, 32>(g, st);

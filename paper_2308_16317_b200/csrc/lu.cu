@@ -1,161 +1,11 @@
-// lu.cu -- K2 (panel LU with restricted partial pivoting), K3 (row interchanges + unit-lower
-// triangular solve), K5 (inverse of the final k x k Schur complement) and the verification-only
-// back-substitution.  SURVEY.md 8(a) a3, a4, a6; "LU factorization of the matrix" PAPER.md:92;
-// "only the first block of the inverted matrix is needed" PAPER.md:62.
-//
-// Pivot rule (reading A14): for the first ne = n-k columns the pivot search covers rows
-// [j, ne) only, so the central-site rows are updated but never selected; the trailing k x k block
-// is then exactly the Schur complement D - C A^{-1} B of the central site.
+// lu.cu -- K3a/K3b (net row permutation of an outer panel, -(L11^-1), row gather/scatter of the trailing
+// columns), K5 (inverse of the final k x k Schur complement) and the verification-only back-substitution.
+// SURVEY.md 8(a) a4, a6; "LU factorization of the matrix" PAPER.md:92; "only the first block of the inverted
+// matrix is needed" PAPER.md:62.  (K2, the panel factorisation itself, is in panel.cu / panel_cluster.cu.)
 #include "common.cuh"
 #include "internal.h"
 
 namespace lsms {
-
-constexpr int PANEL_THREADS = 256;     // 256 x 128 regs: fits beside one Schur-update CTA (look-ahead)
-constexpr int MAX_IB = 16;
-
-// ---------------------------------------------------------------- K2: panel factorisation
-// One CTA per matrix.  Columns [c0, c0+w) of rows [c0, n); w <= MAX_IB.  Unblocked right-looking
-// elimination inside the panel; the max search of column j+1 is fused into the update of step j.
-__global__ void __launch_bounds__(PANEL_THREADS)
-k_panel(c128* __restrict__ base, size_t stride, int n, int c0, int w, int ne, int* __restrict__ piv, int* __restrict__ info) {
-    c128* A = base + (size_t)blockIdx.x * stride;
-    int* pv = piv + (size_t)blockIdx.x * n;
-    __shared__ c128 urow[MAX_IB];
-    __shared__ double red_v[PANEL_THREADS / 32];
-    __shared__ int red_i[PANEL_THREADS / 32];
-    __shared__ int s_piv;
-    __shared__ int s_bad;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-
-    // candidate of this thread for the current column: (value, row); rows j..ne-1
-    double bv = -1.0; int bi = 0x7fffffff;
-    for (int i = c0 + tid; i < ne; i += PANEL_THREADS) {
-        double v = cabs1(A[i + (size_t)c0 * n]);
-        if (v > bv) { bv = v; bi = i; }
-    }
-    for (int jj = 0; jj < w; ++jj) {
-        const int j = c0 + jj;
-        // ---- block arg-max (ties -> smallest row)
-        double v = bv; int ix = bi;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            double ov = __shfl_xor_sync(0xffffffffu, v, o); int oi = __shfl_xor_sync(0xffffffffu, ix, o);
-            if (ov > v || (ov == v && oi < ix)) { v = ov; ix = oi; }
-        }
-        if (lane == 0) { red_v[warp] = v; red_i[warp] = ix; }
-        __syncthreads();
-        if (warp == 0) {
-            v = (lane < PANEL_THREADS / 32) ? red_v[lane] : -1.0; ix = (lane < PANEL_THREADS / 32) ? red_i[lane] : 0x7fffffff;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                double ov = __shfl_xor_sync(0xffffffffu, v, o); int oi = __shfl_xor_sync(0xffffffffu, ix, o);
-                if (ov > v || (ov == v && oi < ix)) { v = ov; ix = oi; }
-            }
-            if (lane == 0) {
-                const bool bad = !(v > 0.0) || !(v < 1.0e300 * 1.0e300);     // zero, NaN or Inf pivot
-                s_bad = bad ? 1 : 0;
-                s_piv = bad ? j : ix;
-                pv[j] = bad ? j : ix;
-                if (bad) atomicCAS(&info[blockIdx.x], 0, j + 1);
-            }
-        }
-        __syncthreads();
-        const int p = s_piv;
-        const bool bad = s_bad != 0;
-        // ---- swap rows j and p inside the panel, publish the pivot row
-        if (tid < w) {
-            c128 a = A[j + (size_t)(c0 + tid) * n];
-            if (p != j) { c128 bq = A[p + (size_t)(c0 + tid) * n]; A[p + (size_t)(c0 + tid) * n] = a; A[j + (size_t)(c0 + tid) * n] = bq; a = bq; }
-            urow[tid] = a;
-        }
-        __syncthreads();
-        // ---- scale column j, rank-1 update of the remaining panel columns, next column's max
-        bv = -1.0; bi = 0x7fffffff;
-        if (!bad) {
-            const c128 rp = crecip(urow[jj]);
-            // all loads of a row are issued before any of its stores (independent L2 round trips in
-            // flight instead of one dependent load->fma->store chain per column)
-            for (int i = j + 1 + tid; i < n; i += PANEL_THREADS) {
-                c128 a[MAX_IB];
-                const c128 l0 = A[i + (size_t)j * n];
-#pragma unroll
-                for (int t = 1; t < MAX_IB; ++t)
-                    if (jj + t < w) a[t] = A[i + (size_t)(j + t) * n];
-                const c128 l = cmul(l0, rp);
-                A[i + (size_t)j * n] = l;
-#pragma unroll
-                for (int t = 1; t < MAX_IB; ++t)
-                    if (jj + t < w) {
-                        cfms(a[t], l, urow[jj + t]);
-                        A[i + (size_t)(j + t) * n] = a[t];
-                    }
-                if (jj + 1 < w && i < ne) { double vv = cabs1(a[1]); if (vv > bv) { bv = vv; bi = i; } }
-            }
-        } else if (jj + 1 < w) {
-            for (int i = j + 1 + tid; i < ne; i += PANEL_THREADS) {
-                double vv = cabs1(A[i + (size_t)(j + 1) * n]);
-                if (vv > bv) { bv = vv; bi = i; }
-            }
-        }
-        __syncthreads();
-    }
-}
-
-// ---------------------------------------------------------------- K3: interchanges + U12 = L11^{-1} A12
-// One thread per target column c in [col_lo, col_hi) (columns of the panel itself are skipped by the
-// caller's ranges).  mode bit 0: apply the w interchanges of panel [c0, c0+w) in order; mode bit 1:
-// solve the w x w unit-lower triangle L11 against rows [c0, c0+w) of the column.
-constexpr int K3_THREADS = 128;
-
-__global__ void __launch_bounds__(K3_THREADS)
-k_swap_trsm(c128* __restrict__ base, size_t stride, int n, int c0, int w, int col_lo, int col_hi, int mode,
-            const int* __restrict__ piv) {
-    const bool do_swap = mode & 1, do_trsm = mode & 2;
-    c128* A = base + (size_t)blockIdx.y * stride;
-    const int* pv = piv + (size_t)blockIdx.y * n + c0;
-    __shared__ c128 L[MAX_IB * MAX_IB];
-    __shared__ int sp[MAX_IB];
-    if (threadIdx.x < w) sp[threadIdx.x] = pv[threadIdx.x];
-    if (do_trsm)
-        for (int e = threadIdx.x; e < w * w; e += K3_THREADS) { int r = e % w, c = e / w; L[r + MAX_IB * c] = A[(c0 + r) + (size_t)(c0 + c) * n]; }
-    __syncthreads();
-    const int c = col_lo + blockIdx.x * K3_THREADS + threadIdx.x;
-    if (c >= col_hi) return;
-    c128* col = A + (size_t)c * n;
-    c128 x[MAX_IB];
-#pragma unroll
-    for (int i = 0; i < MAX_IB; ++i) x[i] = (i < w) ? col[c0 + i] : cmake(0.0, 0.0);
-    // interchanges, in order (a row index may appear more than once)
-#pragma unroll
-    for (int i = 0; i < MAX_IB; ++i) {
-        if (do_swap && i < w) {
-            const int p = sp[i];
-            if (p != c0 + i) {
-                if (p < c0 + w) {
-                    // both rows are in registers: static indexing through a select chain
-                    c128 xi = x[i], xp = xi;
-#pragma unroll
-                    for (int t = 0; t < MAX_IB; ++t) if (t == p - c0) xp = x[t];
-#pragma unroll
-                    for (int t = 0; t < MAX_IB; ++t) if (t == p - c0) x[t] = xi;
-                    x[i] = xp;
-                } else {
-                    c128 t = col[p]; col[p] = x[i]; x[i] = t;
-                }
-            }
-        }
-    }
-    if (do_trsm) {
-#pragma unroll
-        for (int j = 0; j < MAX_IB; ++j)
-#pragma unroll
-            for (int i = j + 1; i < MAX_IB; ++i)
-                if (i < w) cfms(x[i], L[i + MAX_IB * j], x[j]);
-    }
-#pragma unroll
-    for (int i = 0; i < MAX_IB; ++i) if (i < w) col[c0 + i] = x[i];
-}
 
 // ---------------------------------------------------------------- K3a: after an outer panel
 // One CTA per matrix, once the outer panel [J, J+W) is fully factored:
@@ -431,21 +281,12 @@ k_backsolve_central(const c128* __restrict__ LU, size_t stride, int n, int k, co
 
 // ---------------------------------------------------------------- host launchers
 
-int launch_panel(c128* base, size_t stride, int n, int c0, int w, int ne, int batch, int* piv, int* info, cudaStream_t st) {
-    k_panel<<<batch, PANEL_THREADS, 0, st>>>(base, stride, n, c0, w, ne, piv, info);
-    LSMS_LAUNCH_CHECK();
-    return 0;
-}
-
-int launch_swap_trsm(c128* base, size_t stride, int n, int c0, int w, int col_lo, int col_hi, int mode, int batch,
-                     const int* piv, cudaStream_t st) {
-    if (col_hi <= col_lo) return 0;
-    for (int b0 = 0; b0 < batch; b0 += 65535) {
-        int nb = batch - b0 < 65535 ? batch - b0 : 65535;
-        dim3 grid((col_hi - col_lo + K3_THREADS - 1) / K3_THREADS, nb);
-        k_swap_trsm<<<grid, K3_THREADS, 0, st>>>(base + (size_t)b0 * stride, stride, n, c0, w, col_lo, col_hi, mode, piv + (size_t)b0 * n);
-        LSMS_LAUNCH_CHECK();
-    }
+int init_attrs_lu() {
+    // largest outer panel the ABI accepts: W = 96 (LSMS_OPT_NB_OUTER)
+    const size_t Wp = 96;
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_panel_post, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)((Wp * Wp + 16 * Wp) * sizeof(c128) + 3 * Wp * sizeof(int))));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_final_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 96 * 16));
     return 0;
 }
 
@@ -453,8 +294,6 @@ int launch_panel_post(const c128* base, size_t stride, int n, int J, int W, int 
                       int nbmax, cudaStream_t st) {
     const size_t Wp = (size_t)(W + 15) / 16 * 16;
     size_t smem = (Wp * Wp + 16 * Wp) * sizeof(c128) + 3 * (size_t)W * sizeof(int);
-    static size_t attr = 0;
-    if (smem > attr && smem > 48 * 1024) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_panel_post, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     k_panel_post<<<batch, POST_THREADS, smem, st>>>(base, stride, n, J, W, piv, perm, ninv, nbmax);
     LSMS_LAUNCH_CHECK();
     return 0;
@@ -464,8 +303,6 @@ int launch_row_permute(c128* base, size_t stride, int n, int J, int W, int col_l
                        c128* tperm, size_t tperm_stride, int nbmax, cudaStream_t st) {
     if (col_hi <= col_lo) return 0;
     size_t smem = (size_t)PERM_TN * W * sizeof(c128) + (1 + 3 * (size_t)W) * sizeof(int);
-    static size_t attr = 0;
-    if (smem > attr && smem > 48 * 1024) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_row_permute, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = smem; }
     for (int b0 = 0; b0 < batch; b0 += 65535) {
         int nb = batch - b0 < 65535 ? batch - b0 : 65535;
         dim3 grid((col_hi - col_lo + PERM_TN - 1) / PERM_TN, nb);
@@ -479,8 +316,6 @@ int launch_row_permute(c128* base, size_t stride, int n, int J, int W, int col_l
 int launch_final_inverse(c128* base, size_t stride, int n, int k, int batch, c128* tau, int* info, void* ws, cudaStream_t st) {
     const int use_smem = k <= 96;
     size_t smem = use_smem ? (size_t)k * k * sizeof(c128) : 0;
-    static bool attr_set = false;
-    if (!attr_set) { LSMS_CUDA_OK(cudaFuncSetAttribute(k_final_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 96 * 16)); attr_set = true; }
     k_final_inverse<<<batch, K5_THREADS, smem, st>>>(base, stride, n, k, tau, info, (c128*)ws, use_smem);
     LSMS_LAUNCH_CHECK();
     return 0;

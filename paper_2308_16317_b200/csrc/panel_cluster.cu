@@ -61,6 +61,8 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
     const int ncand = NW * (int)ncl;
     const c128 zero = cmake(0.0, 0.0);
 
+    // every CTA of the cluster must be running before its shared memory is written from another CTA
+    pc_sync();
     for (int s0 = 0; s0 < w; s0 += S) {
         const int cs = c0 + s0, sw = min(S, w - s0);
         // ---- 1: sub-panel -> registers

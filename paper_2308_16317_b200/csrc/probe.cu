@@ -42,12 +42,11 @@ __global__ void __launch_bounds__(256) k_probe_dfma(int iters, double* out) {
     if (s == 123.456) out[0] = s;
 }
 
-int run_peak_probe(int which, int iters, double* tflops, cudaStream_t st) {
+int run_peak_probe(int which, int iters, double* sink, double* tflops, cudaStream_t st) {
     int dev = 0, sms = 0;
     LSMS_CUDA_OK(cudaGetDevice(&dev));
     LSMS_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    double* dummy = nullptr;
-    LSMS_CUDA_OK(cudaMalloc(&dummy, 8));
+    double* dummy = sink;
     cudaEvent_t e0, e1;
     LSMS_CUDA_OK(cudaEventCreate(&e0)); LSMS_CUDA_OK(cudaEventCreate(&e1));
     const int ctas = sms * 2, thr = 256;      // 16 warps per SM: enough to saturate the DMMA pipe
@@ -64,7 +63,7 @@ int run_peak_probe(int which, int iters, double* tflops, cudaStream_t st) {
     if (which == 0) flops = (double)ctas * (thr / 32) * (double)iters * PROBE_ACC * 512.0;   // 8*8*4 FMA = 512 flop per warp MMA
     else flops = (double)ctas * thr * (double)iters * PROBE_ACC * 2.0;
     *tflops = flops / (ms * 1e-3) / 1e12;
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(dummy);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
     return 0;
 }
 

@@ -5,6 +5,7 @@ three steps of iterative refinement with the residual in long double, SURVEY.md 
 be compared element by element at full size where the oracle needs minutes per item (H: cond_1 up to 1.6e6).
 
     python tests/golden/make_golden_full_size.py            # ~10 min on 4 cores; calls nothing but oracle/ and synth_liz/
+    python tests/golden/make_golden_full_size.py NC:5       # only the named workload:item cases (NC: ~1 h on one core)
 
 Format: line 1 '# workload item n k', then k*k lines 'row col re im' with 17 significant digits.
 """
@@ -19,7 +20,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 sys.path.insert(0, ROOT)
 
-CASES = (("H", 0), ("H", 23), ("N", 23), ("C", 24))
+CASES = (("H", 0), ("H", 23), ("N", 23), ("C", 24), ("NC", 5), ("P", 24))
 
 
 def one(case):
@@ -42,6 +43,7 @@ def one(case):
 
 if __name__ == "__main__":
     os.environ.setdefault("OMP_NUM_THREADS", "1")
-    with ProcessPoolExecutor(max_workers=min(4, len(CASES))) as ex:
-        for p in ex.map(one, CASES):
+    cases = tuple((a.split(":")[0], int(a.split(":")[1])) for a in sys.argv[1:]) or CASES
+    with ProcessPoolExecutor(max_workers=min(4, len(cases))) as ex:
+        for p in ex.map(one, cases):
             print("wrote", p)

@@ -12,51 +12,83 @@ import paper_2308_16317_b200 as lt
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def header_functions():
-    src = open(os.path.join(ROOT, "include", "lsms_tau.h")).read()
+def header_functions(name):
+    src = open(os.path.join(ROOT, "include", name)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(lsms_[a-zA-Z0-9_]+)\s*\(", src)))
 
 
 def test_library_loads_and_exports_every_declared_symbol():
+    """Both headers: the method's boundary (lsms_tau.h) and the measurement/debug exports (lsms_tau_diag.h)."""
     L = lt.lib()
-    names = header_functions()
-    assert len(names) >= 12
-    for name in names:
+    method, diag = header_functions("lsms_tau.h"), header_functions("lsms_tau_diag.h")
+    assert len(method) >= 12 and len(diag) >= 6 and not set(method) & set(diag)
+    for name in method + diag:
         assert hasattr(L, name), name
-    assert set(names) == set(lt.EXPORTS)
+    assert set(method + diag) == set(lt.EXPORTS)
+    # nothing that measures or debugs is declared in the method's header
+    assert not [n for n in method if any(w in n for w in ("profile", "probe", "debug", "launch_count", "schedule", "schur_update"))]
+    # the library exports nothing beyond the two headers (no process-wide knobs left)
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", lt.LIB_PATH], capture_output=True, text=True).stdout
+    exported = sorted(set(re.findall(r"\b(lsms_[a-zA-Z0-9_]+)\b", out)))
+    assert exported == sorted(method + diag), set(exported) ^ set(method + diag)
     assert "sm_100a" in lt.lsms_version()
 
 
-def test_workspace_queries():
-    assert lt.lsms_workspace_bytes(135, 3, False, 128) >= 128 * 2160 * 4
-    assert lt.lsms_workspace_bytes(0, 3, False, 1) == 0
-    assert lt.lsms_workspace_bytes(13, 9, False, 1) == 0
+def test_handle_options_and_workspace_queries():
+    """Host-only part of the handle API: works without a device (a handle binds to a device on first GPU use)."""
+    h = lt.lsms_create()
+    assert h.get("nb_outer") == 0 and h.get("lookahead") == 1 and h.get("small_mode") == 0
+    L = lt.lib()
+    assert L.lsms_set_option(h.ptr, lt.LSMS_OPT_NB_OUTER, 63) == -3 and L.lsms_set_option(h.ptr, lt.LSMS_OPT_IB_INNER, 17) == -3
+    assert L.lsms_set_option(h.ptr, 99, 0) == -2 and L.lsms_set_option(None, 0, 0) == -1
+    assert L.lsms_set_option(h.ptr, lt.LSMS_OPT_PANEL_CLUSTER, 3) == -3 and L.lsms_set_option(h.ptr, lt.LSMS_OPT_GROUPS, 9) == -3
+    w64 = lt.lsms_workspace_bytes(h, 135, 3, False, 128)
+    assert w64 >= 128 * 2160 * 4
+    h.set("nb_outer", 32)
+    assert lt.lsms_workspace_bytes(h, 135, 3, False, 128) < w64          # the workspace depends on the handle's NB, explicitly
+    h.set("nb_outer", 0)
+    assert lt.lsms_workspace_bytes(h, 0, 3, False, 1) == 0
+    assert lt.lsms_workspace_bytes(h, 13, 9, False, 1) == 0
     n = 13 * 16
-    assert lt.lsms_solve_workspace_bytes(13, 16, False, 2) >= 2 * n * n * 16
-    assert lt.lsms_host_call_scratch_bytes(13, 3, False, 2, 32) >= 32 * n * n * 16
+    assert lt.lsms_solve_workspace_bytes(h, 13, 16, False, 2) >= 2 * n * n * 16
+    assert lt.lsms_host_call_scratch_bytes(h, 13, 3, False, 2, 32) >= 32 * n * n * 16
+    assert lt.lsms_last_schedule(h) == -1
+    h2 = lt.lsms_create(nb_outer=48)                                     # handles are independent
+    assert h2.get("nb_outer") == 48 and h.get("nb_outer") == 0
+    h.destroy(); h2.destroy()
 
 
 def test_invalid_arguments_are_rejected_without_gpu_work():
     L = lt.lib()
+    h = lt.lsms_create()
+    H = h.ptr
     buf = (ctypes.c_double * 64)()
     p = ctypes.addressof(buf)
     p16 = (p + 15) // 16 * 16
-    assert L.lsms_tau00_batched(0, 13, 16, 0, 1, p16, p16, p16, 1 << 20, 0) == -1
-    assert L.lsms_tau00_batched(p16 + 8, 13, 16, 0, 1, p16, p16, p16, 1 << 20, 0) == -1      # misaligned
-    assert L.lsms_tau00_batched(p16, 0, 16, 0, 1, p16, p16, p16, 1 << 20, 0) == -2
-    assert L.lsms_tau00_batched(p16, 13, 15, 0, 1, p16, p16, p16, 1 << 20, 0) == -3          # not a perfect square
-    assert L.lsms_tau00_batched(p16, 13, 16, 0, 0, p16, p16, p16, 1 << 20, 0) == -5
-    assert L.lsms_tau00_batched(p16, 13, 16, 0, 1, 0, p16, p16, 1 << 20, 0) == -6
-    assert L.lsms_tau00_batched(p16, 13, 16, 0, 1, p16, 0, p16, 1 << 20, 0) == -7
-    assert L.lsms_tau00_batched(p16, 13, 16, 0, 1, p16, p16, 0, 1 << 20, 0) == -8
-    assert L.lsms_tau00_batched(p16, 13, 16, 0, 1, p16, p16, p16, 16, 0) == -9               # workspace too small
-    assert L.lsms_build_M_batched(0, p16, 0, p16, 3, 13, 0, 1, p16, p16, 1 << 20, 0) == -1
-    assert L.lsms_build_M_batched(p16, p16, 0, p16, 3, 13, 1, 1, p16, p16, 1 << 20, 0) == -3  # canted needs moments
-    assert L.lsms_build_M_batched(p16, p16, 0, p16, 9, 13, 0, 1, p16, p16, 1 << 20, 0) == -5
-    assert L.lsms_build_M_batched(p16, p16, 0, p16, 3, 13, 0, 1, p16, p16, 16, 0) == -11
-    assert L.lsms_set_blocking(63, 0) == -1 and L.lsms_set_blocking(64, 17) == -2 and L.lsms_set_blocking(0, 0) == 0
-    assert L.lsms_schur_update_batched(p16, 100, 90, 10, 1, 0) == -3
+    assert L.lsms_tau00_batched(None, p16, 13, 16, 0, 1, p16, p16, p16, 1 << 20, 0) == -1
+    assert L.lsms_tau00_batched(H, 0, 13, 16, 0, 1, p16, p16, p16, 1 << 20, 0) == -2
+    assert L.lsms_tau00_batched(H, p16 + 8, 13, 16, 0, 1, p16, p16, p16, 1 << 20, 0) == -2      # misaligned
+    assert L.lsms_tau00_batched(H, p16, 0, 16, 0, 1, p16, p16, p16, 1 << 20, 0) == -3
+    assert L.lsms_tau00_batched(H, p16, 13, 15, 0, 1, p16, p16, p16, 1 << 20, 0) == -4          # not a perfect square
+    assert L.lsms_tau00_batched(H, p16, 13, 16, 0, 0, p16, p16, p16, 1 << 20, 0) == -6
+    assert L.lsms_tau00_batched(H, p16, 13, 16, 0, 1, 0, p16, p16, 1 << 20, 0) == -7
+    assert L.lsms_tau00_batched(H, p16, 13, 16, 0, 1, p16, 0, p16, 1 << 20, 0) == -8
+    assert L.lsms_tau00_batched(H, p16, 13, 16, 0, 1, p16, p16, 0, 1 << 20, 0) == -9
+    assert L.lsms_tau00_batched(H, p16, 13, 16, 0, 1, p16, p16, p16, 16, 0) == -10              # workspace too small
+    assert L.lsms_build_M_batched(None, p16, p16, 0, p16, 3, 13, 0, 1, p16, p16, p16, 1 << 20, 0) == -1
+    assert L.lsms_build_M_batched(H, 0, p16, 0, p16, 3, 13, 0, 1, p16, p16, p16, 1 << 20, 0) == -2
+    assert L.lsms_build_M_batched(H, p16, p16, 0, p16, 3, 13, 1, 1, p16, p16, p16, 1 << 20, 0) == -4  # canted needs moments
+    assert L.lsms_build_M_batched(H, p16, p16, 0, p16, 9, 13, 0, 1, p16, p16, p16, 1 << 20, 0) == -6
+    assert L.lsms_build_M_batched(H, p16, p16, 0, p16, 3, 13, 0, 1, p16, 0, p16, 1 << 20, 0) == -11   # info
+    assert L.lsms_build_M_batched(H, p16, p16, 0, p16, 3, 13, 0, 1, p16, p16, p16, 16, 0) == -13
+    assert L.lsms_tinv_from_phase_shifts(H, p16, p16, p16, 3, 13, 0, 2, 1, p16, p16, 0, 0) == -12
+    assert L.lsms_tau00_from_host(H, p16, p16, p16, p16, 0, 3, 13, 0, 2, 4, 5, p16, p16, p16, 1 << 20, 0, None, None) == -12
+    assert L.lsms_contour_sum_batched(H, p16, p16, 1, 0, 4, p16, 0) == -5
+    assert L.lsms_schur_update_batched(H, p16, 100, 90, 10, 1, 0) == -4
+    assert L.lsms_destroy(None) == -1 and L.lsms_create(None) == -1
+    h.destroy()
 
 
 def test_closed_form_gaunt_matches_oracle_quadrature():

@@ -27,16 +27,38 @@ def lt():
     return m
 
 
+@pytest.fixture()
+def h(lt):
+    """A fresh handle with default options for every test (the library has no process-wide state)."""
+    hd = lt.lsms_create()
+    yield hd
+    torch.cuda.synchronize()
+    hd.destroy()
+
+
 def relF(a, b):
     return np.linalg.norm(a - b) / np.linalg.norm(b)
 
 
-def gpu_M(lt, batch):
+def max_abs_rel(a, b):
+    """largest element-wise deviation relative to the largest reference element"""
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def check_tau(tau, ref, tol=TAU_TOL, what=""):
+    """north_star bar (relative Frobenius error) AND an element-wise bar, so that an error confined to a few
+    elements cannot hide in the norm: max|diff| <= tol * max|ref|."""
+    assert relF(tau, ref) < tol, (what, "rel. Frobenius", relF(tau, ref))
+    assert max_abs_rel(tau, ref) < tol, (what, "max abs / max", max_abs_rel(tau, ref))
+
+
+def gpu_M(lt, h, batch):
     cfg = batch.cfg
     delta, species, z, pos, mom = lt.device_inputs(batch)
-    tinv, kappa = lt.lsms_tinv_from_phase_shifts(delta, species, z, cfg.lmax, cfg.n_sites, cfg.spin_canted, 2, batch.batch)
-    M = lt.lsms_build_M_batched(tinv, pos, mom if cfg.spin_canted else None, kappa, cfg.lmax, cfg.n_sites,
-                                cfg.spin_canted, batch.batch)
+    tinv, kappa, info0 = lt.lsms_tinv_from_phase_shifts(h, delta, species, z, cfg.lmax, cfg.n_sites, cfg.spin_canted, 2, batch.batch)
+    M, info1 = lt.lsms_build_M_batched(h, tinv, pos, mom if cfg.spin_canted else None, kappa, cfg.lmax, cfg.n_sites,
+                                       cfg.spin_canted, batch.batch)
+    assert not info0.cpu().numpy().any() and not info1.cpu().numpy().any()
     return M, tinv, kappa
 
 
@@ -65,11 +87,11 @@ def residual(M, X, k):
 
 # ------------------------------------------------------------------ K1: t^{-1} and assembly
 
-def test_tinv_and_kappa_parity(lt):
+def test_tinv_and_kappa_parity(lt, h):
     batch = sl.make_batch("C", n_atoms=1, n_energies=32)
-    _, tinv, kappa = gpu_M(lt, batch.select([0]))     # shapes only
+    _, tinv, kappa = gpu_M(lt, h, batch.select([0]))     # shapes only
     delta, species, z, pos, mom = lt.device_inputs(batch)
-    tinv, kappa = lt.lsms_tinv_from_phase_shifts(delta, species, z, 3, 135, True, 2, 32)
+    tinv, kappa, _ = lt.lsms_tinv_from_phase_shifts(h, delta, species, z, 3, 135, True, 2, 32)
     tinv, kappa = tinv.cpu().numpy(), kappa.cpu().numpy()
     assert np.max(np.abs(kappa - np.sqrt(batch.z))) < 1e-15 and np.all(kappa.imag >= 0)
     for b in (0, 17, 31):
@@ -81,18 +103,18 @@ def test_tinv_and_kappa_parity(lt):
 
 
 @pytest.mark.parametrize("key,items", [("T", list(range(32))), ("M", [0, 31, 200, 511])])
-def test_assembly_parity_noncanted(lt, key, items):
+def test_assembly_parity_noncanted(lt, h, key, items):
     batch = sl.make_batch(key).select(items)
-    M, _, _ = gpu_M(lt, batch)
+    M, _, _ = gpu_M(lt, h, batch)
     Mg = M.cpu().numpy().transpose(0, 2, 1)
     for i in range(len(items)):
         assert block_rel_err(Mg[i], oracle_M(batch, i), batch.cfg.k) < ASM_TOL
 
 
-def test_assembly_parity_canted_and_high_l(lt):
+def test_assembly_parity_canted_and_high_l(lt, h):
     for key, items in (("C", [0, 63]), ("H", [0, 23])):
         batch = sl.make_batch(key).select(items)
-        M, _, _ = gpu_M(lt, batch)
+        M, _, _ = gpu_M(lt, h, batch)
         for i in range(len(items)):
             Mg = M[i].cpu().numpy().T
             assert block_rel_err(Mg, oracle_M(batch, i), batch.cfg.k) < ASM_TOL
@@ -100,17 +122,17 @@ def test_assembly_parity_canted_and_high_l(lt):
         torch.cuda.empty_cache()
 
 
-def test_assembly_small_lmax_range(lt):
+def test_assembly_small_lmax_range(lt, h):
     for lmax, canted in ((0, False), (1, True), (2, False), (5, False)):
         cfg = sl.custom_config(13, lmax, canted, n_energies=3)
         batch = sl.make_batch(cfg)
-        M, _, _ = gpu_M(lt, batch)
+        M, _, _ = gpu_M(lt, h, batch)
         Mg = M.cpu().numpy().transpose(0, 2, 1)
         for i in range(3):
             assert block_rel_err(Mg[i], oracle_M(batch, i), cfg.k) < ASM_TOL
 
 
-def test_shared_g0_assembly_is_identical_to_per_item_assembly(lt):
+def test_shared_g0_assembly_is_identical_to_per_item_assembly(lt, h):
     """one g0 evaluation per energy shared by all central atoms of a lattice.  Same arithmetic per
     element, so the matrices must be bit-identical to the per-item assembly (which is itself checked against the
     oracle above); plain and spin-canted (per-item moments and t^-1 on the site diagonal), and one oracle block check."""
@@ -118,10 +140,10 @@ def test_shared_g0_assembly_is_identical_to_per_item_assembly(lt):
                 sl.custom_config(13, 4, False, n_atoms=2, n_energies=2)):
         batch = sl.make_batch(cfg)
         delta, species, z, pos, mom = lt.device_inputs(batch)
-        tinv, kappa = lt.lsms_tinv_from_phase_shifts(delta, species, z, cfg.lmax, cfg.n_sites, cfg.spin_canted, 2, batch.batch)
+        tinv, kappa, _ = lt.lsms_tinv_from_phase_shifts(h, delta, species, z, cfg.lmax, cfg.n_sites, cfg.spin_canted, 2, batch.batch)
         momd = mom if cfg.spin_canted else None
-        M_item = lt.lsms_build_M_batched(tinv, pos, momd, kappa, cfg.lmax, cfg.n_sites, cfg.spin_canted, batch.batch)
-        M_shared = lt.lsms_build_M_shared_g0_batched(tinv, pos, momd, kappa, cfg.lmax, cfg.n_sites, cfg.spin_canted,
+        M_item, _ = lt.lsms_build_M_batched(h, tinv, pos, momd, kappa, cfg.lmax, cfg.n_sites, cfg.spin_canted, batch.batch)
+        M_shared, _ = lt.lsms_build_M_shared_g0_batched(h, tinv, pos, momd, kappa, cfg.lmax, cfg.n_sites, cfg.spin_canted,
                                                      cfg.n_atoms, cfg.n_energies)
         torch.cuda.synchronize()
         assert torch.equal(torch.view_as_real(M_item), torch.view_as_real(M_shared))
@@ -131,94 +153,113 @@ def test_shared_g0_assembly_is_identical_to_per_item_assembly(lt):
 
 # ------------------------------------------------------------------ whole path, element-wise
 
-def test_tau00_tiny_full_batch(lt):
+def test_tau00_tiny_full_batch(lt, h):
     batch = sl.make_batch("T")
-    tau, info, _ = lt.tau00_from_liz_batch(batch)
+    tau, info, _ = lt.tau00_from_liz_batch(h, batch)
     assert not info.any()
     ref, oinfo = oracle.tau00_batched(batch, "long double")
     assert not oinfo.any()
     for b in range(32):
-        assert relF(tau[b], ref[b]) < TAU_TOL
-    assert max(relF(tau[b], ref[b]) for b in range(32)) < 1e-12     # expected ~1e-14 at cond ~1e3
+        check_tau(tau[b], ref[b], 1e-12, ("T", b))              # expected ~1e-14 at cond ~1e3
 
 
-def test_tau00_mid_sampled(lt):
+def test_tau00_mid_sampled(lt, h):
     items = [0, 24, 31, 100, 255, 256, 480, 511]
     batch = sl.make_batch("M").select(items)
-    tau, info, _ = lt.tau00_from_liz_batch(batch)
+    tau, info, _ = lt.tau00_from_liz_batch(h, batch)
     assert not info.any()
     ref, _ = oracle.tau00_batched(batch, "long double")
     for b in range(len(items)):
-        assert relF(tau[b], ref[b]) < TAU_TOL
+        check_tau(tau[b], ref[b], TAU_TOL, ("M", items[b]))
 
 
-def test_tau00_reduced_high_l_canted(lt):
+def test_tau00_reduced_high_l_canted(lt, h):
     """H-like (lmax=4, canted, near-resonant Au d channel) at 19 sites: n = 950, k = 50 -- ragged in
-    every blocking (n-k = 900 = 14*64 + 4; inner panels of 16 and 4)."""
+    every blocking (n-k = 900 = 14*64 + 4; inner panels of 16 and 4); both schedules of the batch scheduler."""
     cfg = sl.LizConfig("high-l", 4, 19, 4, True, 1, 6, "arc")
     batch = sl.make_batch(cfg)
-    tau, info, _ = lt.tau00_from_liz_batch(batch)
-    assert not info.any()
     ref, _ = oracle.tau00_batched(batch, "long double")
-    for b in range(batch.batch):
-        assert relF(tau[b], ref[b]) < TAU_TOL
+    for small in (1, 2):
+        h.set("small_mode", small)
+        tau, info, _ = lt.tau00_from_liz_batch(h, batch)
+        assert not info.any()
+        assert (lt.lsms_last_schedule(h) > 0) == (small == 2)
+        for b in range(batch.batch):
+            check_tau(tau[b], ref[b], TAU_TOL, ("high-l 19 sites", small, b))
 
 
-def test_tau00_full_size_mid_batch_residual_every_item(lt):
-    """Full M batch (512 items) in the launch configuration bench.py times: info == 0 everywhere, and the
-    residual of the verification export on every item (computed with torch on the device: test-side
-    cuBLAS, not the product path)."""
+def device_residuals(M, X, n, k):
+    """||M X - E||_F / (||M||_F ||X||_F) of every item, on the device with torch (test-side cuBLAS, not the product path);
+    M [b, col, row], X [b, col(k), row(n)] as the library stores them."""
+    Mm, Xm = M.transpose(1, 2), X.transpose(1, 2)
+    res = []
+    for b0 in range(0, M.shape[0], 16):                     # chunks bound the temporaries
+        R = torch.bmm(Mm[b0:b0 + 16], Xm[b0:b0 + 16])
+        R[:, n - k:, :] -= torch.eye(k, dtype=R.dtype, device=R.device)
+        res.append(torch.linalg.matrix_norm(R) / (torch.linalg.matrix_norm(Mm[b0:b0 + 16]) * torch.linalg.matrix_norm(Xm[b0:b0 + 16])))
+    return torch.cat(res)
+
+
+def test_tau00_full_size_mid_batch_residual_every_item(lt, h):
+    """Full M batch (512 items) in the launch configuration bench.py times (default handle: the scheduler picks the
+    small-matrix mode): info == 0 everywhere, the residual of the verification export on every item, tau00 equal
+    to the central block of X, and the lock-step schedule agreeing with the small-matrix one on every item."""
     batch = sl.make_batch("M")
     cfg = batch.cfg
-    M, _, _ = gpu_M(lt, batch)
-    X, info = lt.lsms_solve_central_column_batched(M, cfg.n_sites, cfg.kmax, False, batch.batch)
-    tau, info2 = lt.lsms_tau00_batched(M.clone(), cfg.n_sites, cfg.kmax, False, batch.batch)
-    torch.cuda.synchronize()
-    assert not info.cpu().numpy().any() and not info2.cpu().numpy().any()
     n, k = cfg.n, cfg.k
-    Mm = M.transpose(1, 2)                     # [b, row, col]
-    Xm = X.transpose(1, 2)                     # [b, n, k]
-    R = torch.bmm(Mm, Xm)
-    R[:, n - k:, :] -= torch.eye(k, dtype=R.dtype, device=R.device)
-    res = torch.linalg.matrix_norm(R) / (torch.linalg.matrix_norm(Mm) * torch.linalg.matrix_norm(Xm))
-    assert float(res.max()) < RES_TOL
-    # tau00 is the central block of X
-    assert float((Xm[:, n - k:, :] - tau.transpose(1, 2)).abs().max()) == 0.0
-
-
-@pytest.mark.parametrize("key,items,mode", [("P", [0, 24, 31, 56, 64, 88, 120, 127], "double"),
-                                             ("C", [0, 16, 24, 31, 32, 47, 56, 63], "double")])
-def test_tau00_production_sizes_sampled(lt, key, items, mode):
-    """2160^2 and 4320^2 (the north-star sizes): eight sampled items each (first and last energy of every atom, the
-    worst-conditioned contour point q = 24) against the oracle's textbook route, which runs one item per host
-    thread, plus the residual of the central block column for the same items on the host."""
-    batch = sl.make_batch(key).select(items)
-    cfg = batch.cfg
-    M, _, _ = gpu_M(lt, batch)
-    X, info = lt.lsms_solve_central_column_batched(M, cfg.n_sites, cfg.kmax, cfg.spin_canted, batch.batch)
-    Mh = [M[i].cpu().numpy().T for i in range(len(items))]
-    Xh = [X[i].cpu().numpy().T for i in range(len(items))]
-    tau, info2 = lt.lsms_tau00_batched(M, cfg.n_sites, cfg.kmax, cfg.spin_canted, batch.batch)
+    M, _, _ = gpu_M(lt, h, batch)
+    X, info = lt.lsms_solve_central_column_batched(h, M, cfg.n_sites, cfg.kmax, False, batch.batch)
+    tau, info2 = lt.lsms_tau00_batched(h, M.clone(), cfg.n_sites, cfg.kmax, False, batch.batch)
+    sched = lt.lsms_last_schedule(h)
+    h.set("small_mode", 1)
+    tau_ls, info3 = lt.lsms_tau00_batched(h, M.clone(), cfg.n_sites, cfg.kmax, False, batch.batch)
     torch.cuda.synchronize()
+    assert sched >= 1 and lt.lsms_last_schedule(h) == 0
+    assert not info.cpu().numpy().any() and not info2.cpu().numpy().any() and not info3.cpu().numpy().any()
+    assert float(device_residuals(M, X, n, k).max()) < RES_TOL
+    assert float((X[:, :, n - k:] - tau).abs().max()) == 0.0            # tau00 is the central block of X
+    d = torch.linalg.matrix_norm(tau - tau_ls) / torch.linalg.matrix_norm(tau_ls)
+    assert float(d.max()) < 1e-11                                      # two schedules, same pivots, different summation order
+
+
+@pytest.mark.parametrize("key,items", [("P", [0, 24, 31, 56, 64, 88, 120, 127]), ("C", [0, 16, 24, 31, 32, 47, 56, 63])])
+def test_tau00_production_full_batch(lt, h, key, items):
+    """2160^2 and 4320^2 (the north-star sizes) as bench.py times them: the FULL batch (128 / 64 items) through a
+    default handle -- two batch groups on separate streams with look-ahead --, info == 0 and the residual of the
+    central block column on EVERY item (SURVEY 8(d) protocol, pin P5), and eight items (first and last energy of
+    every atom, the worst-conditioned contour point q = 24) element by element against the oracle's textbook route."""
+    batch = sl.make_batch(key)
+    cfg = batch.cfg
+    n, k, B = cfg.n, cfg.k, batch.batch
+    M, _, _ = gpu_M(lt, h, batch)
+    X, info = lt.lsms_solve_central_column_batched(h, M, cfg.n_sites, cfg.kmax, cfg.spin_canted, B)
+    torch.cuda.synchronize()
+    assert not info.cpu().numpy().any()
+    res = device_residuals(M, X, n, k)
+    assert float(res.max()) < RES_TOL, float(res.max())
+    tau, info2 = lt.lsms_tau00_batched(h, M, cfg.n_sites, cfg.kmax, cfg.spin_canted, B)       # overwrites M
+    torch.cuda.synchronize()
+    assert lt.lsms_last_schedule(h) == 0 and h.get("groups") == 0 and h.get("lookahead") == 1
+    assert not info2.cpu().numpy().any()
+    assert float((X[:, :, n - k:] - tau).abs().max()) == 0.0
     tau = tau.cpu().numpy().transpose(0, 2, 1)
-    assert not info.cpu().numpy().any() and not info2.cpu().numpy().any()
-    for i in range(len(items)):
-        assert residual(Mh[i], Xh[i], cfg.k) < RES_TOL
-    ref, oinfo = oracle.tau00_batched(batch, mode)
+    del M, X
+    torch.cuda.empty_cache()
+    ref, oinfo = oracle.tau00_batched(batch.select(items), "double")
     assert not oinfo.any()
-    for i in range(len(items)):
-        assert relF(tau[i], ref[i]) < TAU_TOL, (key, items[i], relF(tau[i], ref[i]))
+    for i, b in enumerate(items):
+        check_tau(tau[b], ref[i], TAU_TOL, (key, b))
 
 
-def test_tau00_high_l_full_size_properties(lt):
+def test_tau00_high_l_full_size_properties(lt, h):
     """6750^2 (the paper's CoCrFeMnNi rank): the oracle needs ~10 min per item, so parity is
     by properties that hold at any size: M equals the oracle's M (cheap), the residual of the central block
     column is <= 1e-12, and tau00 equals the central block of that column."""
     items = [0, 23]
     batch = sl.make_batch("H").select(items)
     cfg = batch.cfg
-    M, _, _ = gpu_M(lt, batch)
-    X, info = lt.lsms_solve_central_column_batched(M, cfg.n_sites, cfg.kmax, True, batch.batch)
+    M, _, _ = gpu_M(lt, h, batch)
+    X, info = lt.lsms_solve_central_column_batched(h, M, cfg.n_sites, cfg.kmax, True, batch.batch)
     torch.cuda.synchronize()
     assert not info.cpu().numpy().any()
     for i in range(len(items)):
@@ -227,12 +268,7 @@ def test_tau00_high_l_full_size_properties(lt):
         assert residual(Mo, X[i].cpu().numpy().T, cfg.k) < RES_TOL
 
 
-@pytest.mark.parametrize("key,item", [("H", 0), ("H", 23), ("N", 23), ("C", 24)])
-def test_tau00_full_size_against_stored_oracle_values(lt, key, item):
-    """Element-wise parity at full size where the oracle needs minutes per item: tau00 of single items of the
-    largest workloads (H item 0 is the worst-conditioned matrix of all configs, cond_1 ~ 1.6e6) against values the
-    oracle wrote into tests/golden/ (tests/golden/make_golden_full_size.py: oracle.assemble_M + FP64 LU with
-    long-double iterative refinement; nothing there comes from the CUDA path)."""
+def read_golden(key, item):
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"tau00_full_size_{key}_{item}.txt")
     with open(path) as f:
         head = f.readline().split()
@@ -242,30 +278,40 @@ def test_tau00_full_size_against_stored_oracle_values(lt, key, item):
         for line in f:
             r, c, re, im = line.split()
             ref[int(r), int(c)] = complex(float(re), float(im))
+    return n, k, ref
+
+
+@pytest.mark.parametrize("key,item", [("H", 0), ("H", 23), ("N", 23), ("C", 24), ("P", 24), ("NC", 5)])
+def test_tau00_full_size_against_stored_oracle_values(lt, h, key, item):
+    """Element-wise parity at full size where the oracle needs minutes to an hour per item: tau00 of single items of
+    the largest workloads (H item 0 is the worst-conditioned matrix of all configs, cond_1 ~ 1.6e6; NC is the paper's
+    rank-12450 NiAu shape) against values the oracle wrote into tests/golden/ (tests/golden/make_golden_full_size.py:
+    oracle.assemble_M + FP64 LU with long-double iterative refinement; nothing there comes from the CUDA path)."""
+    n, k, ref = read_golden(key, item)
     batch = sl.make_batch(key).select([item])
     assert batch.cfg.n == n and batch.cfg.k == k
-    tau, info, _ = lt.tau00_from_liz_batch(batch)
+    tau, info, _ = lt.tau00_from_liz_batch(h, batch)
     assert not info.any()
-    assert relF(tau[0], ref) < TAU_TOL, relF(tau[0], ref)
+    check_tau(tau[0], ref, TAU_TOL, (key, item))
 
 
 @pytest.mark.parametrize("key,item", [("N", 23), ("NC", 0)])
-def test_tau00_paper_niau_shapes_properties(lt, key, item):
+def test_tau00_paper_niau_shapes_properties(lt, h, key, item):
     """the paper's own NiAu ranks 6225 and 12450 (N_LIZ = 249, l_max = 4).  Same
     property checks as the high-l case: assembled M equals the oracle's M block by block, the central block column
     solves M X = E to <= 1e-12, and tau00 is the central block of X (checked against lsms_tau00_batched itself)."""
     batch = sl.make_batch(key).select([item])
     cfg = batch.cfg
     assert cfg.n == {"N": 6225, "NC": 12450}[key]
-    M, _, _ = gpu_M(lt, batch)
-    X, info = lt.lsms_solve_central_column_batched(M, cfg.n_sites, cfg.kmax, cfg.spin_canted, 1)
+    M, _, _ = gpu_M(lt, h, batch)
+    X, info = lt.lsms_solve_central_column_batched(h, M, cfg.n_sites, cfg.kmax, cfg.spin_canted, 1)
     torch.cuda.synchronize()
     assert not info.cpu().numpy().any()
     Mo = oracle_M(batch, 0)
     assert block_rel_err(M[0].cpu().numpy().T, Mo, cfg.k) < ASM_TOL
     Xh = X[0].cpu().numpy().T
     assert residual(Mo, Xh, cfg.k) < RES_TOL
-    tau, info2 = lt.lsms_tau00_batched(M, cfg.n_sites, cfg.kmax, cfg.spin_canted, 1)      # overwrites M
+    tau, info2 = lt.lsms_tau00_batched(h, M, cfg.n_sites, cfg.kmax, cfg.spin_canted, 1)      # overwrites M
     torch.cuda.synchronize()
     assert not info2.cpu().numpy().any()
     assert relF(tau[0].cpu().numpy().T, Xh[cfg.n - cfg.k:, :]) < 1e-12
@@ -273,168 +319,294 @@ def test_tau00_paper_niau_shapes_properties(lt, key, item):
 
 # ------------------------------------------------------------------ direct input to lsms_tau00_batched
 
+def lapack_tau00(A, k):
+    """A [col, row] as stored -> central block of the inverse by LAPACK"""
+    n = A.shape[0]
+    return np.linalg.inv(A.T)[n - k:, n - k:]
+
+
+@pytest.mark.parametrize("small", [1, 2, 4])
 @pytest.mark.parametrize("n_sites,kmax,canted", [(7, 9, False), (37, 1, False), (1, 16, False), (2, 4, True),
-                                                  (33, 4, False), (5, 25, True), (129, 1, False)])
-def test_random_matrices_vs_lapack(lt, n_sites, kmax, canted):
+                                                  (33, 4, False), (5, 25, True), (129, 1, False), (23, 9, False), (150, 9, False)])
+def test_random_matrices_vs_lapack(lt, h, n_sites, kmax, canted, small):
+    """Dense random matrices (strong pivoting) of ragged shapes through the lock-step schedule (small = 1), the
+    small-matrix mode with one CTA per matrix (2) and with a 4-CTA cluster per matrix (4)."""
     k = kmax * (2 if canted else 1)
     n = n_sites * k
+    h.set("small_mode", small)
     A = sl.random_dense_matrices(5, n, seed=100 + n)
     M = torch.from_numpy(A).cuda()
-    tau, info = lt.lsms_tau00_batched(M, n_sites, kmax, canted, 5)
+    tau, info = lt.lsms_tau00_batched(h, M, n_sites, kmax, canted, 5)
     torch.cuda.synchronize()
+    assert lt.lsms_last_schedule(h) == {1: 0, 2: 1, 4: 4}[small]
     tau = tau.cpu().numpy().transpose(0, 2, 1)
     assert not info.cpu().numpy().any()
     for b in range(5):
-        ref = np.linalg.inv(A[b].T)[n - k:, n - k:]
-        assert relF(tau[b], ref) < 1e-11
+        check_tau(tau[b], lapack_tau00(A[b], k), 1e-10 if n > 1000 else 1e-11, (n, b))
 
 
-def test_needs_pivoting_and_singular_info(lt):
+@pytest.mark.parametrize("small", [1, 2, 3, 5])
+def test_needs_pivoting_and_singular_info(lt, h, small):
     # zero on the leading diagonal: fails without row interchanges
     n_sites, kmax = 6, 4
     n = 24
+    h.set("small_mode", small)
     rng = np.random.default_rng(3)
     A = rng.standard_normal((3, n, n)) + 1j * rng.standard_normal((3, n, n))
     for j in range(n):
         A[0, j, j] = 0.0                       # column-major storage: [b, col, row]
     A[2, 5, :] = 0.0                           # column 5 identically zero -> exact zero pivot at step 6
     M = torch.from_numpy(np.ascontiguousarray(A)).cuda()
-    tau, info = lt.lsms_tau00_batched(M, n_sites, kmax, False, 3)
+    tau, info = lt.lsms_tau00_batched(h, M, n_sites, kmax, False, 3)
     torch.cuda.synchronize()
     info = info.cpu().numpy()
     tau = tau.cpu().numpy().transpose(0, 2, 1)
     assert info[0] == 0 and info[1] == 0
     for b in (0, 1):
-        assert relF(tau[b], np.linalg.inv(A[b].T)[n - 4:, n - 4:]) < 1e-11
+        check_tau(tau[b], lapack_tau00(A[b], 4), 1e-11)
     assert info[2] == 6
+    # singular central block: the failure is found by the final k x k inverse, step n-k+1 .. n
+    A2 = rng.standard_normal((1, n, n)) + 1j * rng.standard_normal((1, n, n))
+    A2[0, n - 1, :] = 0.0
+    _, info = lt.lsms_tau00_batched(h, torch.from_numpy(A2).cuda(), n_sites, kmax, False, 1)
+    torch.cuda.synchronize()
+    assert n - 4 < int(info.cpu().numpy()[0]) <= n
 
 
-def test_blocking_parameters_do_not_change_the_result(lt):
+@pytest.mark.parametrize("small", [1, 2])
+def test_blocking_parameters_do_not_change_the_result(lt, h, small):
     batch = sl.make_batch("T").select([0, 9])
     ref, _ = oracle.tau00_batched(batch, "long double")
-    try:
-        for nb, ib in ((16, 4), (32, 16), (48, 12), (96, 16), (64, 7)):
-            lt.lsms_set_blocking(nb, ib)
-            tau, info, _ = lt.tau00_from_liz_batch(batch)
-            assert not info.any()
-            assert max(relF(tau[b], ref[b]) for b in range(2)) < 1e-12
-    finally:
-        lt.lsms_set_blocking(0, 0)
+    h.set("small_mode", small)
+    for nb, ib in ((16, 4), (32, 16), (48, 12), (96, 16), (64, 7), (0, 0)):
+        h.set("nb_outer", nb).set("ib_inner", ib)
+        tau, info, _ = lt.tau00_from_liz_batch(h, batch)
+        assert not info.any()
+        for b in range(2):
+            check_tau(tau[b], ref[b], 1e-12, (nb, ib, b))
 
 
-def test_lookahead_on_and_off_give_identical_results(lt):
+def test_lookahead_on_and_off_give_identical_results(lt, h):
     """The look-ahead split of the Schur update only re-orders independent tiles: bitwise equal tau00."""
     batch = sl.make_batch("M").select([3, 300])
-    try:
-        lt.lsms_set_lookahead(False)
-        tau0, info0, _ = lt.tau00_from_liz_batch(batch)
-        lt.lsms_set_lookahead(True)
-        tau1, info1, _ = lt.tau00_from_liz_batch(batch)
-    finally:
-        lt.lsms_set_lookahead(True)
+    h.set("small_mode", 1)
+    h.set("lookahead", 0)
+    tau0, info0, _ = lt.tau00_from_liz_batch(h, batch)
+    h.set("lookahead", 1)
+    tau1, info1, _ = lt.tau00_from_liz_batch(h, batch)
     assert not info0.any() and not info1.any()
     assert np.array_equal(tau0, tau1)
 
 
-@pytest.mark.parametrize("variant", [-1, 0, 1])
-def test_panel_kernel_variants_match_oracle(lt, variant):
-    """Every K2 variant (L2-resident columns, register-blocked sub-panels with 256 / 512 threads) against the
-    oracle on a tiny LIZ, a ragged random matrix (w and sub-panel tails) and a mid LIZ (several row chunks)."""
-    try:
-        lt.lsms_set_panel_variant(variant)
-        batch = sl.make_batch("T").select([0, 17, 31])
-        ref, _ = oracle.tau00_batched(batch, "long double")
-        tau, info, _ = lt.tau00_from_liz_batch(batch)
-        assert not info.any()
-        assert max(relF(tau[b], ref[b]) for b in range(3)) < 1e-12
-        for n_sites, kmax in ((23, 9), (41, 4), (150, 9)):
-            n = n_sites * kmax
-            A = sl.random_dense_matrices(2, n, seed=700 + n)             # column-major storage: [b, col, row]
-            tau, info = lt.lsms_tau00_batched(torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
-            torch.cuda.synchronize()
-            assert not info.cpu().numpy().any()
-            tau = tau.cpu().numpy().transpose(0, 2, 1)
-            for b in range(2):
-                assert relF(tau[b], np.linalg.inv(A[b].T)[n - kmax:, n - kmax:]) < 1e-10
-        mid = sl.make_batch("M").select([5, 400])
-        refm, _ = oracle.tau00_batched(mid, "long double")
-        taum, infom, _ = lt.tau00_from_liz_batch(mid)
-        assert not infom.any()
-        assert max(relF(taum[b], refm[b]) for b in range(2)) < 1e-10
-    finally:
-        lt.lsms_set_panel_variant(1)
+@pytest.mark.parametrize("threads", [0, 1])
+def test_panel_kernel_variants_match_oracle(lt, h, threads):
+    """Both K2 footprints (256 / 512 threads) against the oracle on a tiny LIZ, a ragged random matrix (w and
+    sub-panel tails) and a mid LIZ (several row chunks)."""
+    h.set("panel_threads", threads).set("small_mode", 1)
+    batch = sl.make_batch("T").select([0, 17, 31])
+    ref, _ = oracle.tau00_batched(batch, "long double")
+    tau, info, _ = lt.tau00_from_liz_batch(h, batch)
+    assert not info.any()
+    for b in range(3):
+        check_tau(tau[b], ref[b], 1e-12)
+    for n_sites, kmax in ((23, 9), (41, 4), (150, 9)):
+        n = n_sites * kmax
+        A = sl.random_dense_matrices(2, n, seed=700 + n)             # column-major storage: [b, col, row]
+        tau, info = lt.lsms_tau00_batched(h, torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
+        torch.cuda.synchronize()
+        assert not info.cpu().numpy().any()
+        tau = tau.cpu().numpy().transpose(0, 2, 1)
+        for b in range(2):
+            check_tau(tau[b], lapack_tau00(A[b], kmax), 1e-10)
+    mid = sl.make_batch("M").select([5, 400])
+    refm, _ = oracle.tau00_batched(mid, "long double")
+    taum, infom, _ = lt.tau00_from_liz_batch(h, mid)
+    assert not infom.any()
+    for b in range(2):
+        check_tau(taum[b], refm[b], 1e-10)
 
 
 @pytest.mark.parametrize("cl", [2, 4, 8])
-def test_panel_cluster_kernel_matches_one_cta_kernel_and_oracle(lt, cl):
+def test_panel_cluster_kernel_matches_one_cta_kernel_and_oracle(lt, h, cl):
     """K2 with a cluster of cl CTAs per matrix: same pivots and arithmetic as the one-CTA kernel, so tau00 must be
     bit-identical to it; also against the oracle / LAPACK on a tiny LIZ, ragged random matrices (rows not a multiple
     of the cluster's thread count, sub-panel tails) and a singular matrix (info)."""
-    try:
-        batch = sl.make_batch("T").select([0, 31])
-        ref, _ = oracle.tau00_batched(batch, "long double")
-        lt.lsms_set_panel_cluster(1)
-        tau1, info1, _ = lt.tau00_from_liz_batch(batch)
-        lt.lsms_set_panel_cluster(cl)
-        tau, info, _ = lt.tau00_from_liz_batch(batch)
-        assert not info.any() and not info1.any()
-        assert np.array_equal(tau, tau1)
-        assert max(relF(tau[b], ref[b]) for b in range(2)) < 1e-12
-        for n_sites, kmax in ((23, 9), (150, 9), (131, 16)):
-            n = n_sites * kmax
-            A = sl.random_dense_matrices(2, n, seed=900 + n)             # column-major storage: [b, col, row]
-            lt.lsms_set_panel_cluster(1)
-            t1, i1 = lt.lsms_tau00_batched(torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
-            lt.lsms_set_panel_cluster(cl)
-            t2, i2 = lt.lsms_tau00_batched(torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
-            torch.cuda.synchronize()
-            assert not i1.cpu().numpy().any() and not i2.cpu().numpy().any()
-            assert torch.equal(torch.view_as_real(t1), torch.view_as_real(t2))
-            t2 = t2.cpu().numpy().transpose(0, 2, 1)
-            for b in range(2):
-                assert relF(t2[b], np.linalg.inv(A[b].T)[n - kmax:, n - kmax:]) < 1e-10
-        A = sl.random_dense_matrices(1, 24, seed=3)
-        A[0, 5, :] = 0.0                           # column 5 identically zero -> exact zero pivot at step 6
-        _, i3 = lt.lsms_tau00_batched(torch.from_numpy(A).cuda(), 6, 4, False, 1)
+    h.set("small_mode", 1)
+    batch = sl.make_batch("T").select([0, 31])
+    ref, _ = oracle.tau00_batched(batch, "long double")
+    h.set("panel_cluster", 1)
+    tau1, info1, _ = lt.tau00_from_liz_batch(h, batch)
+    h.set("panel_cluster", cl)
+    tau, info, _ = lt.tau00_from_liz_batch(h, batch)
+    assert not info.any() and not info1.any()
+    assert np.array_equal(tau, tau1)
+    for b in range(2):
+        check_tau(tau[b], ref[b], 1e-12)
+    for n_sites, kmax in ((23, 9), (150, 9), (131, 16)):
+        n = n_sites * kmax
+        A = sl.random_dense_matrices(2, n, seed=900 + n)             # column-major storage: [b, col, row]
+        h.set("panel_cluster", 1)
+        t1, i1 = lt.lsms_tau00_batched(h, torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
+        h.set("panel_cluster", cl)
+        t2, i2 = lt.lsms_tau00_batched(h, torch.from_numpy(A).cuda(), n_sites, kmax, False, 2)
         torch.cuda.synchronize()
-        assert int(i3.cpu().numpy()[0]) == 6
-    finally:
-        lt.lsms_set_panel_cluster(0)
+        assert not i1.cpu().numpy().any() and not i2.cpu().numpy().any()
+        assert torch.equal(torch.view_as_real(t1), torch.view_as_real(t2))
+        t2 = t2.cpu().numpy().transpose(0, 2, 1)
+        for b in range(2):
+            check_tau(t2[b], lapack_tau00(A[b], kmax), 1e-10)
+    A = sl.random_dense_matrices(1, 24, seed=3)
+    A[0, 5, :] = 0.0                           # column 5 identically zero -> exact zero pivot at step 6
+    _, i3 = lt.lsms_tau00_batched(h, torch.from_numpy(A).cuda(), 6, 4, False, 1)
+    torch.cuda.synchronize()
+    assert int(i3.cpu().numpy()[0]) == 6
 
 
-def test_batch_groups_give_identical_results(lt):
+def test_batch_groups_give_identical_results(lt, h):
     """Batch groups run the same per-item elimination on separate streams: bitwise equal tau00 for every
     group count, including counts that do not divide the batch and exceed it."""
     batch = sl.make_batch("T").select(list(range(11)))
     ref, _ = oracle.tau00_batched(batch, "long double")
+    h.set("small_mode", 1)
     out = []
-    try:
-        for g in (1, 2, 3, 8):
-            lt.lsms_set_groups(g)
-            tau, info, _ = lt.tau00_from_liz_batch(batch)
-            assert not info.any()
-            out.append(tau)
-        lt.lsms_set_groups(8)
-        small = sl.make_batch("T").select([0, 5, 9])
-        tau_s, info_s, _ = lt.tau00_from_liz_batch(small)
-        assert not info_s.any()
-    finally:
-        lt.lsms_set_groups(0)
+    for g in (1, 2, 3, 8):
+        h.set("groups", g)
+        tau, info, _ = lt.tau00_from_liz_batch(h, batch)
+        assert not info.any()
+        out.append(tau)
+    small = sl.make_batch("T").select([0, 5, 9])
+    tau_s, info_s, _ = lt.tau00_from_liz_batch(h, small)
+    assert not info_s.any()
     for tau in out[1:]:
         assert np.array_equal(out[0], tau)
-    assert max(relF(out[0][b], ref[b]) for b in range(11)) < 1e-10
+    for b in range(11):
+        check_tau(out[0][b], ref[b], TAU_TOL)
     assert np.array_equal(tau_s, out[0][[0, 5, 9]])
 
 
-def test_schur_update_alone_matches_numpy(lt):
+# ------------------------------------------------------------------ the batch scheduler's small-matrix mode (a7)
+
+def test_small_mode_is_chosen_for_the_small_configs_and_matches_the_oracle(lt, h):
+    """SURVEY 8(a) a7 / north_star "packs small LIZ matrices several per SM": with default options the scheduler
+    runs T (208^2 x 32) and M-sized matrices in the one-launch small-matrix mode and P-sized ones in lock-step; every
+    cluster size gives tau00 within the bar of the oracle on all 32 T items, and the launch count is that of one
+    elimination kernel."""
+    batch = sl.make_batch("T")
+    ref, _ = oracle.tau00_batched(batch, "long double")
+    tau, info, _ = lt.tau00_from_liz_batch(h, batch)
+    assert not info.any()
+    assert lt.lsms_last_schedule(h) >= 1 and lt.lsms_last_launch_count(h) == 1
+    for b in range(32):
+        check_tau(tau[b], ref[b], 1e-12, ("T default", b))
+    for sm, cl in ((2, None), (3, 2), (4, 4), (5, 8)):
+        h.set("small_mode", sm)
+        tau, info, _ = lt.tau00_from_liz_batch(h, batch)
+        assert not info.any()
+        if cl:
+            assert lt.lsms_last_schedule(h) == cl
+        for b in range(32):
+            check_tau(tau[b], ref[b], 1e-12, ("T", sm, b))
+    h.set("small_mode", 0)
+    mid = sl.make_batch("M").select(list(range(0, 512, 37)))
+    refm, _ = oracle.tau00_batched(mid, "long double")
+    taum, infom, _ = lt.tau00_from_liz_batch(h, mid)
+    assert not infom.any() and lt.lsms_last_schedule(h) >= 1
+    for b in range(mid.batch):
+        check_tau(taum[b], refm[b], TAU_TOL, ("M", b))
+    big = sl.make_batch("P").select([0])
+    _, infob, _ = lt.tau00_from_liz_batch(h, big)
+    assert not infob.any() and lt.lsms_last_schedule(h) == 0
+
+
+# ------------------------------------------------------------------ boundary: re-entrancy and input validation
+
+def test_two_host_threads_two_handles_two_streams(lt):
+    """SURVEY 8(b) "re-entrant on different streams": two host threads, each with its own handle (different blockings
+    and schedules), its own stream and its own batch, run lsms_tau00_batched concurrently; the results are
+    bit-identical to the same calls made one after the other."""
+    import threading
+    jobs = [dict(items=list(range(0, 16)), opts=dict(nb_outer=32, ib_inner=8, small_mode=1, groups=2)),
+            dict(items=list(range(16, 32)), opts=dict(nb_outer=64, ib_inner=16, small_mode=1, groups=3))]
+    Ms = []
+    h0 = lt.lsms_create()
+    for j in jobs:
+        M, _, _ = gpu_M(lt, h0, sl.make_batch("M").select(j["items"]))
+        Ms.append(M)
+    torch.cuda.synchronize()
+    cfg = sl.CONFIGS["M"]
+
+    def run(j, M, out, stream):
+        hd = lt.lsms_create(**j["opts"])
+        with torch.cuda.stream(stream):
+            for _ in range(3):                                # several calls back to back keep both threads busy
+                tau, info = lt.lsms_tau00_batched(hd, M.clone(), cfg.n_sites, cfg.kmax, False, len(j["items"]), stream=stream)
+        stream.synchronize()
+        out.append((tau.cpu().numpy(), info.cpu().numpy()))
+        hd.destroy()
+
+    serial = [[], []]
+    for i, j in enumerate(jobs):
+        run(j, Ms[i], serial[i], torch.cuda.Stream())
+    conc = [[], []]
+    threads = [threading.Thread(target=run, args=(j, Ms[i], conc[i], torch.cuda.Stream())) for i, j in enumerate(jobs)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    for i in range(2):
+        assert not serial[i][0][1].any() and not conc[i][0][1].any()
+        assert np.array_equal(serial[i][0][0], conc[i][0][0])
+    h0.destroy()
+
+
+def test_illegal_input_values_are_flagged_per_item(lt, h):
+    """Reading A4: Im z < 0 / Im kappa < 0 and non-finite inputs are rejected per item through info[],
+    on the device and without a sync; legal items of the same batch are unaffected."""
+    batch = sl.make_batch("T").select([0, 1, 2, 3, 4])
+    cfg = batch.cfg
+    ref, _ = oracle.tau00_batched(batch, "long double")
+    delta, species, z, pos, mom = lt.device_inputs(batch)
+    z = z.clone(); species = species.clone()
+    z[1] = complex(0.3, -0.1)                                   # wrong half plane
+    z[3] = complex(float("nan"), 0.0)
+    species[4, 7] = 2                                           # only species 0 and 1 exist
+    tinv, kappa, info0 = lt.lsms_tinv_from_phase_shifts(h, delta, species, z, cfg.lmax, cfg.n_sites, False, 2, 5)
+    assert info0.cpu().numpy().tolist() == [0, -4, 0, -4, -2]
+    kappa2 = kappa.clone()
+    kappa2[1] = complex(0.5, -0.2); kappa2[3] = complex(0.5, 0.2); kappa2[4] = complex(float("inf"), 0.0)
+    tinv2 = torch.nan_to_num(tinv, nan=1.0)
+    M, info1 = lt.lsms_build_M_batched(h, tinv2, pos, None, kappa2, cfg.lmax, cfg.n_sites, False, 5)
+    assert info1.cpu().numpy().tolist() == [0, -5, 0, 0, -5]
+    assert bool(torch.isnan(torch.view_as_real(M[1])).all()) and bool(torch.isnan(torch.view_as_real(M[4])).all())
+    assert bool(torch.isfinite(torch.view_as_real(M[0])).all()) and bool(torch.isfinite(torch.view_as_real(M[3])).all())
+    tau, info2 = lt.lsms_tau00_batched(h, M, cfg.n_sites, cfg.kmax, False, 5)
+    info2 = info2.cpu().numpy()
+    assert info2[0] == 0 and info2[2] == 0 and info2[1] > 0 and info2[4] > 0       # NaN matrices fail at their first pivot
+    tau = tau.cpu().numpy().transpose(0, 2, 1)
+    for b in (0, 2):
+        check_tau(tau[b], ref[b], 1e-12)
+    # a non-finite phase shift
+    d2 = delta.clone(); d2[1, 0, 2] = complex(float("inf"), 0.0)
+    _, _, info3 = lt.lsms_tinv_from_phase_shifts(h, d2, lt.device_inputs(batch)[1], lt.device_inputs(batch)[2], cfg.lmax, cfg.n_sites, False, 2, 5)
+    assert (info3.cpu().numpy() == -1).all()                     # every LIZ of this batch contains species 1
+    # the host entry point reports the first code of the three stages
+    hc = lt.HostCall(h, cfg.n_sites, cfg.lmax, False, 2, 5)
+    hc.load(batch)
+    hc.z[1] = complex(0.3, -0.1)
+    _, info_h = hc.run()
+    info_h = info_h.numpy()
+    assert info_h[1] == -4 and not info_h[[0, 2, 3, 4]].any()
+
+
+def test_schur_update_alone_matches_numpy(lt, h):
     """K4 in isolation: C -= A B on ragged shapes (several tiles + tails in M, N and K; K of 1..6 chunks, so both the
-    one-stage and the three-stage ring are exercised)."""
+    one-stage and the two-stage ring are exercised)."""
     if True:
         for n, c0, kk, nb in ((333, 10, 64, 2), (200, 0, 37, 2), (130, 3, 16, 2), (97, 40, 5, 2), (700, 20, 96, 3), (450, 7, 48, 5),
                               (1100, 0, 64, 1)):
             A = sl.random_dense_matrices(nb, n, seed=n)
             M = torch.from_numpy(A).cuda()
-            lt.lsms_schur_update_batched(M, n, c0, kk, nb)
+            lt.lsms_schur_update_batched(h, M, n, c0, kk, nb)
             torch.cuda.synchronize()
             out = M.cpu().numpy().transpose(0, 2, 1)
             for b in range(nb):
@@ -446,24 +618,24 @@ def test_schur_update_alone_matches_numpy(lt):
 
 # ------------------------------------------------------------------ contour reduction
 
-def test_contour_sum_matches_oracle(lt):
+def test_contour_sum_matches_oracle(lt, h):
     """sum_q w_q tau00_{a,q} on the device vs the oracle's loop: the real tau00 of two tiny-LIZ atoms on the full
     32-point contour, plus ragged shapes (k*k not a multiple of the block, one energy, many atoms)."""
     cfg = sl.custom_config(13, 3, False, n_atoms=2, n_energies=32, index=0)
     batch = sl.make_batch(cfg)
-    tau, info, _ = lt.tau00_from_liz_batch(batch)
+    tau, info, _ = lt.tau00_from_liz_batch(h, batch)
     assert not info.any()
     w = sl.contour_weights("semicircle", 32)
     ref = oracle.contour_sum(tau.reshape(2, 32, cfg.k, cfg.k), w)
     tau_d = torch.from_numpy(np.ascontiguousarray(tau)).cuda()
-    out = lt.lsms_contour_sum_batched(tau_d, torch.from_numpy(w).cuda(), 2, 32, cfg.k)
+    out = lt.lsms_contour_sum_batched(h, tau_d, torch.from_numpy(w).cuda(), 2, 32, cfg.k)
     torch.cuda.synchronize()
     assert relF(out.cpu().numpy(), ref) < 1e-14
     rng = np.random.default_rng(11)
     for na, ne, k in ((1, 1, 1), (5, 24, 50), (300, 3, 7), (2, 33, 13)):
         t = rng.standard_normal((na, ne, k, k)) + 1j * rng.standard_normal((na, ne, k, k))
         ww = rng.standard_normal(ne) + 1j * rng.standard_normal(ne)
-        out = lt.lsms_contour_sum_batched(torch.from_numpy(t).cuda(), torch.from_numpy(ww).cuda(), na, ne, k)
+        out = lt.lsms_contour_sum_batched(h, torch.from_numpy(t).cuda(), torch.from_numpy(ww).cuda(), na, ne, k)
         torch.cuda.synchronize()
         ref = oracle.contour_sum(t, ww)
         assert np.max(np.abs(out.cpu().numpy() - ref)) < 1e-13 * np.sqrt(ne) * np.abs(t).max() * np.abs(ww).max()
@@ -471,15 +643,27 @@ def test_contour_sum_matches_oracle(lt):
 
 # ------------------------------------------------------------------ end-to-end host entry point
 
-def test_host_entry_point_matches_device_path(lt):
+def test_host_entry_point_matches_device_path(lt, h):
     batch = sl.make_batch("T")
     cfg = batch.cfg
-    hc = lt.HostCall(cfg.n_sites, cfg.lmax, cfg.spin_canted, 2, batch.batch)
+    hc = lt.HostCall(h, cfg.n_sites, cfg.lmax, cfg.spin_canted, 2, batch.batch)
     hc.load(batch)
     tau_h, info_h = hc.run()
-    tau_d, info_d, _ = lt.tau00_from_liz_batch(batch)
+    launches = lt.lsms_last_launch_count(h)
+    tau_d, info_d, _ = lt.tau00_from_liz_batch(h, batch)
     assert not info_h.numpy().any()
     assert np.array_equal(tau_h.numpy().transpose(0, 2, 1), tau_d)
     assert hc.h2d_bytes == batch.delta.nbytes + batch.species.nbytes + batch.z.nbytes + batch.site_pos.nbytes
     assert hc.d2h_bytes == 32 * 16 * 16 * 16 + 32 * 4
-    assert lt.lsms_last_launch_count() > 10
+    assert 4 <= launches <= 6           # t^-1, two tables, assembly, ONE elimination launch (small-matrix mode)
+    # f3 through the host call: (atoms x energies) on one lattice -> shared-g0 assembly, same bits
+    cfg2 = sl.custom_config(13, 2, True, n_atoms=3, n_energies=4)
+    b2 = sl.make_batch(cfg2)
+    out = []
+    for ne in (0, cfg2.n_energies):
+        hc2 = lt.HostCall(h, cfg2.n_sites, cfg2.lmax, True, 2, b2.batch, n_energies=ne)
+        hc2.load(b2)
+        t, i = hc2.run()
+        assert not i.numpy().any()
+        out.append(t.numpy().copy())
+    assert np.array_equal(out[0], out[1])
