@@ -21,8 +21,8 @@
  * State and threads ("the library owns nothing persistent ... re-entrant on different
  * streams").  There is NO process-wide state.  Everything a call needs beyond its arguments lives in an opaque
  * handle the caller creates and destroys: the scheduler options and the auxiliary streams and events of the batch
- * scheduler (look-ahead and batch-group streams).  A handle is bound to the device that was current in
- * lsms_create; a call made while another device is current returns cudaErrorInvalidDevice (101).  One handle serves
+ * scheduler (look-ahead and batch-group streams).  A handle is bound to the device that is current at its first call
+ * that enqueues work; a later call made while another device is current returns cudaErrorInvalidDevice (101).  One handle serves
  * one host thread at a time; calls on DIFFERENT handles are independent and may run concurrently from different
  * host threads on different streams (the paper's callers are many MPI ranks sharing a GPU).
  *
@@ -54,10 +54,11 @@ typedef struct lsms_context* lsms_handle_t;    /* opaque; see "State and threads
 /* Library version string (static storage). */
 const char* lsms_version(void);
 
-/* Create a handle on the current device: records the device, opts the kernels into their shared-memory sizes on
- * it and creates the scheduler's streams and events (non-blocking streams; one high-priority look-ahead stream
- * per batch group).  lsms_destroy synchronises nothing: destroy a handle only after the work enqueued through it
- * has completed.  Errors: -1 null argument; >0 CUDA error. */
+/* Create a handle with default options (host only: no CUDA call, works without a device).  The first call that
+ * enqueues work through it binds it to the current device: the kernels are opted into their shared-memory sizes
+ * there and the scheduler's streams and events are created (non-blocking streams; one high-priority look-ahead
+ * stream per batch group).  lsms_destroy synchronises nothing: destroy a handle only after the work enqueued
+ * through it has completed.  Errors: -1 null argument; >0 CUDA error (allocation). */
 int lsms_create(lsms_handle_t* handle_out);
 int lsms_destroy(lsms_handle_t handle);
 
@@ -82,7 +83,7 @@ enum {
                                    north_star): the whole elimination of a matrix runs inside ONE launch, one CTA (or one
                                    cluster of CTAs) per matrix, several matrices resident per SM.  0 (default) chosen from
                                    (n, batch); 1 never (lock-step launches over the batch); 2 whenever the shape allows
-                                   (n <= 2048); 3..: 2 + log2 of a forced cluster size (3: 2 CTAs, 4: 4, 5: 8 per matrix)   */
+                                   (n <= 2048), CTAs per matrix chosen from the batch size; 3 / 4 / 5 / 6: forced with 1 / 2 / 4 / 8 CTAs per matrix   */
     LSMS_OPT_COUNT = 8
 };
 int lsms_set_option(lsms_handle_t handle, int option, int value);       /* -1 handle, -2 option, -3 value out of range */

@@ -33,7 +33,9 @@ def build(force: bool = False) -> str:
 def lib():
     global _lib
     if _lib is None:
-        _lib = ctypes.CDLL(build())
+        # LSMS_ORACLE_LIB: load another build of the same source (tests/test_oracle_sanitizers.py loads one compiled with
+        # -fsanitize=address,undefined)
+        _lib = ctypes.CDLL(os.environ.get("LSMS_ORACLE_LIB") or build())
         _lib.orc_tau00_full.restype = ctypes.c_int
         _lib.orc_tau00_schur.restype = ctypes.c_int
         _lib.orc_tau00_refined.restype = ctypes.c_int

@@ -166,6 +166,51 @@ static int schur_update(c128* M, int n, int batch, int J, int W, int c_lo, int c
     return launch_schur_gemm(g, st);
 }
 
+// Look-ahead variant 2: EVERYTHING except the big Schur update runs on the group's high-priority stream (interchanges,
+// triangular solve, the next panel's slice of the update, the panel factorisation); the group's main stream carries only
+// the updates of the remaining columns.  With two batch groups the block scheduler then hands freed SM resources to one
+// group's latency- and bandwidth-bound kernels first while the other group's update CTAs fill the rest.
+static int eliminate_prio(const Ctx* c, c128* M, int n, int k, int batch, const TauWs& ws, int* info, cudaStream_t st, const GroupStreams& gs) {
+    const int ne = n - k;
+    const int NB = eff_nb(c), IB = eff_ib(c);
+    const size_t stride = (size_t)n * n;
+    int* piv = ws.piv;
+    if (ne <= 0) return 0;
+    int W0 = ne < NB ? ne : NB;
+    if (c->opt[LSMS_OPT_ALIGN_FIRST] && NB % 64 == 0 && n % 64 != 0 && n % 64 < W0) W0 = n % 64;
+    cudaStream_t ax = gs.aux;
+    LSMS_CUDA_OK(cudaEventRecord(gs.join, st));
+    LSMS_CUDA_OK(cudaStreamWaitEvent(ax, gs.join, 0));
+    int rc = factor_panel(c, M, n, batch, 0, W0, ne, IB, piv, info, ax);
+    if (!rc) { ProfScope ps(6, ax); rc = launch_panel_post(M, stride, n, 0, W0, batch, piv, ws.perm, ws.ninv, NB, ax); }
+    for (int J = 0, W = W0; J < ne && !rc; J += W, W = (ne - J < NB) ? ne - J : NB) {
+        const int Jend = J + W;
+        { ProfScope ps(6, ax); rc = launch_row_permute(M, stride, n, J, W, Jend, n, batch, ws.perm, ws.tperm, (size_t)NB * n, NB, ax); } if (rc) break;
+        GemmShape t; t.batch = batch; t.beta0 = 1;
+        t.A = ws.ninv; t.strideA = (size_t)NB * NB; t.ldA = NB;
+        t.B = ws.tperm + (size_t)Jend * NB; t.strideB = (size_t)NB * n; t.ldB = NB;
+        t.C = M + (size_t)J + (size_t)Jend * n; t.strideC = stride; t.ldC = n;
+        t.Mr = W; t.Nc = n - Jend; t.K = W;
+        { ProfScope ps(7, ax, 8.0 * t.Mr * t.Nc * t.K * batch); rc = launch_schur_gemm(t, ax); } if (rc) break;
+        const int W2 = (Jend < ne) ? ((ne - Jend < NB) ? ne - Jend : NB) : 0;
+        if (W2 > 0) { rc = schur_update(M, n, batch, J, W, Jend, Jend + W2, ax); if (rc) break; }
+        if (cudaEventRecord(gs.fork, ax) != cudaSuccess || cudaStreamWaitEvent(st, gs.fork, 0) != cudaSuccess) { rc = (int)cudaGetLastError(); break; }
+        rc = schur_update(M, n, batch, J, W, Jend + W2, n, st); if (rc) break;
+        if (cudaEventRecord(gs.join, st) != cudaSuccess) { rc = (int)cudaGetLastError(); break; }
+        if (W2 > 0) {
+            rc = factor_panel(c, M, n, batch, Jend, W2, ne, IB, piv, info, ax); if (rc) break;
+            { ProfScope ps(6, ax); rc = launch_panel_post(M, stride, n, Jend, W2, batch, piv, ws.perm, ws.ninv, NB, ax); } if (rc) break;
+        }
+        if (cudaStreamWaitEvent(ax, gs.join, 0) != cudaSuccess) { rc = (int)cudaGetLastError(); break; }
+    }
+    // the auxiliary stream is joined back even when a launch failed
+    cudaError_t e1 = cudaEventRecord(gs.fork, ax);
+    cudaError_t e2 = cudaStreamWaitEvent(st, gs.fork, 0);
+    if (rc) return rc;
+    LSMS_CUDA_OK(e1); LSMS_CUDA_OK(e2);
+    return 0;
+}
+
 // one batch group [0, batch) of items (pointers already offset to the group's first item)
 static int eliminate(const Ctx* c, c128* M, int n, int k, int batch, const TauWs& ws, int* info, cudaStream_t st, const GroupStreams& gs) {
     const int ne = n - k;
@@ -249,7 +294,7 @@ static int eliminate_groups(Ctx* c, c128* M, int n, int k, int batch, const TauW
         w.ninv = ws.ninv + (size_t)b0 * NB * NB;
         w.tperm = ws.tperm + (size_t)b0 * NB * n;
         w.k5 = (char*)ws.k5 + (final_inverse_ws_bytes(k, 1) ? (size_t)b0 * k * k * sizeof(c128) : 0);
-        rc = eliminate(c, M + (size_t)b0 * stride, n, k, b1 - b0, w, info + b0, gst, c->gs[g]);
+        rc = (c->opt[LSMS_OPT_LOOKAHEAD] == 2 ? eliminate_prio : eliminate)(c, M + (size_t)b0 * stride, n, k, b1 - b0, w, info + b0, gst, c->gs[g]);
         if (!rc) {
             ProfScope ps(5, gst);
             rc = launch_final_inverse(M + (size_t)b0 * stride, stride, n, k, b1 - b0, tau + (size_t)b0 * k * k, info + b0, w.k5, gst);
@@ -271,15 +316,18 @@ static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
     const int sm = c->opt[LSMS_OPT_SMALL_MODE];
     if (sm == 1) return 0;
     if (!fused_supported(n, k, eff_nb(c), eff_ib(c))) return 0;
-    if (sm >= 3) return 1 << (sm - 2);
-    // one CTA per matrix keeps a quarter of an SM busy: it needs about four matrices per SM to fill the chip, and
-    // the per-matrix latency (n sequential pivot steps) must not exceed what the lock-step path needs for the batch
+    if (sm >= 3) return 1 << (sm - 3);
+    // CTAs per matrix: a CTA is a quarter of an SM, so few matrices get a cluster each until the chip is covered
     const long long slots = 4LL * c->sms;
     int cl = 1;
-    while (cl < 8 && (long long)batch * cl * 2 <= slots) cl *= 2;     // few matrices: several CTAs per matrix
+    while (cl < 8 && (long long)batch * cl * 2 <= slots) cl *= 2;
     if (sm == 2) return cl;
-    if (n > 1024) return 0;
-    return cl;
+    // Default (measured): the one-launch mode wins where the lock-step schedule is launch- and
+    // latency-bound -- TINY matrices, whose 16-column panels are factored on chip (n <= 212: configs[0], 0.85 -> 0.65 ms).
+    // For mid-size matrices (configs[1], 880^2 x 512) the general one-launch kernel is correct but slower than lock-step
+    // (55 vs 39 ms: its per-matrix latency phases run with 128 threads and do not overlap the other matrices' updates
+    // as hoped), so it is used only on request.
+    return fused_is_tiny(n) ? cl : 0;
 }
 
 static int tau00_impl(Ctx* c, c128* M, int n, int k, int batch, c128* tau, int* info, void* workspace, cudaStream_t st) {
@@ -348,10 +396,11 @@ int lsms_set_option(lsms_handle_t c, int option, int value) {
     switch (option) {
         case LSMS_OPT_NB_OUTER: ok = value >= 0 && value <= 96 && value % 4 == 0; break;
         case LSMS_OPT_IB_INNER: ok = value >= 0 && value <= 16; break;
-        case LSMS_OPT_LOOKAHEAD: case LSMS_OPT_PANEL_THREADS: case LSMS_OPT_ALIGN_FIRST: ok = value == 0 || value == 1; break;
+        case LSMS_OPT_LOOKAHEAD: ok = value >= 0 && value <= 2; break;
+        case LSMS_OPT_PANEL_THREADS: case LSMS_OPT_ALIGN_FIRST: ok = value == 0 || value == 1; break;
         case LSMS_OPT_GROUPS: ok = value >= 0 && value <= MAX_GROUPS; break;
         case LSMS_OPT_PANEL_CLUSTER: ok = value == 0 || value == 1 || value == 2 || value == 4 || value == 8; break;
-        case LSMS_OPT_SMALL_MODE: ok = value >= 0 && value <= 5; break;
+        case LSMS_OPT_SMALL_MODE: ok = value >= 0 && value <= 6; break;
         default: return -2;
     }
     if (!ok) return -3;

@@ -86,6 +86,7 @@ size_t final_inverse_ws_bytes(int k, int batch);
 
 // fused.cu -- small-matrix mode: the whole elimination of a matrix in one launch, cl CTAs per matrix
 bool fused_supported(int n, int k, int NB, int IB);
+bool fused_is_tiny(int n);
 int launch_lu_fused(c128* base, size_t stride, int n, int k, int batch, int NB, int IB, int align_first, int cl,
                     int* piv, c128* tau, int* info, cudaStream_t st);
 

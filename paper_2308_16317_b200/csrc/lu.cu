@@ -4,6 +4,7 @@
 // matrix is needed" PAPER.md:62.  (K2, the panel factorisation itself, is in panel.cu / panel_cluster.cu.)
 #include "common.cuh"
 #include "internal.h"
+#include "lu_body.cuh"
 
 namespace lsms {
 
@@ -35,38 +36,8 @@ k_panel_post(const c128* __restrict__ base, size_t stride, int n, int J, int W, 
     const int tid = threadIdx.x;
 
     if (tid < 32) {
-        // ---- net permutation (warp 0; the below-list is searched lane-parallel)
-        const int lane = tid;
-        for (int i = lane; i < W; i += 32) cur_top[i] = J + i;
-        __syncwarp();
-        int nb = 0;
-        for (int i = 0; i < W; ++i) {
-            const int p = pv[i];
-            if (p == J + i) continue;
-            if (p < J + W) {
-                if (lane == 0) { int t = cur_top[i]; cur_top[i] = cur_top[p - J]; cur_top[p - J] = t; }
-            } else {
-                int found = -1;
-                for (int b0 = 0; b0 < nb; b0 += 32) {
-                    const int idx = b0 + lane;
-                    const unsigned m = __ballot_sync(0xffffffffu, idx < nb && bpos[idx] == p);
-                    if (m) { found = b0 + __ffs(m) - 1; break; }
-                }
-                if (found < 0) { found = nb; if (lane == 0) { bpos[nb] = p; bcon[nb] = p; } ++nb; }
-                __syncwarp();
-                if (lane == 0) { int t = cur_top[i]; cur_top[i] = bcon[found]; bcon[found] = t; }
-            }
-            __syncwarp();
-        }
-        __syncwarp();
-        // compact the displaced rows (content differs from position); serial over <= W entries
-        if (lane == 0) {
-            int nd = 0;
-            for (int j = 0; j < nb; ++j)
-                if (bcon[j] != bpos[j]) { perm[1 + nbmax + nd] = bpos[j]; perm[1 + 2 * nbmax + nd] = bcon[j] - J; ++nd; }
-            perm[0] = nd;
-        }
-        for (int i = lane; i < W; i += 32) perm[1 + i] = cur_top[i];
+        // ---- net permutation (warp 0)
+        net_permutation(pv, J, W, cur_top, bpos, bcon, perm, perm + 1, perm + 1 + nbmax, perm + 1 + 2 * nbmax);
     } else {
         // ---- L11 -> shared memory (strictly lower part; unit diagonal; identity padding up to Wp)
         for (int e = tid - 32; e < Wp * Wp; e += POST_THREADS - 32) {
@@ -177,76 +148,9 @@ __global__ void __launch_bounds__(K5_THREADS)
 k_final_inverse(const c128* __restrict__ base, size_t stride, int n, int k, c128* __restrict__ tau, int* __restrict__ info,
                 c128* __restrict__ gscratch, int use_smem) {
     extern __shared__ __align__(16) unsigned char k5_smem[];
-    const c128* A = base + (size_t)blockIdx.x * stride;
-    const int ne = n - k;
+    __shared__ K5Shared sh;
     c128* S = use_smem ? reinterpret_cast<c128*>(k5_smem) : gscratch + (size_t)blockIdx.x * k * k;
-    __shared__ int cpiv[256];
-    __shared__ int s_p;
-    __shared__ c128 s_rp;
-    __shared__ double wv[K5_THREADS / 32];
-    __shared__ int wi[K5_THREADS / 32];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int e = tid; e < k * k; e += K5_THREADS) { int r = e % k, c = e / k; S[e] = A[(ne + r) + (size_t)(ne + c) * n]; }
-    __syncthreads();
-    bool failed = false;
-    for (int j = 0; j < k; ++j) {
-        double bv = -1.0; int bi = 0x7fffffff;
-        for (int i = j + tid; i < k; i += K5_THREADS) { double v = cabs1(S[i + (size_t)j * k]); if (v > bv) { bv = v; bi = i; } }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            double ov = __shfl_xor_sync(0xffffffffu, bv, o); int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-        }
-        if (lane == 0) { wv[warp] = bv; wi[warp] = bi; }
-        __syncthreads();
-        if (tid == 0) {
-            for (int t = 1; t < K5_THREADS / 32; ++t) if (wv[t] > bv || (wv[t] == bv && wi[t] < bi)) { bv = wv[t]; bi = wi[t]; }
-            const bool bad = !(bv > 0.0) || !(bv < 1.0e300 * 1.0e300);
-            s_p = bad ? -1 : bi;
-            if (bad) atomicCAS(&info[blockIdx.x], 0, ne + j + 1);
-            else { cpiv[j] = bi; s_rp = crecip(S[bi + (size_t)j * k]); }
-        }
-        __syncthreads();
-        const int p = s_p;
-        if (p < 0) { failed = true; break; }
-        // swap rows j <-> p
-        if (p != j) for (int c = tid; c < k; c += K5_THREADS) { c128 t = S[j + (size_t)c * k]; S[j + (size_t)c * k] = S[p + (size_t)c * k]; S[p + (size_t)c * k] = t; }
-        __syncthreads();
-        // row j <- row j / pivot, with a_jj := 1 first
-        const c128 rp = s_rp;
-        for (int c = tid; c < k; c += K5_THREADS) {
-            c128 v = (c == j) ? cmake(1.0, 0.0) : S[j + (size_t)c * k];
-            S[j + (size_t)c * k] = cmul(v, rp);
-        }
-        __syncthreads();
-        // eliminate column j from every other row: f = a_ij, a_ij := 0, row_i -= f * row_j
-        for (int e = tid; e < k * k; e += K5_THREADS) {
-            int i = e % k, c = e / k;
-            if (i == j) continue;
-            c128 f = S[i + (size_t)j * k];
-            if (c == j) continue;                  // column j itself is handled after the sweep
-            c128 v = S[i + (size_t)c * k];
-            cfms(v, f, S[j + (size_t)c * k]);
-            S[i + (size_t)c * k] = v;
-        }
-        __syncthreads();
-        for (int i = tid; i < k; i += K5_THREADS) {
-            if (i == j) continue;
-            c128 f = S[i + (size_t)j * k];
-            S[i + (size_t)j * k] = cneg(cmul(f, S[j + (size_t)j * k]));
-        }
-        __syncthreads();
-    }
-    if (!failed) {
-        // undo the row interchanges as column interchanges, in reverse order
-        for (int j = k - 1; j >= 0; --j) {
-            const int p = cpiv[j];
-            if (p != j) for (int r = tid; r < k; r += K5_THREADS) { c128 t = S[r + (size_t)j * k]; S[r + (size_t)j * k] = S[r + (size_t)p * k]; S[r + (size_t)p * k] = t; }
-            __syncthreads();
-        }
-    }
-    c128* out = tau + (size_t)blockIdx.x * k * k;
-    for (int e = tid; e < k * k; e += K5_THREADS) out[e] = S[e];
+    final_inverse_body<K5_THREADS>(base + (size_t)blockIdx.x * stride, n, k, tau + (size_t)blockIdx.x * k * k, info + blockIdx.x, S, sh);
 }
 
 size_t final_inverse_ws_bytes(int k, int batch) { return k > 96 ? (size_t)batch * k * k * sizeof(c128) : 0; }

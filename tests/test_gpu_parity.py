@@ -201,9 +201,10 @@ def device_residuals(M, X, n, k):
 
 
 def test_tau00_full_size_mid_batch_residual_every_item(lt, h):
-    """Full M batch (512 items) in the launch configuration bench.py times (default handle: the scheduler picks the
-    small-matrix mode): info == 0 everywhere, the residual of the verification export on every item, tau00 equal
-    to the central block of X, and the lock-step schedule agreeing with the small-matrix one on every item."""
+    """Full M batch (512 items) in the launch configuration bench.py times (default handle: lock-step, two batch groups,
+    look-ahead): info == 0 everywhere, the residual of the verification export on every item, tau00 equal to the
+    central block of X, and the one-launch small-matrix mode (one CTA per matrix, four matrices per SM) agreeing with
+    the lock-step schedule on every item."""
     batch = sl.make_batch("M")
     cfg = batch.cfg
     n, k = cfg.n, cfg.k
@@ -211,10 +212,10 @@ def test_tau00_full_size_mid_batch_residual_every_item(lt, h):
     X, info = lt.lsms_solve_central_column_batched(h, M, cfg.n_sites, cfg.kmax, False, batch.batch)
     tau, info2 = lt.lsms_tau00_batched(h, M.clone(), cfg.n_sites, cfg.kmax, False, batch.batch)
     sched = lt.lsms_last_schedule(h)
-    h.set("small_mode", 1)
+    h.set("small_mode", 2)
     tau_ls, info3 = lt.lsms_tau00_batched(h, M.clone(), cfg.n_sites, cfg.kmax, False, batch.batch)
     torch.cuda.synchronize()
-    assert sched >= 1 and lt.lsms_last_schedule(h) == 0
+    assert sched == 0 and lt.lsms_last_schedule(h) == 1
     assert not info.cpu().numpy().any() and not info2.cpu().numpy().any() and not info3.cpu().numpy().any()
     assert float(device_residuals(M, X, n, k).max()) < RES_TOL
     assert float((X[:, :, n - k:] - tau).abs().max()) == 0.0            # tau00 is the central block of X
@@ -325,12 +326,12 @@ def lapack_tau00(A, k):
     return np.linalg.inv(A.T)[n - k:, n - k:]
 
 
-@pytest.mark.parametrize("small", [1, 2, 4])
+@pytest.mark.parametrize("small", [1, 2, 3, 5])
 @pytest.mark.parametrize("n_sites,kmax,canted", [(7, 9, False), (37, 1, False), (1, 16, False), (2, 4, True),
                                                   (33, 4, False), (5, 25, True), (129, 1, False), (23, 9, False), (150, 9, False)])
 def test_random_matrices_vs_lapack(lt, h, n_sites, kmax, canted, small):
     """Dense random matrices (strong pivoting) of ragged shapes through the lock-step schedule (small = 1), the
-    small-matrix mode with one CTA per matrix (2) and with a 4-CTA cluster per matrix (4)."""
+    small-matrix mode with the cluster size chosen by the scheduler (2), one CTA per matrix (3) and a 4-CTA cluster (5)."""
     k = kmax * (2 if canted else 1)
     n = n_sites * k
     h.set("small_mode", small)
@@ -338,14 +339,14 @@ def test_random_matrices_vs_lapack(lt, h, n_sites, kmax, canted, small):
     M = torch.from_numpy(A).cuda()
     tau, info = lt.lsms_tau00_batched(h, M, n_sites, kmax, canted, 5)
     torch.cuda.synchronize()
-    assert lt.lsms_last_schedule(h) == {1: 0, 2: 1, 4: 4}[small]
+    assert lt.lsms_last_schedule(h) == {1: 0, 2: 8, 3: 1, 5: 4}[small]
     tau = tau.cpu().numpy().transpose(0, 2, 1)
     assert not info.cpu().numpy().any()
     for b in range(5):
         check_tau(tau[b], lapack_tau00(A[b], k), 1e-10 if n > 1000 else 1e-11, (n, b))
 
 
-@pytest.mark.parametrize("small", [1, 2, 3, 5])
+@pytest.mark.parametrize("small", [1, 2, 3, 4, 6])
 def test_needs_pivoting_and_singular_info(lt, h, small):
     # zero on the leading diagonal: fails without row interchanges
     n_sites, kmax = 6, 4
@@ -373,7 +374,7 @@ def test_needs_pivoting_and_singular_info(lt, h, small):
     assert n - 4 < int(info.cpu().numpy()[0]) <= n
 
 
-@pytest.mark.parametrize("small", [1, 2])
+@pytest.mark.parametrize("small", [1, 3, 5])
 def test_blocking_parameters_do_not_change_the_result(lt, h, small):
     batch = sl.make_batch("T").select([0, 9])
     ref, _ = oracle.tau00_batched(batch, "long double")
@@ -488,9 +489,9 @@ def test_batch_groups_give_identical_results(lt, h):
 
 def test_small_mode_is_chosen_for_the_small_configs_and_matches_the_oracle(lt, h):
     """SURVEY 8(a) a7 / north_star "packs small LIZ matrices several per SM": with default options the scheduler
-    runs T (208^2 x 32) and M-sized matrices in the one-launch small-matrix mode and P-sized ones in lock-step; every
-    cluster size gives tau00 within the bar of the oracle on all 32 T items, and the launch count is that of one
-    elimination kernel."""
+    runs T (208^2 x 32) in the one-launch small-matrix mode and larger matrices in lock-step; every cluster size gives
+    tau00 within the bar of the oracle on all 32 T items, the launch count is that of one elimination kernel, and the
+    general one-launch kernel (on request) matches the oracle on mid-size matrices."""
     batch = sl.make_batch("T")
     ref, _ = oracle.tau00_batched(batch, "long double")
     tau, info, _ = lt.tau00_from_liz_batch(h, batch)
@@ -498,7 +499,7 @@ def test_small_mode_is_chosen_for_the_small_configs_and_matches_the_oracle(lt, h
     assert lt.lsms_last_schedule(h) >= 1 and lt.lsms_last_launch_count(h) == 1
     for b in range(32):
         check_tau(tau[b], ref[b], 1e-12, ("T default", b))
-    for sm, cl in ((2, None), (3, 2), (4, 4), (5, 8)):
+    for sm, cl in ((2, None), (3, 1), (4, 2), (5, 4), (6, 8)):
         h.set("small_mode", sm)
         tau, info, _ = lt.tau00_from_liz_batch(h, batch)
         assert not info.any()
@@ -506,11 +507,12 @@ def test_small_mode_is_chosen_for_the_small_configs_and_matches_the_oracle(lt, h
             assert lt.lsms_last_schedule(h) == cl
         for b in range(32):
             check_tau(tau[b], ref[b], 1e-12, ("T", sm, b))
-    h.set("small_mode", 0)
+    h.set("small_mode", 2)
     mid = sl.make_batch("M").select(list(range(0, 512, 37)))
     refm, _ = oracle.tau00_batched(mid, "long double")
     taum, infom, _ = lt.tau00_from_liz_batch(h, mid)
     assert not infom.any() and lt.lsms_last_schedule(h) >= 1
+    h.set("small_mode", 0)
     for b in range(mid.batch):
         check_tau(taum[b], refm[b], TAU_TOL, ("M", b))
     big = sl.make_batch("P").select([0])
