@@ -317,13 +317,16 @@ static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
     if (sm == 1) return 0;
     if (!fused_supported(n, k, eff_nb(c), eff_ib(c))) return 0;
     if (sm >= 3) return 1 << (sm - 3);
-    // CTAs per matrix: a CTA is a quarter of an SM, so few matrices get a cluster each until the chip is covered
+    // CTAs per matrix: a CTA is a quarter of an SM, so few matrices get a cluster each until the chip is covered.
+    // Tiny matrices: at most 4 -- their panel chain is serial, rank 0 factors under the other ranks' updates, and a
+    // third to seventh helper only adds barrier traffic (208^2 x 32: 0.56 ms with 4 CTAs per matrix, 0.61 with 8).
     const long long slots = 4LL * c->sms;
+    const int cl_max = fused_is_tiny(n) ? 4 : 8;
     int cl = 1;
-    while (cl < 8 && (long long)batch * cl * 2 <= slots) cl *= 2;
+    while (cl < cl_max && (long long)batch * cl * 2 <= slots) cl *= 2;
     if (sm == 2) return cl;
     // Default (measured): the one-launch mode wins where the lock-step schedule is launch- and
-    // latency-bound -- TINY matrices, whose 16-column panels are factored on chip (n <= 212: configs[0], 0.85 -> 0.65 ms).
+    // latency-bound -- TINY matrices, whose 16-column panels are factored on chip (n <= 212: configs[0], 0.85 -> 0.56 ms).
     // For mid-size matrices (configs[1], 880^2 x 512) the general one-launch kernel is correct but slower than lock-step
     // (55 vs 39 ms: its per-matrix latency phases run with 128 threads and do not overlap the other matrices' updates
     // as hoped), so it is used only on request.

@@ -75,13 +75,13 @@ __device__ __forceinline__ void phase_sync(uint32_t ncl) {
 // C[Mr x Nc] -= A[Mr x K] B[K x Nc] of ONE matrix: the tiles are dealt round-robin to the CTAs of the cluster,
 // row-major over the tile grid.  Ends with the CTA synchronised.
 __device__ __forceinline__ void gemm_phase(const c128* A, const c128* B, c128* C, int ld, int Mr, int Nc, int K,
-                                           uint32_t rank, uint32_t ncl, c128* ring, uint64_t* full, uint32_t& cc) {
+                                           int rank, int ncl, c128* ring, uint64_t* full, uint32_t& cc) {
     if (Mr <= 0 || Nc <= 0 || K <= 0) return;
     GemmShape g;
     g.A = A; g.B = B; g.C = C; g.strideA = g.strideB = g.strideC = 0; g.ldA = g.ldB = g.ldC = ld;
     g.Mr = Mr; g.Nc = Nc; g.K = K; g.beta0 = 0; g.batch = 1;
     const int tiles_m = (Mr + BM - 1) / BM, tiles_n = (Nc + F_BN - 1) / F_BN;
-    for (int t = (int)rank; t < tiles_m * tiles_n; t += (int)ncl) {
+    for (int t = rank; t < tiles_m * tiles_n; t += ncl) {
         const int tm = t / tiles_n, tn = t % tiles_n;
         const int m0 = tm * BM, n0 = tn * F_BN;
         gemm_tile<F_STAGES, F_BN>(g, A + m0, B + (size_t)n0 * ld, C + m0 + (size_t)n0 * ld, min(BM, Mr - m0), min(F_BN, Nc - n0),
@@ -198,7 +198,7 @@ k_lu_fused(c128* __restrict__ base, size_t stride, int n, int k, int NB, int IB,
             const int rem = Jend - (c0 + w);
             if (rem > 0) {                                                                                     // P2
                 gemm_phase(A + (size_t)(c0 + w) + (size_t)c0 * n, A + (size_t)c0 + (size_t)(c0 + w) * n,
-                           A + (size_t)(c0 + w) + (size_t)(c0 + w) * n, n, n - (c0 + w), rem, w, rank, ncl, ring, full, cc);
+                           A + (size_t)(c0 + w) + (size_t)(c0 + w) * n, n, n - (c0 + w), rem, w, (int)rank, (int)ncl, ring, full, cc);
                 phase_sync(ncl);
             }
             F_TOC(2);
@@ -263,14 +263,14 @@ k_lu_fused(c128* __restrict__ base, size_t stride, int n, int k, int NB, int IB,
             const int below = Jend - (c0 + w);
             if (below > 0) {
                 gemm_phase(A + (size_t)(c0 + w) + (size_t)c0 * n, A + (size_t)c0 + (size_t)Jend * n,
-                           A + (size_t)(c0 + w) + (size_t)Jend * n, n, below, ntrail, w, rank, ncl, ring, full, cc);
+                           A + (size_t)(c0 + w) + (size_t)Jend * n, n, below, ntrail, w, (int)rank, (int)ncl, ring, full, cc);
                 phase_sync(ncl);
             }
         }
         F_TOC(5);
         // ---------------- P6: Schur update
         gemm_phase(A + (size_t)Jend + (size_t)J * n, A + (size_t)J + (size_t)Jend * n, A + (size_t)Jend + (size_t)Jend * n,
-                   n, ntrail, ntrail, W, rank, ncl, ring, full, cc);
+                   n, ntrail, ntrail, W, (int)rank, (int)ncl, ring, full, cc);
         phase_sync(ncl);
         F_TOC(6);
     }
@@ -288,11 +288,66 @@ k_lu_fused(c128* __restrict__ base, size_t stride, int n, int k, int NB, int IB,
 // phase is trimmed for latency -- at this size nothing but the chain of dependent steps costs time:
 //   T1  panel_smem: panel loaded once, w column steps on chip, stored once                          (rank 0)
 //   T2  net permutation of the w interchanges                                                       (every CTA, warp 0)
-//   T3  trailing columns, one strip per CTA staged in shared memory: interchanges in place, then the w x w unit-lower
-//       solve straight from the staged rows (no second pass over the matrix)
-//   T4  rank-w DMMA update of the trailing matrix, tiles dealt to all CTAs of the cluster
-// Three cluster barriers per panel.
-constexpr int TINY_MAXCOLS = 96;              // trailing columns per CTA and strip: 2 x 96 x 16 staged values + L11 = 52 KB
+//   T3  trailing columns, strips staged in shared memory: interchanges in place, then the w x w unit-lower solve
+//       straight from the staged rows (no second pass over the matrix)
+//   T4  rank-w DMMA update of the trailing matrix
+// LOOK-AHEAD inside the cluster: the panel factorisation is the critical path (16 dependent column steps, ~26 us) and
+// only one CTA can work on it.  So rank 0 takes the NEXT panel's columns through T3 and T4 by itself and factors that
+// panel at once, while ranks 1.. do T3 and T4 on all other trailing columns.  The cluster barrier is split
+// (barrier.cluster.arrive / .wait): rank 0 arrives before it starts the panel and waits after it, so the other ranks
+// never wait for the panel unless they run out of work.  Two cluster barriers per panel.
+constexpr int TINY_MAXCOLS = 96;              // trailing columns per strip: 2 x 96 x 16 staged values + L11 = 52 KB
+
+__device__ __forceinline__ void cluster_arrive() {
+    asm volatile("fence.proxy.async;" ::: "memory");
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+// T3 for the columns [col_lo, col_hi) by this CTA: permutation of the panel's w interchanges (top_src / ddst / dsrc, nd
+// in perm[0]) applied in place and U rows = L11^{-1} (permuted top block).  Ends with the CTA synchronised.
+__device__ __forceinline__ void tiny_t3(c128* __restrict__ A, int n, int c0, int w, int col_lo, int col_hi, c128* ring, const int* perm) {
+    const int tid = threadIdx.x, cend = c0 + w;
+    const int* top_src = perm + 1; const int* ddst = top_src + w; const int* dsrc = ddst + w;
+    c128* Told = ring;                                      // [cols][w]   old top block
+    c128* Tnew = ring + TINY_MAXCOLS * F_MAXIB;             // [cols][w]   permuted top block
+    c128* L11 = ring + 2 * TINY_MAXCOLS * F_MAXIB;          // [16][16]    unit lower triangle of the panel
+    __syncthreads();                                        // T2's result (warp 0) before its use; scratch free
+    for (int c_first = col_lo; c_first < col_hi; c_first += TINY_MAXCOLS) {
+        const int ncol = min(TINY_MAXCOLS, col_hi - c_first);
+        for (int e = tid; e < ncol * w; e += FT) {
+            const int i = e % w, c = e / w;
+            Told[c * w + i] = A[(size_t)(c0 + i) + (size_t)(c_first + c) * n];
+        }
+        for (int e = tid; e < w * w; e += FT) { const int r = e % w, c = e / w; L11[r + F_MAXIB * c] = A[(size_t)(c0 + r) + (size_t)(c0 + c) * n]; }
+        __syncthreads();
+        const int nd = perm[0];
+        for (int e = tid; e < ncol * w; e += FT) {
+            const int i = e % w, c = e / w;
+            const int src = top_src[i];
+            Tnew[c * w + i] = (src < cend) ? Told[c * w + (src - c0)] : A[(size_t)src + (size_t)(c_first + c) * n];
+        }
+        __syncthreads();              // rows below are read (gather) before they are overwritten (scatter)
+        for (int e = tid; e < ncol * nd; e += FT) {
+            const int j = e % nd, c = e / nd;
+            A[(size_t)ddst[j] + (size_t)(c_first + c) * n] = Told[c * w + dsrc[j]];
+        }
+        for (int c = tid; c < ncol; c += FT) {             // U rows of this column: forward substitution from the staged values
+            c128 x[F_MAXIB];
+#pragma unroll
+            for (int i = 0; i < F_MAXIB; ++i) x[i] = (i < w) ? Tnew[c * w + i] : cmake(0.0, 0.0);
+#pragma unroll
+            for (int jq = 0; jq < F_MAXIB; ++jq)
+#pragma unroll
+                for (int i = jq + 1; i < F_MAXIB; ++i)
+                    if (i < w) cfms(x[i], L11[i + F_MAXIB * jq], x[jq]);
+            c128* col = A + (size_t)(c_first + c) * n + c0;
+#pragma unroll
+            for (int i = 0; i < F_MAXIB; ++i) if (i < w) col[i] = x[i];
+        }
+        __syncthreads();
+    }
+}
 
 __global__ void __launch_bounds__(FT, 3)
 k_lu_tiny(c128* __restrict__ base, size_t stride, int n, int k, int IB, int* __restrict__ piv,
@@ -317,65 +372,53 @@ k_lu_tiny(c128* __restrict__ base, size_t stride, int n, int k, int IB, int* __r
     }
     phase_sync(ncl);
     uint32_t cc = 0;
+    bool factored = false;                  // is the current panel already factored (by the previous iteration's look-ahead)?
     F_TIC();
     for (int c0 = 0; c0 < ne; c0 += IB) {
         const int w = min(IB, ne - c0), cend = c0 + w, ntrail = n - cend;
-        if (rank == 0) panel_smem(A, n, c0, w, ne, pv, inf, ring, red_v, red_i);                             // T1
+        if (!factored) {
+            if (rank == 0) panel_smem(A, n, c0, w, ne, pv, inf, ring, red_v, red_i);                         // T1
+            phase_sync(ncl);
+        }
         F_TOC(0);
-        phase_sync(ncl);
-        F_TOC(1);
         int* top_src = perm + 1; int* ddst = top_src + w; int* dsrc = ddst + w;
         if (tid < 32) net_permutation(pv + c0, c0, w, dsrc + w, dsrc + 2 * w, dsrc + 3 * w, perm, top_src, ddst, dsrc);   // T2
-        // T3: this CTA's share of the trailing columns, in strips of at most TINY_MAXCOLS columns
-        {
-            const int per = (ntrail + (int)ncl - 1) / (int)ncl;
-            const int my_lo = cend + (int)rank * per, my_hi = min(n, my_lo + per);
-            c128* Told = ring;                                      // [cols][w]   old top block
-            c128* Tnew = ring + TINY_MAXCOLS * F_MAXIB;             // [cols][w]   permuted top block
-            c128* L11 = ring + 2 * TINY_MAXCOLS * F_MAXIB;          // [16][16]    unit lower triangle of the panel
-            for (int c_first = my_lo; c_first < my_hi; c_first += TINY_MAXCOLS) {
-                const int ncol = min(TINY_MAXCOLS, my_hi - c_first);
-                for (int e = tid; e < ncol * w; e += FT) {
-                    const int i = e % w, c = e / w;
-                    Told[c * w + i] = A[(size_t)(c0 + i) + (size_t)(c_first + c) * n];
-                }
-                for (int e = tid; e < w * w; e += FT) { const int r = e % w, c = e / w; L11[r + F_MAXIB * c] = A[(size_t)(c0 + r) + (size_t)(c0 + c) * n]; }
-                __syncthreads();                                   // also orders T2's result before its use
-                const int nd = perm[0];
-                for (int e = tid; e < ncol * w; e += FT) {
-                    const int i = e % w, c = e / w;
-                    const int src = top_src[i];
-                    Tnew[c * w + i] = (src < cend) ? Told[c * w + (src - c0)] : A[(size_t)src + (size_t)(c_first + c) * n];
-                }
-                __syncthreads();              // rows below are read (gather) before they are overwritten (scatter)
-                for (int e = tid; e < ncol * nd; e += FT) {
-                    const int j = e % nd, c = e / nd;
-                    A[(size_t)ddst[j] + (size_t)(c_first + c) * n] = Told[c * w + dsrc[j]];
-                }
-                for (int c = tid; c < ncol; c += FT) {             // U rows of this column: forward substitution from the staged values
-                    c128 x[F_MAXIB];
-#pragma unroll
-                    for (int i = 0; i < F_MAXIB; ++i) x[i] = (i < w) ? Tnew[c * w + i] : cmake(0.0, 0.0);
-#pragma unroll
-                    for (int jq = 0; jq < F_MAXIB; ++jq)
-#pragma unroll
-                        for (int i = jq + 1; i < F_MAXIB; ++i)
-                            if (i < w) cfms(x[i], L11[i + F_MAXIB * jq], x[jq]);
-                    c128* col = A + (size_t)(c_first + c) * n + c0;
-#pragma unroll
-                    for (int i = 0; i < F_MAXIB; ++i) if (i < w) col[i] = x[i];
-                }
-                __syncthreads();
+        const int w2 = (cend < ne) ? min(IB, ne - cend) : 0;           // width of the next panel
+        const c128* L21 = A + (size_t)cend + (size_t)c0 * n;           // rows below the panel, its columns
+        if (ncl > 1 && w2 > 0) {
+            // ---- look-ahead: rank 0 alone brings the next panel's columns up to date and factors them
+            if (rank == 0) {
+                tiny_t3(A, n, c0, w, cend, cend + w2, ring, perm);
+                phase_sync(1);
+                gemm_phase(L21, A + (size_t)c0 + (size_t)cend * n, A + (size_t)cend + (size_t)cend * n, n, ntrail, w2, w, 0, 1, ring, full, cc);
+                F_TOC(1);
+                cluster_arrive();
+                panel_smem(A, n, cend, w2, ne, pv, inf, ring, red_v, red_i);
+                F_TOC(2);
+                cluster_wait();
+                cluster_arrive(); cluster_wait();
+                F_TOC(3);
+            } else {
+                const int lo = cend + w2, rest = n - lo, nr = (int)ncl - 1, r1 = (int)rank - 1;
+                const int per = (rest + nr - 1) / nr;
+                tiny_t3(A, n, c0, w, min(n, lo + r1 * per), min(n, lo + (r1 + 1) * per), ring, perm);
+                F_TOC(1);
+                cluster_arrive(); cluster_wait();
+                F_TOC(2);
+                gemm_phase(L21, A + (size_t)c0 + (size_t)lo * n, A + (size_t)cend + (size_t)lo * n, n, ntrail, rest, w, r1, nr, ring, full, cc);
+                F_TOC(3);
+                cluster_arrive(); cluster_wait();
+                F_TOC(4);
             }
+            factored = true;
+        } else {
+            const int per = (ntrail + (int)ncl - 1) / (int)ncl;
+            tiny_t3(A, n, c0, w, min(n, cend + (int)rank * per), min(n, cend + ((int)rank + 1) * per), ring, perm);
+            phase_sync(ncl);
+            gemm_phase(L21, A + (size_t)c0 + (size_t)cend * n, A + (size_t)cend + (size_t)cend * n, n, ntrail, ntrail, w, (int)rank, (int)ncl, ring, full, cc);
+            phase_sync(ncl);
+            factored = false;
         }
-        F_TOC(2);
-        phase_sync(ncl);
-        F_TOC(3);
-        gemm_phase(A + (size_t)cend + (size_t)c0 * n, A + (size_t)c0 + (size_t)cend * n, A + (size_t)cend + (size_t)cend * n,
-                   n, ntrail, ntrail, w, rank, ncl, ring, full, cc);                                           // T4
-        F_TOC(4);
-        phase_sync(ncl);
-        F_TOC(5);
     }
     if (rank == 0) {
         K5Shared& ksh = *reinterpret_cast<K5Shared*>(fsm);

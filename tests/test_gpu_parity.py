@@ -339,7 +339,7 @@ def test_random_matrices_vs_lapack(lt, h, n_sites, kmax, canted, small):
     M = torch.from_numpy(A).cuda()
     tau, info = lt.lsms_tau00_batched(h, M, n_sites, kmax, canted, 5)
     torch.cuda.synchronize()
-    assert lt.lsms_last_schedule(h) == {1: 0, 2: 8, 3: 1, 5: 4}[small]
+    assert lt.lsms_last_schedule(h) == {1: 0, 2: 4 if n <= 212 else 8, 3: 1, 5: 4}[small]
     tau = tau.cpu().numpy().transpose(0, 2, 1)
     assert not info.cpu().numpy().any()
     for b in range(5):
