@@ -83,7 +83,10 @@ enum {
                                    north_star): the whole elimination of a matrix runs inside ONE launch, one CTA (or one
                                    cluster of CTAs) per matrix, several matrices resident per SM.  0 (default) chosen from
                                    (n, batch); 1 never (lock-step launches over the batch); 2 whenever the shape allows
-                                   (n <= 2048), CTAs per matrix chosen from the batch size; 3 / 4 / 5 / 6: forced with 1 / 2 / 4 / 8 CTAs per matrix   */
+                                   (n <= 2048), CTAs per matrix chosen from the batch size; 3 / 4 / 5 / 6: forced with
+                                   1 / 2 / 4 / 8 CTAs per matrix, matrix in L2; 7: the on-chip variant (matrix held in the
+                                   distributed shared memory of a cluster; n <= ~216), which is also what 0 picks when the
+                                   matrix fits                                                                             */
     LSMS_OPT_COUNT = 8
 };
 int lsms_set_option(lsms_handle_t handle, int option, int value);       /* -1 handle, -2 option, -3 value out of range */

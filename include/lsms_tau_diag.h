@@ -19,7 +19,8 @@ extern "C" {
 int lsms_last_launch_count(lsms_handle_t handle);
 
 /* Which schedule the last lsms_tau00_batched call through this handle used: 0 lock-step launches over the batch,
- * c >= 1: small-matrix mode with c CTAs per matrix.  -1 before the first call. */
+ * 1 <= c <= 8: small-matrix mode through L2 with c CTAs per matrix; 100 + c: on-chip small-matrix mode, the matrix held
+ * in the distributed shared memory of a cluster of c CTAs.  -1 before the first call. */
 int lsms_last_schedule(lsms_handle_t handle);
 
 /* Per-kernel-class timing.  Between lsms_profile_begin and lsms_profile_end every kernel enqueued through the

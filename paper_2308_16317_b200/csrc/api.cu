@@ -43,7 +43,8 @@ static inline int eff_ib(const Ctx* c) { return c->opt[LSMS_OPT_IB_INNER] > 0 ? 
 static int bind_device(Ctx* c, int dev) {
     LSMS_CUDA_OK(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
     int rc;
-    if ((rc = init_attrs_gemm()) || (rc = init_attrs_lu()) || (rc = init_attrs_assemble()) || (rc = init_attrs_fused())) return rc;
+    if ((rc = init_attrs_gemm()) || (rc = init_attrs_lu()) || (rc = init_attrs_assemble()) || (rc = init_attrs_fused()) ||
+        (rc = init_attrs_resident())) return rc;
     int lo = 0, hi = 0;
     LSMS_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
     LSMS_CUDA_OK(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
@@ -312,9 +313,14 @@ static int eliminate_groups(Ctx* c, c128* M, int n, int k, int batch, const TauW
 // ---- the batch scheduler's first decision (north_star: "packs small LIZ matrices several per SM and lets large
 // ones span the whole chip").  Small-matrix mode eliminates a matrix start to finish inside one launch, `cl` CTAs per
 // matrix; 0 = lock-step launches over the batch.  See fused.cu for the measurements behind the thresholds.
+// Return value: 0 lock-step; cl > 0: one-launch mode through global memory / L2 (fused.cu), cl CTAs per matrix;
+// -cl < 0: on-chip mode (resident.cu), the matrix in the distributed shared memory of a cluster of cl CTAs.
 static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
     const int sm = c->opt[LSMS_OPT_SMALL_MODE];
     if (sm == 1) return 0;
+    const int rcl = resident_cluster_size(n, k);
+    if (sm == 7) return rcl > 0 ? -rcl : 0;
+    if (sm == 0 && rcl > 0) return -rcl;            // default for matrices that fit on chip (n <= ~216 with 4 SMs each)
     if (!fused_supported(n, k, eff_nb(c), eff_ib(c))) return 0;
     if (sm >= 3) return 1 << (sm - 3);
     // CTAs per matrix: a CTA is a quarter of an SM, so few matrices get a cluster each until the chip is covered.
@@ -325,18 +331,21 @@ static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
     int cl = 1;
     while (cl < cl_max && (long long)batch * cl * 2 <= slots) cl *= 2;
     if (sm == 2) return cl;
-    // Default (measured): the one-launch mode wins where the lock-step schedule is launch- and
-    // latency-bound -- TINY matrices, whose 16-column panels are factored on chip (n <= 212: configs[0], 0.85 -> 0.56 ms).
-    // For mid-size matrices (configs[1], 880^2 x 512) the general one-launch kernel is correct but slower than lock-step
-    // (55 vs 39 ms: its per-matrix latency phases run with 128 threads and do not overlap the other matrices' updates
-    // as hoped), so it is used only on request.
+    // Default (measured): the one-launch modes win where the lock-step schedule is launch- and
+    // latency-bound -- matrices of a few hundred rows.  For mid-size matrices (configs[1], 880^2 x 512) the general
+    // one-launch kernel is correct but slower than lock-step (55 vs 39 ms: its per-matrix latency phases run with 128
+    // threads and do not overlap the other matrices' updates as hoped), so it is used only on request.
     return fused_is_tiny(n) ? cl : 0;
 }
 
 static int tau00_impl(Ctx* c, c128* M, int n, int k, int batch, c128* tau, int* info, void* workspace, cudaStream_t st) {
     const TauWs ws = tau_ws_layout(workspace, eff_nb(c), n, k, batch);
     const int cl = pick_small_mode(c, n, k, batch);
-    c->last_schedule = cl;
+    c->last_schedule = cl < 0 ? 100 - cl : cl;
+    if (cl < 0) {
+        ProfScope ps(2, st, 8.0 / 3.0 * (double)n * n * n * batch);
+        return launch_lu_resident(M, (size_t)n * n, n, k, batch, -cl, ws.piv, tau, info, st);
+    }
     if (cl > 0) {
         ProfScope ps(2, st, 8.0 / 3.0 * (double)n * n * n * batch);
         return launch_lu_fused(M, (size_t)n * n, n, k, batch, eff_nb(c), eff_ib(c), c->opt[LSMS_OPT_ALIGN_FIRST], cl, ws.piv, tau, info, st);
@@ -403,7 +412,7 @@ int lsms_set_option(lsms_handle_t c, int option, int value) {
         case LSMS_OPT_PANEL_THREADS: case LSMS_OPT_ALIGN_FIRST: ok = value == 0 || value == 1; break;
         case LSMS_OPT_GROUPS: ok = value >= 0 && value <= MAX_GROUPS; break;
         case LSMS_OPT_PANEL_CLUSTER: ok = value == 0 || value == 1 || value == 2 || value == 4 || value == 8; break;
-        case LSMS_OPT_SMALL_MODE: ok = value >= 0 && value <= 6; break;
+        case LSMS_OPT_SMALL_MODE: ok = value >= 0 && value <= 7; break;
         default: return -2;
     }
     if (!ok) return -3;

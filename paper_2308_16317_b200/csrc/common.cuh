@@ -29,6 +29,23 @@ __device__ __forceinline__ c128 crecip(c128 a) {
     if (fabs(a.x) >= fabs(a.y)) { double r = a.y / a.x, d = a.x + a.y * r; return cmake(1.0 / d, -r / d); }
     double r = a.x / a.y, d = a.x * r + a.y; return cmake(r / d, -1.0 / d);
 }
+// 1/a without a division instruction, for the latency-bound pivot steps of the small-matrix kernels: a is scaled by a
+// power of two taken from the exponent of |re|+|im|, so that the squared modulus d lies in [1/2, 4] for any finite
+// non-zero a; 1/d = hardware seed (rcp.approx.ftz.f64, ~20 bits) + three Newton steps (6 dependent DFMAs, no special
+// cases to branch on).  Within 2 ulp of crecip.  a = 0 / Inf / NaN give garbage (callers flag such pivots themselves).
+__device__ __forceinline__ c128 crecip_fast(c128 a) {
+    long long e = (__double_as_longlong(fabs(a.x) + fabs(a.y)) >> 52) & 0x7FF;
+    e = e < 2 ? 2 : (e > 2044 ? 2044 : e);
+    const double sc = __longlong_as_double((2046 - e) << 52);           // 2^(1023 - e): sc * (|re|+|im|) in [1, 2)
+    const double xs = a.x * sc, ys = a.y * sc;
+    const double d = fma(xs, xs, ys * ys);
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+#pragma unroll
+    for (int i = 0; i < 3; ++i) r = fma(r, fma(-d, r, 1.0), r);
+    const double inv = r * sc;
+    return cmake(xs * inv, -ys * inv);
+}
 __device__ __forceinline__ c128 cdiv(c128 a, c128 b) { return cmul(a, crecip(b)); }
 // LAPACK's cabs1: |re| + |im| (the pivot-search magnitude of izamax)
 __device__ __forceinline__ double cabs1(c128 a) { return fabs(a.x) + fabs(a.y); }

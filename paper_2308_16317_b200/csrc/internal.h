@@ -49,6 +49,7 @@ int init_attrs_gemm();
 int init_attrs_lu();
 int init_attrs_assemble();
 int init_attrs_fused();
+int init_attrs_resident();
 
 // assemble.cu
 size_t gaunt_table_bytes(int lmax);
@@ -89,6 +90,10 @@ bool fused_supported(int n, int k, int NB, int IB);
 bool fused_is_tiny(int n);
 int launch_lu_fused(c128* base, size_t stride, int n, int k, int batch, int NB, int IB, int align_first, int cl,
                     int* piv, c128* tau, int* info, cudaStream_t st);
+
+// resident.cu -- small-matrix mode, on-chip variant: the matrix lives in the distributed shared memory of a cluster
+int resident_cluster_size(int n, int k);             // smallest cluster that holds an n x n matrix on chip (0: none)
+int launch_lu_resident(c128* base, size_t stride, int n, int k, int batch, int cl, int* piv, c128* tau, int* info, cudaStream_t st);
 
 // reduce.cu
 int launch_contour_sum(const c128* tau, const c128* w, int n_atoms, int n_e, int kk, c128* out, cudaStream_t st);

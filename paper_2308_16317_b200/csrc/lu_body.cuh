@@ -118,4 +118,57 @@ __device__ __forceinline__ void final_inverse_body(const c128* __restrict__ A, i
     for (int e = tid; e < k * k; e += THREADS) out[e] = S[e];
 }
 
+// K5 for a SMALL block (k*k <= 4*THREADS, e.g. k = 16 or 32 with 512 threads), trimmed for latency: one thread per
+// element (up to four), every thread finds the pivot of column j for itself (k broadcast reads, no exchange), the new
+// value of each element is computed from the OLD matrix, then written: two CTA barriers per elimination step instead
+// of six plus a serial section.  Same in-place Gauss-Jordan arithmetic and pivot rule as final_inverse_body.
+template <int THREADS>
+__device__ __forceinline__ void final_inverse_small(const c128* __restrict__ A, int n, int k, c128* __restrict__ out,
+                                                    int* __restrict__ info, c128* S, int* cpiv) {
+    const int ne = n - k, tid = threadIdx.x, kk = k * k;
+    for (int e = tid; e < kk; e += THREADS) { const int r = e % k, c = e / k; S[e] = A[(ne + r) + (size_t)(ne + c) * n]; }
+    __syncthreads();
+    bool failed = false;
+    for (int j = 0; j < k; ++j) {
+        double bv = -1.0; int p = j;
+        for (int i = j; i < k; ++i) { const double a = cabs1(S[i + j * k]); if (a > bv) { bv = a; p = i; } }
+        if (!(bv > 0.0) || !(bv < 1.0e300 * 1.0e300)) {            // the same for every thread
+            if (tid == 0) atomicCAS(info, 0, ne + j + 1);
+            failed = true;
+            break;
+        }
+        if (tid == 0) cpiv[j] = p;
+        const c128 rp = crecip_fast(S[p + j * k]);
+        c128 nv[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int e = tid + u * THREADS;
+            if (e < kk) {
+                const int i = e % k, c = e / k;
+                const c128 rowj = cmul((c == j) ? cmake(1.0, 0.0) : S[p + c * k], rp);      // new row j, column c
+                if (i == j) nv[u] = rowj;
+                else {
+                    const int src = (i == p) ? j : i;                                        // rows j and p change places
+                    const c128 f = S[src + j * k];
+                    if (c == j) nv[u] = cneg(cmul(f, rp));
+                    else { c128 x = S[src + c * k]; cfms(x, f, rowj); nv[u] = x; }
+                }
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const int e = tid + u * THREADS; if (e < kk) S[e] = nv[u]; }
+        __syncthreads();
+    }
+    if (!failed && tid < k) {
+        // undo the row interchanges as column interchanges, in reverse order; thread r owns row r
+        for (int j = k - 1; j >= 0; --j) {
+            const int p = cpiv[j];
+            if (p != j) { const c128 t = S[tid + j * k]; S[tid + j * k] = S[tid + p * k]; S[tid + p * k] = t; }
+        }
+    }
+    __syncthreads();
+    for (int e = tid; e < kk; e += THREADS) out[e] = S[e];
+}
+
 }  // namespace lsms

@@ -1,0 +1,389 @@
+// resident.cu -- small-matrix mode, ON-CHIP variant (SURVEY.md 8(a) a7 / 7.3 hard part 5; BASELINE.json north_star:
+// "a batch scheduler that packs small LIZ matrices several per SM and lets large ones span the whole chip").
+//
+// For matrices of a few hundred rows (BASELINE.json configs[0]: 208 x 208, 692 KB) nothing but the chain of n-k
+// dependent pivot steps costs time, and every trip to L2 lengthens it.  Here a matrix never leaves the chip between its
+// first and its last elimination step: a thread-block CLUSTER of 1 / 2 / 4 / 8 CTAs (one CTA per SM) holds it in
+// distributed shared memory, column blocks of RW = 8 dealt round-robin over the CTAs, and the whole elimination
+// ("LU factorization"; restricted pivoting, reading A14; only the central block of
+// the inverse is wanted) runs in one launch:
+//
+//   for each panel p (columns [8p, 8p+8), owner = CTA p mod ncl):
+//     R1  owner, one matrix row per thread, the row's 8 panel entries in registers: 8 pivot steps with ONE barrier
+//         each (every warp publishes its arg-max candidate -- found by two redux.sync on a 64-bit key -- TOGETHER
+//         with that row's entries and the reciprocal of the would-be pivot, so the winner's row is already in shared
+//         memory when the barrier opens); rows never move between threads, each thread tracks the position of its
+//         row in the pivoted arrangement; result -> the owner's panel buffer
+//     R2  cluster barrier (all CTAs are done with the previous panel), then the panel buffer is sent to the other
+//         CTAs by the TMA engine: bulk copies shared -> remote shared (cp.async.bulk.shared::cluster.shared::cta),
+//         completion counted on an mbarrier of the RECEIVING CTA -- no second cluster barrier
+//     R3  every CTA, its own trailing columns: the panel's interchanges and the 8 x 8 unit-lower solve, one thread per
+//         column (rows of U -> a small operand buffer and, for the verification export, to global memory)
+//     R4  rank-8 update of its trailing columns on the FP64 tensor pipe (DMMA.8x8x4 from shared memory; operand
+//         strides chosen conflict-free: ld = 1, ldp = 2, ldu = 4 (mod 8) complex units)
+//   K5  the trailing k x k block goes to global memory and rank 0 inverts it (final_inverse_body).
+//
+// Global traffic: the matrix is read once (TMA bulk loads, one per column); U and the final block are written once.
+#include "common.cuh"
+#include "internal.h"
+#include "gemm_body.cuh"
+#include "lu_body.cuh"
+
+namespace lsms {
+
+constexpr int RS_T = 512;            // threads per CTA
+constexpr int RS_PT = 256;           // panel threads = largest n
+constexpr int RW = 8;                // panel width = column-block width
+constexpr int RS_LDU = RW + 4;       // U operand buffer stride (complex), == 4 (mod 8)
+constexpr size_t RS_SMEM_MAX = 232448;
+
+struct ResLayout {
+    int ld, ldp, ncols_max;
+    size_t off_L, off_piv, off_U, off_red, off_bar, total;
+};
+// red region: 2 parities x 8 warp slots x (8 row entries + 1/candidate + key)
+constexpr size_t RS_SLOT = (RW + 2) * sizeof(c128);               // row entries, reciprocal of the candidate, arg-max key
+constexpr size_t RS_RED_PAR = 8 * RS_SLOT;
+__host__ __device__ inline ResLayout res_layout(int n, int ncl) {
+    ResLayout L;
+    const int nblk = (n + RW - 1) / RW, blk_max = (nblk + ncl - 1) / ncl;
+    L.ncols_max = blk_max * RW;
+    L.ld = (n + 6) / 8 * 8 + 1;                  // >= n, == 1 (mod 8)
+    L.ldp = (n + 5) / 8 * 8 + 2;                 // >= n, == 2 (mod 8)
+    size_t o = (size_t)L.ncols_max * L.ld * sizeof(c128);
+    L.off_L = o; o += (size_t)RW * L.ldp * sizeof(c128);
+    L.off_piv = o; o += 32 * sizeof(c128);       // 8 pivot ints (32 B, bulk-copied) + slack for tile over-reads
+    L.off_U = o; o += (size_t)L.ncols_max * RS_LDU * sizeof(c128);
+    L.off_red = o; o += 2 * RS_RED_PAR;
+    L.off_bar = o; o += 64;
+    L.total = o;
+    return L;
+}
+
+#ifdef LSMS_RES_TIMING
+// working aid (not compiled by default): per-phase cycles of thread 0 of CTA 0
+__device__ unsigned long long g_res_cyc[16];
+#define R_TIC() long long t__ = clock64()
+#define R_TOC(i) do { if (threadIdx.x == 0 && blockIdx.x == 0) { long long n__ = clock64(); atomicAdd(&g_res_cyc[i], (unsigned long long)(n__ - t__)); t__ = clock64(); } } while (0)
+extern "C" int lsms_work_res_cycles(unsigned long long* out_host, int reset) {
+    if (out_host) cudaMemcpyFromSymbol(out_host, g_res_cyc, sizeof(unsigned long long) * 16);
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_res_cyc, z, sizeof(z)); }
+    return 0;
+}
+#else
+#define R_TIC() do {} while (0)
+#define R_TOC(i) do {} while (0)
+#endif
+
+__device__ __forceinline__ uint32_t rs_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t rs_ncl() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t rs_mapa(uint32_t addr, uint32_t rank) {
+    uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank)); return r;
+}
+__device__ __forceinline__ void rs_cluster_sync() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared (this CTA) -> shared of another CTA of the cluster, by the TMA engine; completion on the receiver's mbarrier
+__device__ __forceinline__ void rs_bulk_s2r(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(bar_cluster) : "memory");
+}
+__global__ void __launch_bounds__(RS_T, 1)
+k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restrict__ piv, c128* __restrict__ tau,
+              int* __restrict__ info) {
+    extern __shared__ __align__(128) unsigned char rsm[];
+    const int ncl = (int)rs_ncl(), rank = (int)rs_rank();
+    const ResLayout L = res_layout(n, ncl);
+    c128* Aloc = reinterpret_cast<c128*>(rsm);
+    c128* Lbuf = reinterpret_cast<c128*>(rsm + L.off_L);
+    int* spiv = reinterpret_cast<int*>(rsm + L.off_piv);
+    c128* Ubuf = reinterpret_cast<c128*>(rsm + L.off_U);
+    unsigned char* red = rsm + L.off_red;
+    uint64_t* bar_load = reinterpret_cast<uint64_t*>(rsm + L.off_bar);
+    uint64_t* bar_full = bar_load + 1;
+    const int ld = L.ld, ldp = L.ldp;
+
+    const int item = blockIdx.x / ncl;
+    c128* A = base + (size_t)item * stride;
+    int* pv = piv + (size_t)item * n;
+    int* inf = info + item;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ne = n - k;
+    const int nblk = (n + RW - 1) / RW;
+    const int my_blocks = (nblk > rank) ? (nblk - rank + ncl - 1) / ncl : 0;
+    const int my_cols = my_blocks * RW;                       // local columns incl. the padding of a ragged last block
+    auto gcol = [&](int lc) { return ((lc / RW) * ncl + rank) * RW + lc % RW; };
+
+    if (tid == 0) {
+        mbar_init(bar_load, 1); mbar_init(bar_full, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // padding columns of a ragged last block and the U buffer start as zeros
+    for (int lc = tid; lc < my_cols; lc += RS_T) if (gcol(lc) >= n) for (int r = 0; r < ld; ++r) Aloc[(size_t)lc * ld + r] = cmake(0.0, 0.0);
+    for (int e = tid; e < L.ncols_max * RS_LDU; e += RS_T) Ubuf[e] = cmake(0.0, 0.0);
+    asm volatile("fence.proxy.async;" ::: "memory");
+    __syncthreads();
+    // ---- the CTA's column blocks -> shared memory: one TMA bulk copy per column
+    {
+        int nvalid = 0;
+        for (int lc = 0; lc < my_cols; ++lc) nvalid += gcol(lc) < n;
+        if (tid == 0) mbar_expect_tx(bar_load, (uint32_t)((size_t)nvalid * n * sizeof(c128)));
+        __syncthreads();
+        for (int lc = tid; lc < my_cols; lc += RS_T) {
+            const int g = gcol(lc);
+            if (g < n) tma_bulk_g2s(Aloc + (size_t)lc * ld, A + (size_t)g * n, (uint32_t)(n * sizeof(c128)), bar_load);
+        }
+    }
+    R_TIC();
+    rs_cluster_sync();                           // every CTA of the cluster is running and its mbarriers are initialised
+    mbar_wait(bar_load, 0);
+    R_TOC(0);
+    uint32_t full_parity = 0;
+
+    const int np = (ne + RW - 1) / RW;
+    for (int p = 0; p < np; ++p) {
+        const int c0 = p * RW, wv = min(RW, ne - c0), m = n - c0;
+        const int owner = p % ncl;
+        const int lcp = (p / ncl) * RW;                         // the panel's first local column in its owner
+        if (rank == owner) {
+            // ================= R1: panel factorisation, one row per thread.  Rows are never moved between threads:
+            // thread t keeps the row it loaded and tracks the POSITION (row index relative to c0) at which that row
+            // stands in the pivoted arrangement; pivot rows are published through shared memory only.
+            const int npt = ((m + 31) / 32) * 32;                          // panel threads: whole warps covering the m rows
+            if (tid < npt) {
+                const int t = tid;
+                int pos = t;
+                int ppos_all[RW];
+                c128 v[RW];
+#pragma unroll
+                for (int c = 0; c < RW; ++c) v[c] = (t < m) ? Aloc[(size_t)(lcp + c) * ld + c0 + t] : cmake(0.0, 0.0);
+                if (t < 2 * (RS_PT / 32)) {                                // keys of the warps that sit this panel out
+                    const int w8 = t >> 1;
+                    if (w8 >= npt / 32) reinterpret_cast<unsigned long long*>(reinterpret_cast<c128*>(red + (size_t)(t & 1) * RS_RED_PAR + (size_t)w8 * RS_SLOT) + RW + 1)[0] = 0ull;
+                }
+                // reciprocal of every row's own entry of the coming column: only the pivot row's is used, but computed
+                // here (and, for the later columns, right after the entry's last update) its latency hides behind the
+                // rest of the rank-1 update and the arg-max reduction
+                c128 rinv = crecip_fast(v[0]);
+#pragma unroll
+                for (int j = 0; j < RW; ++j) {
+                    ppos_all[j] = j;
+                    if (j < wv) {
+                        unsigned char* rp_ = red + (size_t)(j & 1) * RS_RED_PAR;
+                        // Arg-max key: the bits of |re|+|im| with the low 11 mantissa bits replaced by (255 - pos, warp):
+                        // one unsigned 64-bit maximum picks the largest magnitude and, among (nearly) equal ones, the
+                        // lowest row of the current arrangement (LAPACK's rule up to 2^-41); 0 = not eligible.
+                        // Two redux.sync per warp instead of fifteen shuffles.
+                        const bool elig = (pos >= j && t < m && c0 + pos < ne);
+                        uint32_t khi = 0, klo = 0;
+                        if (elig) {
+                            const unsigned long long kb = (unsigned long long)__double_as_longlong(cabs1(v[j]));
+                            khi = (uint32_t)(kb >> 32); klo = ((uint32_t)kb & ~0x7FFu) | ((uint32_t)(255 - pos) << 3) | (uint32_t)warp;
+                        }
+                        R_TOC(8);
+                        const uint32_t mhi = __reduce_max_sync(0xffffffffu, khi);
+                        const uint32_t mlo = __reduce_max_sync(0xffffffffu, (khi == mhi) ? klo : 0u);
+                        c128* slot = reinterpret_cast<c128*>(rp_ + (size_t)warp * RS_SLOT);
+                        R_TOC(9);
+                        if (elig && khi == mhi && klo == mlo) {
+#pragma unroll
+                            for (int c = j + 1; c < RW; ++c) slot[c] = v[c];
+                            slot[RW] = rinv;
+                        }
+                        if (lane == 0) reinterpret_cast<unsigned long long*>(slot + RW + 1)[0] = ((unsigned long long)mhi << 32) | mlo;
+                        R_TOC(10);
+                        asm volatile("bar.sync 1, %0;" ::"r"(npt) : "memory");
+                        R_TOC(11);
+                        // every thread picks the winner among the warp candidates
+                        unsigned long long wk[RS_PT / 32];
+#pragma unroll
+                        for (int w8 = 0; w8 < RS_PT / 32; ++w8)
+                            wk[w8] = reinterpret_cast<const unsigned long long*>(reinterpret_cast<const c128*>(rp_ + (size_t)w8 * RS_SLOT) + RW + 1)[0];
+#pragma unroll
+                        for (int o = RS_PT / 64; o > 0; o >>= 1)
+#pragma unroll
+                            for (int w8 = 0; w8 < o; ++w8) wk[w8] = wk[w8] > wk[w8 + o] ? wk[w8] : wk[w8 + o];
+                        const unsigned long long wkey = wk[0];
+                        const uint32_t wexp = (uint32_t)(wkey >> 52);
+                        const bool bad = (wkey >> 11) == 0ull || wexp >= 0x7FFu;           // zero, NaN or Inf pivot
+                        const int ppos = bad ? j : 255 - (int)((wkey >> 3) & 0xFFull);      // position of the pivot row
+                        ppos_all[j] = bad ? -1 - j : ppos;
+                        R_TOC(12);
+                        if (!bad) {
+                            const c128* ps = reinterpret_cast<const c128*>(rp_ + (size_t)(wkey & 7ull) * RS_SLOT);
+                            c128 prow[RW];
+#pragma unroll
+                            for (int c = j + 1; c < RW; ++c) prow[c] = ps[c];
+                            const c128 rp = ps[RW];
+                            // the pivot row takes position j, the row that stood there takes the pivot row's position
+                            if (pos == ppos) pos = j; else if (pos == j) pos = ppos;
+                            R_TOC(13);
+                            if (pos > j && t < m) {
+                                const c128 l = cmul(v[j], rp);
+                                v[j] = l;
+                                if (j + 1 < RW) { cfms(v[j + 1], l, prow[j + 1]); rinv = crecip_fast(v[j + 1]); }
+#pragma unroll
+                                for (int c = j + 2; c < RW; ++c) cfms(v[c], l, prow[c]);
+                            }
+                        }
+                        R_TOC(14);
+                    }
+                }
+                if (t == 0) {
+#pragma unroll
+                    for (int j = 0; j < RW; ++j) {
+                        const int pp = ppos_all[j] < 0 ? -1 - ppos_all[j] : ppos_all[j];
+                        spiv[j] = c0 + pp;
+                        if (j < wv) { pv[c0 + j] = c0 + pp; if (ppos_all[j] < 0) atomicCAS(inf, 0, c0 + j + 1); }
+                    }
+                }
+                R_TOC(6);
+                // the factored panel: L (and U11) -> panel buffer, rows in their pivoted positions; columns beyond wv
+                // (central columns inside the last panel's block) have received all their updates here and go back
+                // to the matrix
+                if (t < m) {
+#pragma unroll
+                    for (int c = 0; c < RW; ++c) {
+                        Lbuf[(size_t)c * ldp + pos] = (c < wv) ? v[c] : cmake(0.0, 0.0);
+                        if (c >= wv) Aloc[(size_t)(lcp + c) * ld + c0 + pos] = v[c];
+                    }
+                    // rows of U held by this block: verification export (k_backsolve_central reads U11, U12)
+                    if (pos < wv) {
+#pragma unroll
+                        for (int c = 0; c < RW; ++c) if (c >= pos && c0 + c < n) A[(size_t)(c0 + pos) + (size_t)(c0 + c) * n] = v[c];
+                    }
+                }
+            }
+            R_TOC(7);
+            asm volatile("fence.proxy.async;" ::: "memory");
+            __syncthreads();
+            R_TOC(1);
+        } else if (tid == 0) {
+            mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * m * sizeof(c128) + RW * sizeof(int)));
+        }
+        // ================= R2: every CTA has finished the previous panel's update; ship the panel
+        if (ncl > 1) {
+            rs_cluster_sync();
+            if (rank == owner) {
+                if (tid < (ncl - 1) * (RW + 1)) {
+                    const int d = tid / (RW + 1), c = tid % (RW + 1);
+                    const uint32_t dst = (uint32_t)((d >= rank) ? d + 1 : d);
+                    const uint32_t rbar = rs_mapa(smem_u32(bar_full), dst);
+                    if (c < RW) rs_bulk_s2r(rs_mapa(smem_u32(Lbuf + (size_t)c * ldp), dst), smem_u32(Lbuf + (size_t)c * ldp), (uint32_t)(m * sizeof(c128)), rbar);
+                    else rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv), (uint32_t)(RW * sizeof(int)), rbar);
+                }
+            } else {
+                mbar_wait(bar_full, full_parity); full_parity ^= 1;
+            }
+        }
+        R_TOC(2);
+        // ================= R3: interchanges + 8 x 8 unit-lower solve, one thread per trailing local column
+        const int tl0 = (p >= rank) ? ((p - rank) / ncl + 1) * RW : 0;          // first local column right of block p
+        const int ntl = my_cols - tl0;
+        for (int lc = tl0 + tid; lc < my_cols; lc += RS_T) {
+            c128* col = Aloc + (size_t)lc * ld;
+            for (int i = 0; i < wv; ++i) {
+                const int pr = spiv[i];
+                if (pr != c0 + i) { const c128 a = col[c0 + i]; col[c0 + i] = col[pr]; col[pr] = a; }
+            }
+            c128 x[RW];
+#pragma unroll
+            for (int i = 0; i < RW; ++i) x[i] = (i < wv) ? col[c0 + i] : cmake(0.0, 0.0);
+#pragma unroll
+            for (int jq = 0; jq < RW; ++jq)
+#pragma unroll
+                for (int i = jq + 1; i < RW; ++i)
+                    if (i < wv) cfms(x[i], Lbuf[(size_t)jq * ldp + i], x[jq]);
+            const int g = gcol(lc);
+#pragma unroll
+            for (int i = 0; i < RW; ++i) {
+                Ubuf[(size_t)lc * RS_LDU + i] = x[i];
+                if (i < wv && g < n) A[(size_t)(c0 + i) + (size_t)g * n] = x[i];
+            }
+        }
+        __syncthreads();
+        R_TOC(3);
+        // ================= R4: rank-8 update of rows [c0+wv, n) x trailing local columns on DMMA, warp tiles of 32 x 8
+        {
+            const int r_lo = c0 + wv, mrows = n - r_lo;
+            const int tiles_m = (mrows + 31) / 32, tiles_n = ntl / RW;
+            const int gq = lane >> 2, q = lane & 3;
+            for (int tt = warp; tt < tiles_m * tiles_n; tt += RS_T / 32) {
+                const int tm = tt % tiles_m, tn = tt / tiles_m;
+                const int r0 = r_lo + tm * 32, lc0 = tl0 + tn * RW;
+                double cr[4][2], ci[4][2];
+                c128* Cb = Aloc + (size_t)(lc0 + 2 * q) * ld + r0 + gq;
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) { const c128 cv = Cb[(size_t)e * ld + mt * 8]; cr[mt][e] = cv.x; ci[mt][e] = cv.y; }
+#pragma unroll
+                for (int ks = 0; ks < RW / 4; ++ks) {
+                    const c128 b = Ubuf[(size_t)(lc0 + gq) * RS_LDU + ks * 4 + q];
+                    const double nbr = -b.x, nbi = -b.y;
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt) {
+                        const c128 a = Lbuf[(size_t)(ks * 4 + q) * ldp + (r0 - c0) + mt * 8 + gq];
+                        dmma884(cr[mt][0], cr[mt][1], a.x, nbr);
+                        dmma884(ci[mt][0], ci[mt][1], a.x, nbi);
+                        dmma884(cr[mt][0], cr[mt][1], a.y, b.y);
+                        dmma884(ci[mt][0], ci[mt][1], a.y, nbr);
+                    }
+                }
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e)
+                        if (r0 + mt * 8 + gq < n) Cb[(size_t)e * ld + mt * 8] = cmake(cr[mt][e], ci[mt][e]);
+            }
+        }
+        __syncthreads();
+        R_TOC(4);
+    }
+    // ================= K5: the trailing k x k block -> global memory, inverted by rank 0
+    for (int e = tid; e < my_cols * k; e += RS_T) {
+        const int lc = e / k, r = e % k, g = gcol(lc);
+        if (g >= ne && g < n) A[(size_t)(ne + r) + (size_t)g * n] = Aloc[(size_t)lc * ld + ne + r];
+    }
+    if (ncl > 1) { __threadfence(); rs_cluster_sync(); } else __syncthreads();
+    if (rank == 0) {
+        c128* S = reinterpret_cast<c128*>(rsm + 8192);
+        if (k * k <= 4 * RS_T) final_inverse_small<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, reinterpret_cast<int*>(rsm));
+        else final_inverse_body<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, *reinterpret_cast<K5Shared*>(rsm));
+    }
+    R_TOC(5);
+    if (ncl > 1) rs_cluster_sync();             // no CTA leaves while its shared memory may still be a copy target
+}
+
+// smallest cluster whose CTAs can hold the matrix (0: none)
+int resident_cluster_size(int n, int k) {
+    if (n < 1 || n > RS_PT || k < 1 || k > n || 8192 + (size_t)k * k * sizeof(c128) > 160 * 1024) return 0;
+    for (int cl = 1; cl <= 8; cl *= 2)
+        if (res_layout(n, cl).total <= RS_SMEM_MAX && 8192 + (size_t)k * k * sizeof(c128) <= res_layout(n, cl).total) return cl;
+    return 0;
+}
+
+int init_attrs_resident() {
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_lu_resident, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS_SMEM_MAX));
+    return 0;
+}
+
+int launch_lu_resident(c128* base, size_t stride, int n, int k, int batch, int cl, int* piv, c128* tau, int* info, cudaStream_t st) {
+    const int cl_min = resident_cluster_size(n, k);
+    if (cl_min == 0 || cl < cl_min || (cl != 1 && cl != 2 && cl != 4 && cl != 8)) return -1;
+    const size_t smem = res_layout(n, cl).total;
+    for (int b0 = 0; b0 < batch; b0 += 16384) {
+        const int nb = batch - b0 < 16384 ? batch - b0 : 16384;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(nb * cl)); cfg.blockDim = dim3(RS_T); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = (unsigned)cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        LSMS_CUDA_OK(cudaLaunchKernelEx(&cfg, k_lu_resident, base + (size_t)b0 * stride, stride, n, k, piv + (size_t)b0 * n,
+                                        tau + (size_t)b0 * k * k, info + b0));
+        LSMS_LAUNCH_CHECK();
+    }
+    return 0;
+}
+
+}  // namespace lsms

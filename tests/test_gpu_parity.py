@@ -326,12 +326,15 @@ def lapack_tau00(A, k):
     return np.linalg.inv(A.T)[n - k:, n - k:]
 
 
-@pytest.mark.parametrize("small", [1, 2, 3, 5])
+@pytest.mark.parametrize("small", [0, 1, 2, 3, 5, 7])
 @pytest.mark.parametrize("n_sites,kmax,canted", [(7, 9, False), (37, 1, False), (1, 16, False), (2, 4, True),
-                                                  (33, 4, False), (5, 25, True), (129, 1, False), (23, 9, False), (150, 9, False)])
+                                                  (33, 4, False), (5, 25, True), (129, 1, False), (23, 9, False), (150, 9, False),
+                                                  (13, 16, False), (27, 4, True), (2, 25, True), (43, 4, False)])
 def test_random_matrices_vs_lapack(lt, h, n_sites, kmax, canted, small):
     """Dense random matrices (strong pivoting) of ragged shapes through the lock-step schedule (small = 1), the
-    small-matrix mode with the cluster size chosen by the scheduler (2), one CTA per matrix (3) and a 4-CTA cluster (5)."""
+    small-matrix mode through L2 with the cluster size chosen by the scheduler (2), one CTA per matrix (3) and a 4-CTA
+    cluster (5), the on-chip small-matrix mode (7: matrix in the distributed shared memory of a 1/2/4-CTA cluster, shapes
+    with ragged last column blocks, ragged last panels and k up to 100) and the scheduler's own choice (0)."""
     k = kmax * (2 if canted else 1)
     n = n_sites * k
     h.set("small_mode", small)
@@ -339,14 +342,21 @@ def test_random_matrices_vs_lapack(lt, h, n_sites, kmax, canted, small):
     M = torch.from_numpy(A).cuda()
     tau, info = lt.lsms_tau00_batched(h, M, n_sites, kmax, canted, 5)
     torch.cuda.synchronize()
-    assert lt.lsms_last_schedule(h) == {1: 0, 2: 4 if n <= 212 else 8, 3: 1, 5: 4}[small]
+    sched = lt.lsms_last_schedule(h)
+    if small in (0, 7):            # on chip (100 + cluster size) when the matrix fits the shared memory of <= 8 SMs
+        if n <= 216:
+            assert sched == 101 if n <= 112 else sched > 101
+        if n > 256:
+            assert sched == 0
+    else:
+        assert sched == {1: 0, 2: 4 if n <= 212 else 8, 3: 1, 5: 4}[small]
     tau = tau.cpu().numpy().transpose(0, 2, 1)
     assert not info.cpu().numpy().any()
     for b in range(5):
         check_tau(tau[b], lapack_tau00(A[b], k), 1e-10 if n > 1000 else 1e-11, (n, b))
 
 
-@pytest.mark.parametrize("small", [1, 2, 3, 4, 6])
+@pytest.mark.parametrize("small", [0, 1, 2, 3, 4, 6, 7])
 def test_needs_pivoting_and_singular_info(lt, h, small):
     # zero on the leading diagonal: fails without row interchanges
     n_sites, kmax = 6, 4
@@ -496,10 +506,10 @@ def test_small_mode_is_chosen_for_the_small_configs_and_matches_the_oracle(lt, h
     ref, _ = oracle.tau00_batched(batch, "long double")
     tau, info, _ = lt.tau00_from_liz_batch(h, batch)
     assert not info.any()
-    assert lt.lsms_last_schedule(h) >= 1 and lt.lsms_last_launch_count(h) == 1
+    assert lt.lsms_last_schedule(h) == 104 and lt.lsms_last_launch_count(h) == 1     # on chip, 4 SMs per matrix
     for b in range(32):
         check_tau(tau[b], ref[b], 1e-12, ("T default", b))
-    for sm, cl in ((2, None), (3, 1), (4, 2), (5, 4), (6, 8)):
+    for sm, cl in ((2, None), (3, 1), (4, 2), (5, 4), (6, 8), (7, 104)):
         h.set("small_mode", sm)
         tau, info, _ = lt.tau00_from_liz_batch(h, batch)
         assert not info.any()
