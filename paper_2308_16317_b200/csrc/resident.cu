@@ -8,7 +8,7 @@
 // ("LU factorization"; restricted pivoting, reading A14; only the central block of
 // the inverse is wanted) runs in one launch:
 //
-//   for each panel p (columns [8p, 8p+8), owner = CTA p mod ncl):
+//   for each panel p (columns [8p, 8p+8), owner = CTA p mod ncl; R1 of panel p+1 runs DURING step p, see below):
 //     R1  owner, one matrix row per thread, the row's 8 panel entries in registers: 8 pivot steps with ONE barrier
 //         each (every warp publishes its arg-max candidate -- found by two redux.sync on a 64-bit key -- TOGETHER
 //         with that row's entries and the reciprocal of the would-be pivot, so the winner's row is already in shared
@@ -21,7 +21,9 @@
 //         column (rows of U -> a small operand buffer and, for the verification export, to global memory)
 //     R4  rank-8 update of its trailing columns on the FP64 tensor pipe (DMMA.8x8x4 from shared memory; operand
 //         strides chosen conflict-free: ld = 1, ldp = 2, ldu = 4 (mod 8) complex units)
-//   K5  the trailing k x k block goes to global memory and rank 0 inverts it (final_inverse_body).
+//   K5  the trailing k x k block goes to global memory and rank 0 inverts it (final_inverse_small).
+// LOOK-AHEAD: the CTA that owns panel p+1 updates that block first (R3, R4 on its 8 columns), then half of its warps
+// factor panel p+1 (R1) while the other half -- and the other CTAs -- finish step p.
 //
 // Global traffic: the matrix is read once (TMA bulk loads, one per column); U and the final block are written once.
 #include "common.cuh"
@@ -52,7 +54,7 @@ __host__ __device__ inline ResLayout res_layout(int n, int ncl) {
     L.ldp = (n + 5) / 8 * 8 + 2;                 // >= n, == 2 (mod 8)
     size_t o = (size_t)L.ncols_max * L.ld * sizeof(c128);
     L.off_L = o; o += (size_t)RW * L.ldp * sizeof(c128);
-    L.off_piv = o; o += 32 * sizeof(c128);       // 8 pivot ints (32 B, bulk-copied) + slack for tile over-reads
+    L.off_piv = o; o += 32 * sizeof(c128);       // net row permutation of the panel (96 B, bulk-copied) + slack for tile over-reads
     L.off_U = o; o += (size_t)L.ncols_max * RS_LDU * sizeof(c128);
     L.off_red = o; o += 2 * RS_RED_PAR;
     L.off_bar = o; o += 64;
@@ -139,127 +141,212 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
     mbar_wait(bar_load, 0);
     R_TOC(0);
     uint32_t full_parity = 0;
-
     const int np = (ne + RW - 1) / RW;
-    for (int p = 0; p < np; ++p) {
+
+    // ---- state of a panel factorisation: lives in the registers of the owner's panel threads from R1 (which may run
+    // during the PREVIOUS panel's update, see the look-ahead below) to the publication at the top of the panel's own step
+    c128 v[RW];
+    int pos = 0, ppos_all[RW];
+#pragma unroll
+    for (int c = 0; c < RW; ++c) { v[c] = cmake(0.0, 0.0); ppos_all[c] = c; }
+
+    // ================= R1: panel factorisation, one row per thread (threads < npt of the owner).  Rows are never moved
+    // between threads: thread t keeps the row it loaded and tracks the POSITION (row index relative to c0) at which
+    // that row stands in the pivoted arrangement; pivot rows are published through shared memory only.
+    auto panel_factor = [&](int p) {
         const int c0 = p * RW, wv = min(RW, ne - c0), m = n - c0;
-        const int owner = p % ncl;
-        const int lcp = (p / ncl) * RW;                         // the panel's first local column in its owner
-        if (rank == owner) {
-            // ================= R1: panel factorisation, one row per thread.  Rows are never moved between threads:
-            // thread t keeps the row it loaded and tracks the POSITION (row index relative to c0) at which that row
-            // stands in the pivoted arrangement; pivot rows are published through shared memory only.
-            const int npt = ((m + 31) / 32) * 32;                          // panel threads: whole warps covering the m rows
-            if (tid < npt) {
-                const int t = tid;
-                int pos = t;
-                int ppos_all[RW];
-                c128 v[RW];
+        const int lcp = (p / ncl) * RW;                                // the panel's first local column in its owner
+        const int npt = ((m + 31) / 32) * 32;                          // panel threads: whole warps covering the m rows
+        if (tid >= npt) return;
+        const int t = tid;
+        pos = t;
 #pragma unroll
-                for (int c = 0; c < RW; ++c) v[c] = (t < m) ? Aloc[(size_t)(lcp + c) * ld + c0 + t] : cmake(0.0, 0.0);
-                if (t < 2 * (RS_PT / 32)) {                                // keys of the warps that sit this panel out
-                    const int w8 = t >> 1;
-                    if (w8 >= npt / 32) reinterpret_cast<unsigned long long*>(reinterpret_cast<c128*>(red + (size_t)(t & 1) * RS_RED_PAR + (size_t)w8 * RS_SLOT) + RW + 1)[0] = 0ull;
+        for (int c = 0; c < RW; ++c) v[c] = (t < m) ? Aloc[(size_t)(lcp + c) * ld + c0 + t] : cmake(0.0, 0.0);
+        if (t < 2 * (RS_PT / 32)) {                                    // keys of the warps that sit this panel out
+            const int w8 = t >> 1;
+            if (w8 >= npt / 32) reinterpret_cast<unsigned long long*>(reinterpret_cast<c128*>(red + (size_t)(t & 1) * RS_RED_PAR + (size_t)w8 * RS_SLOT) + RW + 1)[0] = 0ull;
+        }
+        // reciprocal of every row's own entry of the coming column: only the pivot row's is used, but computed here
+        // (and, for the later columns, right after the entry's last update) its latency hides behind the rest of the
+        // rank-1 update and the arg-max reduction
+        c128 rinv = crecip_fast(v[0]);
+#pragma unroll
+        for (int j = 0; j < RW; ++j) {
+            ppos_all[j] = j;
+            if (j < wv) {
+                unsigned char* rp_ = red + (size_t)(j & 1) * RS_RED_PAR;
+                // Arg-max key: the bits of |re|+|im| with the low 11 mantissa bits replaced by (255 - pos, warp): one
+                // unsigned 64-bit maximum picks the largest magnitude and, among (nearly) equal ones, the lowest row of
+                // the current arrangement (LAPACK's rule up to 2^-41); 0 = not eligible.  Two redux.sync per warp
+                // instead of fifteen shuffles.
+                const bool elig = (pos >= j && t < m && c0 + pos < ne);
+                uint32_t khi = 0, klo = 0;
+                if (elig) {
+                    const unsigned long long kb = (unsigned long long)__double_as_longlong(cabs1(v[j]));
+                    khi = (uint32_t)(kb >> 32); klo = ((uint32_t)kb & ~0x7FFu) | ((uint32_t)(255 - pos) << 3) | (uint32_t)warp;
                 }
-                // reciprocal of every row's own entry of the coming column: only the pivot row's is used, but computed
-                // here (and, for the later columns, right after the entry's last update) its latency hides behind the
-                // rest of the rank-1 update and the arg-max reduction
-                c128 rinv = crecip_fast(v[0]);
+                const uint32_t mhi = __reduce_max_sync(0xffffffffu, khi);
+                const uint32_t mlo = __reduce_max_sync(0xffffffffu, (khi == mhi) ? klo : 0u);
+                c128* slot = reinterpret_cast<c128*>(rp_ + (size_t)warp * RS_SLOT);
+                if (elig && khi == mhi && klo == mlo) {
 #pragma unroll
-                for (int j = 0; j < RW; ++j) {
-                    ppos_all[j] = j;
-                    if (j < wv) {
-                        unsigned char* rp_ = red + (size_t)(j & 1) * RS_RED_PAR;
-                        // Arg-max key: the bits of |re|+|im| with the low 11 mantissa bits replaced by (255 - pos, warp):
-                        // one unsigned 64-bit maximum picks the largest magnitude and, among (nearly) equal ones, the
-                        // lowest row of the current arrangement (LAPACK's rule up to 2^-41); 0 = not eligible.
-                        // Two redux.sync per warp instead of fifteen shuffles.
-                        const bool elig = (pos >= j && t < m && c0 + pos < ne);
-                        uint32_t khi = 0, klo = 0;
-                        if (elig) {
-                            const unsigned long long kb = (unsigned long long)__double_as_longlong(cabs1(v[j]));
-                            khi = (uint32_t)(kb >> 32); klo = ((uint32_t)kb & ~0x7FFu) | ((uint32_t)(255 - pos) << 3) | (uint32_t)warp;
-                        }
-                        R_TOC(8);
-                        const uint32_t mhi = __reduce_max_sync(0xffffffffu, khi);
-                        const uint32_t mlo = __reduce_max_sync(0xffffffffu, (khi == mhi) ? klo : 0u);
-                        c128* slot = reinterpret_cast<c128*>(rp_ + (size_t)warp * RS_SLOT);
-                        R_TOC(9);
-                        if (elig && khi == mhi && klo == mlo) {
-#pragma unroll
-                            for (int c = j + 1; c < RW; ++c) slot[c] = v[c];
-                            slot[RW] = rinv;
-                        }
-                        if (lane == 0) reinterpret_cast<unsigned long long*>(slot + RW + 1)[0] = ((unsigned long long)mhi << 32) | mlo;
-                        R_TOC(10);
-                        asm volatile("bar.sync 1, %0;" ::"r"(npt) : "memory");
-                        R_TOC(11);
-                        // every thread picks the winner among the warp candidates
-                        unsigned long long wk[RS_PT / 32];
-#pragma unroll
-                        for (int w8 = 0; w8 < RS_PT / 32; ++w8)
-                            wk[w8] = reinterpret_cast<const unsigned long long*>(reinterpret_cast<const c128*>(rp_ + (size_t)w8 * RS_SLOT) + RW + 1)[0];
-#pragma unroll
-                        for (int o = RS_PT / 64; o > 0; o >>= 1)
-#pragma unroll
-                            for (int w8 = 0; w8 < o; ++w8) wk[w8] = wk[w8] > wk[w8 + o] ? wk[w8] : wk[w8 + o];
-                        const unsigned long long wkey = wk[0];
-                        const uint32_t wexp = (uint32_t)(wkey >> 52);
-                        const bool bad = (wkey >> 11) == 0ull || wexp >= 0x7FFu;           // zero, NaN or Inf pivot
-                        const int ppos = bad ? j : 255 - (int)((wkey >> 3) & 0xFFull);      // position of the pivot row
-                        ppos_all[j] = bad ? -1 - j : ppos;
-                        R_TOC(12);
-                        if (!bad) {
-                            const c128* ps = reinterpret_cast<const c128*>(rp_ + (size_t)(wkey & 7ull) * RS_SLOT);
-                            c128 prow[RW];
-#pragma unroll
-                            for (int c = j + 1; c < RW; ++c) prow[c] = ps[c];
-                            const c128 rp = ps[RW];
-                            // the pivot row takes position j, the row that stood there takes the pivot row's position
-                            if (pos == ppos) pos = j; else if (pos == j) pos = ppos;
-                            R_TOC(13);
-                            if (pos > j && t < m) {
-                                const c128 l = cmul(v[j], rp);
-                                v[j] = l;
-                                if (j + 1 < RW) { cfms(v[j + 1], l, prow[j + 1]); rinv = crecip_fast(v[j + 1]); }
-#pragma unroll
-                                for (int c = j + 2; c < RW; ++c) cfms(v[c], l, prow[c]);
-                            }
-                        }
-                        R_TOC(14);
-                    }
+                    for (int c = j + 1; c < RW; ++c) slot[c] = v[c];
+                    slot[RW] = rinv;
                 }
-                if (t == 0) {
+                if (lane == 0) reinterpret_cast<unsigned long long*>(slot + RW + 1)[0] = ((unsigned long long)mhi << 32) | mlo;
+                asm volatile("bar.sync 1, %0;" ::"r"(npt) : "memory");
+                // every thread picks the winner among the warp candidates
+                unsigned long long wk[RS_PT / 32];
 #pragma unroll
-                    for (int j = 0; j < RW; ++j) {
-                        const int pp = ppos_all[j] < 0 ? -1 - ppos_all[j] : ppos_all[j];
-                        spiv[j] = c0 + pp;
-                        if (j < wv) { pv[c0 + j] = c0 + pp; if (ppos_all[j] < 0) atomicCAS(inf, 0, c0 + j + 1); }
-                    }
-                }
-                R_TOC(6);
-                // the factored panel: L (and U11) -> panel buffer, rows in their pivoted positions; columns beyond wv
-                // (central columns inside the last panel's block) have received all their updates here and go back
-                // to the matrix
-                if (t < m) {
+                for (int w8 = 0; w8 < RS_PT / 32; ++w8)
+                    wk[w8] = reinterpret_cast<const unsigned long long*>(reinterpret_cast<const c128*>(rp_ + (size_t)w8 * RS_SLOT) + RW + 1)[0];
 #pragma unroll
-                    for (int c = 0; c < RW; ++c) {
-                        Lbuf[(size_t)c * ldp + pos] = (c < wv) ? v[c] : cmake(0.0, 0.0);
-                        if (c >= wv) Aloc[(size_t)(lcp + c) * ld + c0 + pos] = v[c];
-                    }
-                    // rows of U held by this block: verification export (k_backsolve_central reads U11, U12)
-                    if (pos < wv) {
+                for (int o = RS_PT / 64; o > 0; o >>= 1)
 #pragma unroll
-                        for (int c = 0; c < RW; ++c) if (c >= pos && c0 + c < n) A[(size_t)(c0 + pos) + (size_t)(c0 + c) * n] = v[c];
+                    for (int w8 = 0; w8 < o; ++w8) wk[w8] = wk[w8] > wk[w8 + o] ? wk[w8] : wk[w8 + o];
+                const unsigned long long wkey = wk[0];
+                const bool bad = (wkey >> 11) == 0ull || (uint32_t)(wkey >> 52) >= 0x7FFu;    // zero, NaN or Inf pivot
+                const int ppos = bad ? j : 255 - (int)((wkey >> 3) & 0xFFull);                // position of the pivot row
+                ppos_all[j] = bad ? -1 - j : ppos;
+                if (!bad) {
+                    const c128* ps = reinterpret_cast<const c128*>(rp_ + (size_t)(wkey & 7ull) * RS_SLOT);
+                    c128 prow[RW];
+#pragma unroll
+                    for (int c = j + 1; c < RW; ++c) prow[c] = ps[c];
+                    const c128 rp = ps[RW];
+                    // the pivot row takes position j, the row that stood there takes the pivot row's position
+                    if (pos == ppos) pos = j; else if (pos == j) pos = ppos;
+                    if (pos > j && t < m) {
+                        const c128 l = cmul(v[j], rp);
+                        v[j] = l;
+                        if (j + 1 < RW) { cfms(v[j + 1], l, prow[j + 1]); rinv = crecip_fast(v[j + 1]); }
+#pragma unroll
+                        for (int c = j + 2; c < RW; ++c) cfms(v[c], l, prow[c]);
                     }
                 }
             }
-            R_TOC(7);
+        }
+    };
+    // The factored panel -> shared memory: L (and U11) into the panel buffer, rows in their pivoted positions, and the net
+    // row permutation of the panel's interchanges (spiv[8..16): top_src, row whose content ends in top position i;
+    // spiv[16..24): ddst, row below the top block that receives the ORIGINAL top row i, or -1).  Columns beyond wv
+    // (central columns inside the last panel's block) have received all their updates in R1 and go back to the matrix.
+    auto panel_publish = [&](int p) {
+        const int c0 = p * RW, wv = min(RW, ne - c0), m = n - c0;
+        const int lcp = (p / ncl) * RW;
+        if (tid < m) {
+#pragma unroll
+            for (int c = 0; c < RW; ++c) {
+                Lbuf[(size_t)c * ldp + pos] = (c < wv) ? v[c] : cmake(0.0, 0.0);
+                if (c >= wv) Aloc[(size_t)(lcp + c) * ld + c0 + pos] = v[c];
+            }
+            if (pos < wv) spiv[RW + pos] = c0 + tid;
+            if (tid < RW) {
+                spiv[2 * RW + tid] = (tid < wv && pos >= wv) ? c0 + pos : -1;
+                if (tid >= wv) spiv[RW + tid] = c0 + tid;          // positions of a ragged last panel that are no pivots
+            }
+        }
+    };
+    // ... -> global memory (off the critical path: after the panel has been shipped): pivot vector, status, and the rows
+    // of U held by this block for the verification export (k_backsolve_central reads U11, U12)
+    auto panel_export = [&](int p) {
+        const int c0 = p * RW, wv = min(RW, ne - c0), m = n - c0;
+        if (tid == 0) {
+#pragma unroll
+            for (int j = 0; j < RW; ++j) {
+                const int pp = ppos_all[j] < 0 ? -1 - ppos_all[j] : ppos_all[j];
+                if (j < wv) { pv[c0 + j] = c0 + pp; if (ppos_all[j] < 0) atomicCAS(inf, 0, c0 + j + 1); }
+            }
+        }
+        if (tid < m && pos < wv) {
+#pragma unroll
+            for (int c = 0; c < RW; ++c) if (c >= pos && c0 + c < n) A[(size_t)(c0 + pos) + (size_t)(c0 + c) * n] = v[c];
+        }
+    };
+    // ================= R3: panel p's interchanges + 8 x 8 unit-lower solve for the local columns [lc_lo, lc_hi) by the
+    // threads tbase .. tbase+nthr-1: EIGHT threads per column (same warp) apply the net permutation -- thread i reads
+    // the old and the new content of top position i, then the displaced rows are written -- and the first of them
+    // solves for the column's rows of U.
+    auto swap_solve = [&](int p, int lc_lo, int lc_hi, int tbase, int nthr) {
+        const int c0 = p * RW, wv = min(RW, ne - c0);
+        const int i = tid & 7;
+        const int top_src = spiv[RW + i], ddst = spiv[2 * RW + i];
+        const int ncols = lc_hi - lc_lo, rounds = (ncols * 8 + nthr - 1) / nthr;
+        for (int r = 0; r < rounds; ++r) {
+            const int lc = lc_lo + (r * nthr + (tid - tbase)) / 8;
+            const bool live = lc < lc_hi;
+            c128* col = Aloc + (size_t)(live ? lc : lc_lo) * ld;
+            const c128 a = col[c0 + i], b = col[top_src];
+            __syncwarp();
+            if (live && ddst >= 0) col[ddst] = a;
+            if (live) Ubuf[(size_t)lc * RS_LDU + i] = b;
+            __syncwarp();
+            if (live && i == 0) {
+                c128 x[RW];
+#pragma unroll
+                for (int q = 0; q < RW; ++q) x[q] = (q < wv) ? Ubuf[(size_t)lc * RS_LDU + q] : cmake(0.0, 0.0);
+#pragma unroll
+                for (int jq = 0; jq < RW; ++jq)
+#pragma unroll
+                    for (int q = jq + 1; q < RW; ++q)
+                        if (q < wv) cfms(x[q], Lbuf[(size_t)jq * ldp + q], x[jq]);
+                const int g = gcol(lc);
+#pragma unroll
+                for (int q = 0; q < RW; ++q) {
+                    Ubuf[(size_t)lc * RS_LDU + q] = x[q];
+                    if (q < wv && g < n) A[(size_t)(c0 + q) + (size_t)g * n] = x[q];
+                }
+            }
+        }
+    };
+    // ================= R4: rank-8 update of rows [c0+wv, n) x local columns [lc_lo, lc_hi) on DMMA, warp tiles of
+    // 32 x 8 dealt to the warps wbase .. wbase+nw-1
+    auto rank8_update = [&](int p, int lc_lo, int lc_hi, int wbase, int nw) {
+        const int c0 = p * RW, wv = min(RW, ne - c0);
+        const int r_lo = c0 + wv, mrows = n - r_lo;
+        const int tiles_m = (mrows + 31) / 32, tiles_n = (lc_hi - lc_lo) / RW;
+        const int gq = lane >> 2, q = lane & 3;
+        for (int tt = warp - wbase; tt < tiles_m * tiles_n; tt += nw) {
+            const int tm = tt % tiles_m, tn = tt / tiles_m;
+            const int r0 = r_lo + tm * 32, lc0 = lc_lo + tn * RW;
+            double cr[4][2], ci[4][2];
+            c128* Cb = Aloc + (size_t)(lc0 + 2 * q) * ld + r0 + gq;
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) { const c128 cv = Cb[(size_t)e * ld + mt * 8]; cr[mt][e] = cv.x; ci[mt][e] = cv.y; }
+#pragma unroll
+            for (int ks = 0; ks < RW / 4; ++ks) {
+                const c128 b = Ubuf[(size_t)(lc0 + gq) * RS_LDU + ks * 4 + q];
+                const double nbr = -b.x, nbi = -b.y;
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    const c128 a = Lbuf[(size_t)(ks * 4 + q) * ldp + (r0 - c0) + mt * 8 + gq];
+                    dmma884(cr[mt][0], cr[mt][1], a.x, nbr);
+                    dmma884(ci[mt][0], ci[mt][1], a.x, nbi);
+                    dmma884(cr[mt][0], cr[mt][1], a.y, b.y);
+                    dmma884(ci[mt][0], ci[mt][1], a.y, nbr);
+                }
+            }
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                for (int e = 0; e < 2; ++e)
+                    if (r0 + mt * 8 + gq < n) Cb[(size_t)e * ld + mt * 8] = cmake(cr[mt][e], ci[mt][e]);
+        }
+    };
+
+    if (np > 0 && rank == 0) panel_factor(0);            // the first panel has nothing to hide behind
+    for (int p = 0; p < np; ++p) {
+        const int m = n - p * RW;
+        const int owner = p % ncl;
+        if (rank == owner) {
+            panel_publish(p);
             asm volatile("fence.proxy.async;" ::: "memory");
             __syncthreads();
             R_TOC(1);
         } else if (tid == 0) {
-            mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * m * sizeof(c128) + RW * sizeof(int)));
+            mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * m * sizeof(c128) + 3 * RW * sizeof(int)));
         }
         // ================= R2: every CTA has finished the previous panel's update; ship the panel
         if (ncl > 1) {
@@ -270,75 +357,36 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
                     const uint32_t dst = (uint32_t)((d >= rank) ? d + 1 : d);
                     const uint32_t rbar = rs_mapa(smem_u32(bar_full), dst);
                     if (c < RW) rs_bulk_s2r(rs_mapa(smem_u32(Lbuf + (size_t)c * ldp), dst), smem_u32(Lbuf + (size_t)c * ldp), (uint32_t)(m * sizeof(c128)), rbar);
-                    else rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv), (uint32_t)(RW * sizeof(int)), rbar);
+                    else rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv), (uint32_t)(3 * RW * sizeof(int)), rbar);
                 }
             } else {
                 mbar_wait(bar_full, full_parity); full_parity ^= 1;
             }
         }
+        if (rank == owner) panel_export(p);
         R_TOC(2);
-        // ================= R3: interchanges + 8 x 8 unit-lower solve, one thread per trailing local column
         const int tl0 = (p >= rank) ? ((p - rank) / ncl + 1) * RW : 0;          // first local column right of block p
-        const int ntl = my_cols - tl0;
-        for (int lc = tl0 + tid; lc < my_cols; lc += RS_T) {
-            c128* col = Aloc + (size_t)lc * ld;
-            for (int i = 0; i < wv; ++i) {
-                const int pr = spiv[i];
-                if (pr != c0 + i) { const c128 a = col[c0 + i]; col[c0 + i] = col[pr]; col[pr] = a; }
+        if (p + 1 < np && (p + 1) % ncl == rank) {
+            // ---- LOOK-AHEAD: this CTA owns the next panel, whose factorisation is the critical path (8 dependent pivot
+            // steps).  Its block (local columns [tl0, tl0+8)) is brought up to date first by the whole CTA; then warps
+            // 0-7 factor it while warps 8-15 take panel p through the CTA's other columns.
+            swap_solve(p, tl0, tl0 + RW, 0, RS_T);
+            __syncthreads();
+            rank8_update(p, tl0, tl0 + RW, 0, RS_T / 32);
+            __syncthreads();
+            if (tid < RS_PT) panel_factor(p + 1);
+            else {
+                swap_solve(p, tl0 + RW, my_cols, RS_PT, RS_T - RS_PT);
+                asm volatile("bar.sync 2, %0;" ::"r"(RS_T - RS_PT) : "memory");
+                rank8_update(p, tl0 + RW, my_cols, RS_PT / 32, (RS_T - RS_PT) / 32);
             }
-            c128 x[RW];
-#pragma unroll
-            for (int i = 0; i < RW; ++i) x[i] = (i < wv) ? col[c0 + i] : cmake(0.0, 0.0);
-#pragma unroll
-            for (int jq = 0; jq < RW; ++jq)
-#pragma unroll
-                for (int i = jq + 1; i < RW; ++i)
-                    if (i < wv) cfms(x[i], Lbuf[(size_t)jq * ldp + i], x[jq]);
-            const int g = gcol(lc);
-#pragma unroll
-            for (int i = 0; i < RW; ++i) {
-                Ubuf[(size_t)lc * RS_LDU + i] = x[i];
-                if (i < wv && g < n) A[(size_t)(c0 + i) + (size_t)g * n] = x[i];
-            }
+        } else {
+            swap_solve(p, tl0, my_cols, 0, RS_T);
+            __syncthreads();
+            rank8_update(p, tl0, my_cols, 0, RS_T / 32);
         }
         __syncthreads();
         R_TOC(3);
-        // ================= R4: rank-8 update of rows [c0+wv, n) x trailing local columns on DMMA, warp tiles of 32 x 8
-        {
-            const int r_lo = c0 + wv, mrows = n - r_lo;
-            const int tiles_m = (mrows + 31) / 32, tiles_n = ntl / RW;
-            const int gq = lane >> 2, q = lane & 3;
-            for (int tt = warp; tt < tiles_m * tiles_n; tt += RS_T / 32) {
-                const int tm = tt % tiles_m, tn = tt / tiles_m;
-                const int r0 = r_lo + tm * 32, lc0 = tl0 + tn * RW;
-                double cr[4][2], ci[4][2];
-                c128* Cb = Aloc + (size_t)(lc0 + 2 * q) * ld + r0 + gq;
-#pragma unroll
-                for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) { const c128 cv = Cb[(size_t)e * ld + mt * 8]; cr[mt][e] = cv.x; ci[mt][e] = cv.y; }
-#pragma unroll
-                for (int ks = 0; ks < RW / 4; ++ks) {
-                    const c128 b = Ubuf[(size_t)(lc0 + gq) * RS_LDU + ks * 4 + q];
-                    const double nbr = -b.x, nbi = -b.y;
-#pragma unroll
-                    for (int mt = 0; mt < 4; ++mt) {
-                        const c128 a = Lbuf[(size_t)(ks * 4 + q) * ldp + (r0 - c0) + mt * 8 + gq];
-                        dmma884(cr[mt][0], cr[mt][1], a.x, nbr);
-                        dmma884(ci[mt][0], ci[mt][1], a.x, nbi);
-                        dmma884(cr[mt][0], cr[mt][1], a.y, b.y);
-                        dmma884(ci[mt][0], ci[mt][1], a.y, nbr);
-                    }
-                }
-#pragma unroll
-                for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e)
-                        if (r0 + mt * 8 + gq < n) Cb[(size_t)e * ld + mt * 8] = cmake(cr[mt][e], ci[mt][e]);
-            }
-        }
-        __syncthreads();
-        R_TOC(4);
     }
     // ================= K5: the trailing k x k block -> global memory, inverted by rank 0
     for (int e = tid; e < my_cols * k; e += RS_T) {
