@@ -342,8 +342,11 @@ class Bench:
         if schedule_used > 0:
             sm = prof["small_mode_lu"]
             ach = sm["flops"] / (sm["ms"] * 1e-3) / 1e12 if sm["ms"] > 0 else 0.0
-            roofline = {"kernel": f"k_lu_fused (small-matrix mode, {schedule_used} CTA(s) per matrix: whole elimination in one launch; "
-                                  "DMMA Schur updates inside)",
+            kname = (f"k_lu_resident (on-chip small-matrix mode: matrix in the distributed shared memory of a {schedule_used - 100}-CTA "
+                     "cluster, whole elimination in one launch; rank-8 DMMA updates from shared memory)" if schedule_used > 100 else
+                     f"k_lu_fused (small-matrix mode through L2, {schedule_used} CTA(s) per matrix: whole elimination in one launch; "
+                     "DMMA Schur updates inside)")
+            roofline = {"kernel": kname,
                         "achieved": ach, "frac": ach / peak_fp64 if peak_fp64 else None, "traffic": None,
                         "launches_per_step": sm["launches"], "avg_launch_ms": sm["ms"] / max(sm["launches"], 1),
                         "flops_per_launch_avg": sm["flops"] / max(sm["launches"], 1),
@@ -468,7 +471,8 @@ class Bench:
                                       f"{gathered} tau00 blocks gathered after the timed region"},
             "tflops": tflops, "tflops_convention": "8/3 n^3 per matrix",
             "frac_fp64_peak": tflops / peak_fp64 if peak_fp64 else None,
-            "schedule": {"mode": ("small-matrix mode, %d CTA(s) per matrix, one launch" % schedule_used) if schedule_used > 0
+            "schedule": {"mode": ("on-chip small-matrix mode, cluster of %d CTA(s) (SMs) per matrix, one launch" % (schedule_used - 100)) if schedule_used > 100
+                         else ("small-matrix mode through L2, %d CTA(s) per matrix, one launch" % schedule_used) if schedule_used > 0
                          else "lock-step over the batch", "groups": args.groups or "auto", "lookahead": not args.no_lookahead,
                          "panel_threads": args.panel, "nb": args.nb or 64, "ib": args.ib or 16, "align_first_panel": not args.no_align,
                          "assembly": "one g0 per energy shared by all atoms (f3)" if shared_g0 else "every item assembled independently"},

@@ -320,22 +320,25 @@ static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
     if (sm == 1) return 0;
     const int rcl = resident_cluster_size(n, k);
     if (sm == 7) return rcl > 0 ? -rcl : 0;
-    if (sm == 0 && rcl > 0) return -rcl;            // default for matrices that fit on chip (n <= ~216 with 4 SMs each)
+    // Default for matrices that fit on chip (n <= ~216 with 4 SMs each), while the batch needs at most ~3.5 waves of
+    // clusters: the on-chip kernel is built for latency (208^2 x 32: 0.25 ms against 0.56 ms through L2 and 0.85 ms in
+    // lock-step), but it holds 4 SMs per matrix for the whole elimination, and from ~150 matrices of 208^2 on the
+    // lock-step schedule has the higher throughput (1024 matrices: 3.5 ms against 6.4 ms on chip).
+    if (sm == 0 && rcl > 0 && 2LL * batch * rcl <= 7LL * c->sms) return -rcl;
+    if (sm == 0) return 0;
     if (!fused_supported(n, k, eff_nb(c), eff_ib(c))) return 0;
     if (sm >= 3) return 1 << (sm - 3);
-    // CTAs per matrix: a CTA is a quarter of an SM, so few matrices get a cluster each until the chip is covered.
-    // Tiny matrices: at most 4 -- their panel chain is serial, rank 0 factors under the other ranks' updates, and a
-    // third to seventh helper only adds barrier traffic (208^2 x 32: 0.56 ms with 4 CTAs per matrix, 0.61 with 8).
+    // sm == 2: the one-launch mode through L2 (fused.cu).  CTAs per matrix: a CTA is a quarter of an SM, so few matrices
+    // get a cluster each until the chip is covered.  Tiny matrices: at most 4 -- their panel chain is serial, rank 0
+    // factors under the other ranks' updates, and a third to seventh helper only adds barrier traffic (208^2 x 32:
+    // 0.56 ms with 4 CTAs per matrix, 0.61 with 8).  Measured against the other schedules it never wins by default:
+    // 208^2 x 32: 0.56 ms (on chip 0.25); 208^2 x 1024: 4.1 ms (lock-step 3.5); 880^2 x 512: 55 ms (lock-step 39: its
+    // per-matrix latency phases run with 128 threads and do not overlap the other matrices' updates as hoped).
     const long long slots = 4LL * c->sms;
     const int cl_max = fused_is_tiny(n) ? 4 : 8;
     int cl = 1;
     while (cl < cl_max && (long long)batch * cl * 2 <= slots) cl *= 2;
-    if (sm == 2) return cl;
-    // Default (measured): the one-launch modes win where the lock-step schedule is launch- and
-    // latency-bound -- matrices of a few hundred rows.  For mid-size matrices (configs[1], 880^2 x 512) the general
-    // one-launch kernel is correct but slower than lock-step (55 vs 39 ms: its per-matrix latency phases run with 128
-    // threads and do not overlap the other matrices' updates as hoped), so it is used only on request.
-    return fused_is_tiny(n) ? cl : 0;
+    return cl;
 }
 
 static int tau00_impl(Ctx* c, c128* M, int n, int k, int batch, c128* tau, int* info, void* workspace, cudaStream_t st) {

@@ -64,16 +64,21 @@ __host__ __device__ inline ResLayout res_layout(int n, int ncl) {
 
 #ifdef LSMS_RES_TIMING
 // working aid (not compiled by default): per-phase cycles of thread 0 of CTA 0
-__device__ unsigned long long g_res_cyc[16];
+__device__ unsigned long long g_res_cyc[32];
+__device__ unsigned long long g_res_tl[64 * 8];
+__device__ __forceinline__ unsigned long long rs_gt() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define R_STAMP(p, i) do { if (threadIdx.x == 0 && blockIdx.x < 4 && (p) < 64) g_res_tl[(p) * 8 + (i)] = rs_gt(); } while (0)
 #define R_TIC() long long t__ = clock64()
-#define R_TOC(i) do { if (threadIdx.x == 0 && blockIdx.x == 0) { long long n__ = clock64(); atomicAdd(&g_res_cyc[i], (unsigned long long)(n__ - t__)); t__ = clock64(); } } while (0)
+#define R_TOC(i) do { if (threadIdx.x == 0 && blockIdx.x < 4) { long long n__ = clock64(); atomicAdd(&g_res_cyc[blockIdx.x * 8 + ((i) & 7)], (unsigned long long)(n__ - t__)); t__ = clock64(); } } while (0)
+extern "C" int lsms_work_res_timeline(unsigned long long* out_host) { cudaMemcpyFromSymbol(out_host, g_res_tl, sizeof(unsigned long long) * 64 * 8); return 0; }
 extern "C" int lsms_work_res_cycles(unsigned long long* out_host, int reset) {
-    if (out_host) cudaMemcpyFromSymbol(out_host, g_res_cyc, sizeof(unsigned long long) * 16);
-    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_res_cyc, z, sizeof(z)); }
+    if (out_host) cudaMemcpyFromSymbol(out_host, g_res_cyc, sizeof(unsigned long long) * 32);
+    if (reset) { unsigned long long z[32] = {0}; cudaMemcpyToSymbol(g_res_cyc, z, sizeof(z)); }
     return 0;
 }
 #else
 #define R_TIC() do {} while (0)
+#define R_STAMP(p, i) do {} while (0)
 #define R_TOC(i) do {} while (0)
 #endif
 
@@ -342,9 +347,10 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
         const int owner = p % ncl;
         if (rank == owner) {
             panel_publish(p);
-            asm volatile("fence.proxy.async;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncthreads();
             R_TOC(1);
+            R_STAMP(p, 0);
         } else if (tid == 0) {
             mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * m * sizeof(c128) + 3 * RW * sizeof(int)));
         }
@@ -352,34 +358,46 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
         if (ncl > 1) {
             rs_cluster_sync();
             if (rank == owner) {
-                if (tid < (ncl - 1) * (RW + 1)) {
-                    const int d = tid / (RW + 1), c = tid % (RW + 1);
-                    const uint32_t dst = (uint32_t)((d >= rank) ? d + 1 : d);
-                    const uint32_t rbar = rs_mapa(smem_u32(bar_full), dst);
-                    if (c < RW) rs_bulk_s2r(rs_mapa(smem_u32(Lbuf + (size_t)c * ldp), dst), smem_u32(Lbuf + (size_t)c * ldp), (uint32_t)(m * sizeof(c128)), rbar);
-                    else rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv), (uint32_t)(3 * RW * sizeof(int)), rbar);
+                // the CTA that owns the NEXT panel is served first: its step is the critical path
+                if (tid < RW + 1) {
+                    const int c = tid;
+                    for (int d = 1; d < ncl; ++d) {
+                        const uint32_t dst = (uint32_t)((rank + d) % ncl);
+                        const uint32_t rbar = rs_mapa(smem_u32(bar_full), dst);
+                        if (c < RW) rs_bulk_s2r(rs_mapa(smem_u32(Lbuf + (size_t)c * ldp), dst), smem_u32(Lbuf + (size_t)c * ldp), (uint32_t)(m * sizeof(c128)), rbar);
+                        else rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv), (uint32_t)(3 * RW * sizeof(int)), rbar);
+                    }
                 }
             } else {
                 mbar_wait(bar_full, full_parity); full_parity ^= 1;
+                if ((p + 1) % ncl == rank) R_STAMP(p, 2);
             }
+            if (rank == owner) R_STAMP(p, 1);
         }
         if (rank == owner) panel_export(p);
         R_TOC(2);
         const int tl0 = (p >= rank) ? ((p - rank) / ncl + 1) * RW : 0;          // first local column right of block p
         if (p + 1 < np && (p + 1) % ncl == rank) {
             // ---- LOOK-AHEAD: this CTA owns the next panel, whose factorisation is the critical path (8 dependent pivot
-            // steps).  Its block (local columns [tl0, tl0+8)) is brought up to date first by the whole CTA; then warps
-            // 0-7 factor it while warps 8-15 take panel p through the CTA's other columns.
-            swap_solve(p, tl0, tl0 + RW, 0, RS_T);
-            __syncthreads();
-            rank8_update(p, tl0, tl0 + RW, 0, RS_T / 32);
-            __syncthreads();
-            if (tid < RS_PT) panel_factor(p + 1);
-            else {
+            // steps).  Warps 0-7 bring its block (local columns [tl0, tl0+8)) up to date and factor it while warps 8-15
+            // take panel p through the CTA's other columns.
+            if (tid < RS_PT) {
+                swap_solve(p, tl0, tl0 + RW, 0, RS_PT);
+                asm volatile("bar.sync 3, %0;" ::"r"(RS_PT) : "memory");
+                rank8_update(p, tl0, tl0 + RW, 0, RS_PT / 32);
+                asm volatile("bar.sync 3, %0;" ::"r"(RS_PT) : "memory");
+                R_TOC(4);
+                R_STAMP(p, 3);
+                panel_factor(p + 1);
+                R_STAMP(p, 4);
+            } else {
                 swap_solve(p, tl0 + RW, my_cols, RS_PT, RS_T - RS_PT);
                 asm volatile("bar.sync 2, %0;" ::"r"(RS_T - RS_PT) : "memory");
                 rank8_update(p, tl0 + RW, my_cols, RS_PT / 32, (RS_T - RS_PT) / 32);
             }
+            R_TOC(5);
+            __syncthreads();
+            R_TOC(6);
         } else {
             swap_solve(p, tl0, my_cols, 0, RS_T);
             __syncthreads();
@@ -399,7 +417,7 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
         if (k * k <= 4 * RS_T) final_inverse_small<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, reinterpret_cast<int*>(rsm));
         else final_inverse_body<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, *reinterpret_cast<K5Shared*>(rsm));
     }
-    R_TOC(5);
+    R_TOC(0);
     if (ncl > 1) rs_cluster_sync();             // no CTA leaves while its shared memory may still be a copy target
 }
 
