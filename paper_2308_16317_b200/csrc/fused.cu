@@ -142,7 +142,7 @@ __device__ __forceinline__ void panel_smem(c128* __restrict__ A, int n, int c0, 
         if (!bad) {
             // every thread updates its rows; the columns are taken four at a time so that four independent
             // load -> fma -> store chains are in flight (a one-column-at-a-time loop is bound by shared-memory latency)
-            const c128 rp = crecip(P[q * m + q]);
+            const c128 rp = crecip_fast(P[q * m + q]);
             for (int r = q + 1 + tid; r < m; r += FT) {
                 const c128 l = cmul(P[q * m + r], rp);
                 P[q * m + r] = l;

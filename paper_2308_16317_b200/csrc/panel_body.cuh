@@ -26,17 +26,28 @@
 
 namespace lsms {
 
+#ifdef LSMS_PANEL_TIMING
+// working aid (not compiled by default): per-phase cycles of thread 0 of CTA 0 of k_panel_reg
+static __device__ unsigned long long g_panel_cyc[8];
+#define P_TIC() long long pt__ = clock64()
+#define P_TOC(i) do { if (threadIdx.x == 0 && blockIdx.x == 0) { long long n__ = clock64(); atomicAdd(&g_panel_cyc[i], (unsigned long long)(n__ - pt__)); pt__ = clock64(); } } while (0)
+#else
+#define P_TIC() do {} while (0)
+#define P_TOC(i) do {} while (0)
+#endif
+
 constexpr int P2_MAXW = 16;       // inner panel width limit
 constexpr int P2_MAXOUT = 128;    // outer panel width limit (column threads of step 4)
 
 // Shared-memory state of one panel factorisation (sized for the widest sub-panel, S = 4, and 16 warps).
 struct PanelShared {
-    c128 prow[4], jrow[4];
+    // column-step exchange, double-buffered by the parity of the column: per warp the arg-max candidate's row (S
+    // entries), the reciprocal of its would-be pivot and the arg-max key; the row that stands at the pivot position
+    c128 cand[2][16][4 + 2];
+    c128 jrow[2][4];
     c128 L11[4 * 4];                 // L11[i*S + q] = multiplier of row cs+i, column cs+q (q < i)
     c128 Us[4 * P2_MAXW];            // Us[q*P2_MAXW + c] = U(cs+q, cs+sw+c)
     c128 Lw[P2_MAXW * P2_MAXW];      // step 6: the w x w unit-lower triangle
-    double red_v[16];
-    int red_i[16];
     int spiv[4], canon[4];
 };
 
@@ -49,12 +60,12 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
                                            int* __restrict__ pv, int* __restrict__ info, PanelShared& sh) {
     constexpr int NW = THREADS / 32;
     static_assert(S <= 4 && NW <= 16, "PanelShared is sized for S <= 4 and <= 16 warps");
-    double* red_v = sh.red_v; int* red_i = sh.red_i;
-    c128* prow = sh.prow; c128* jrow = sh.jrow; c128* L11 = sh.L11; c128* Us = sh.Us;
+    c128* L11 = sh.L11; c128* Us = sh.Us;
     int* spiv = sh.spiv; int* canon = sh.canon;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const c128 zero = cmake(0.0, 0.0);
 
+    P_TIC();
     for (int s0 = 0; s0 < w; s0 += S) {
         const int cs = c0 + s0, sw = min(S, w - s0);
         // ---- 1: sub-panel -> registers
@@ -65,71 +76,90 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
 #pragma unroll
             for (int q = 0; q < S; ++q) v[r][q] = (row < n && q < sw) ? A[row + (size_t)(cs + q) * n] : zero;
         }
-        // ---- 2: column steps
+        P_TOC(0);
+        // ---- 2: column steps, ONE CTA barrier each.  Arg-max key of a row: the bits of |re|+|im| with the low 18
+        // mantissa bits replaced by (16383 - (row - c0), warp), so that one unsigned 64-bit maximum picks the largest
+        // magnitude and, among (nearly) equal ones, the lowest row (LAPACK's izamax up to 2^-34); 0 = not eligible.  Every warp
+        // finds its candidate with two redux.sync and publishes the candidate's row TOGETHER with the key (and with
+        // the reciprocal of the would-be pivot, computed under the reduction), the owner of row j publishes that row:
+        // when the barrier opens every thread has what it needs for the interchange and the rank-1 update.
+        int piv_reg[S];
 #pragma unroll
         for (int q = 0; q < S; ++q) {
+            piv_reg[q] = cs + q;
             if (q < sw) {
-                const int j = cs + q;
-                double bv = -1.0; int bi = 0x7fffffff;
+                const int j = cs + q, par = q & 1;
+                unsigned long long key = 0ull; int rb = 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const int row = c0 + tid + r * THREADS;
-                    const double a = cabs1(v[r][q]);
-                    if (row >= j && row < ne && a > bv) { bv = a; bi = row; }
-                }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-                    const double ov = __shfl_xor_sync(0xffffffffu, bv, o); const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-                }
-                if (lane == 0) { red_v[warp] = bv; red_i[warp] = bi; }
-                __syncthreads();
-                bv = red_v[lane % NW]; bi = red_i[lane % NW];
-#pragma unroll
-                for (int o = NW / 2; o > 0; o >>= 1) {
-                    const double ov = __shfl_xor_sync(0xffffffffu, bv, o); const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-                }
-                const bool bad = !(bv > 0.0) || !(bv < 1.0e300 * 1.0e300);     // zero, NaN or Inf pivot
-                const int p = bad ? j : bi;
-                if (tid == 0) { spiv[q] = p; pv[j] = p; if (bad) atomicCAS(info, 0, j + 1); }
-                // ---- pivot row and row j through shared memory
-                const int tj = (j - c0) % THREADS, rj = (j - c0) / THREADS;
-                const int tp = (p - c0) % THREADS, rp_ = (p - c0) / THREADS;
-                if (tid == tp) {
-#pragma unroll
-                    for (int r = 0; r < R; ++r) if (r == rp_) {
-#pragma unroll
-                        for (int t = 0; t < S; ++t) prow[t] = v[r][t];
+                    if (row >= j && row < ne) {
+                        const unsigned long long kk = ((unsigned long long)__double_as_longlong(cabs1(v[r][q])) & ~0x3FFFFull) |
+                                                      ((unsigned long long)(16383 - (row - c0)) << 4) | (unsigned long long)warp;
+                        if (kk > key) { key = kk; rb = r; }
                     }
                 }
-                if (p != j && tid == tj) {
+                c128 cr_[S];
+#pragma unroll
+                for (int t = 0; t < S; ++t) cr_[t] = v[0][t];
+#pragma unroll
+                for (int r = 1; r < R; ++r) if (r == rb) {
+#pragma unroll
+                    for (int t = 0; t < S; ++t) cr_[t] = v[r][t];
+                }
+                const c128 rinv = crecip_fast(cr_[q]);
+                const uint32_t khi = (uint32_t)(key >> 32), klo = (uint32_t)key;
+                const uint32_t mhi = __reduce_max_sync(0xffffffffu, khi);
+                const uint32_t mlo = __reduce_max_sync(0xffffffffu, (khi == mhi) ? klo : 0u);
+                c128* slot = sh.cand[par][warp];
+                if (key != 0ull && khi == mhi && klo == mlo) {
+#pragma unroll
+                    for (int t = 0; t < S; ++t) slot[t] = cr_[t];
+                    slot[4] = rinv;
+                }
+                if (lane == 0) reinterpret_cast<unsigned long long*>(slot + 5)[0] = ((unsigned long long)mhi << 32) | mlo;
+                const int tj = (j - c0) % THREADS, rj = (j - c0) / THREADS;
+                if (tid == tj) {
 #pragma unroll
                     for (int r = 0; r < R; ++r) if (r == rj) {
 #pragma unroll
-                        for (int t = 0; t < S; ++t) jrow[t] = v[r][t];
+                        for (int t = 0; t < S; ++t) sh.jrow[par][t] = v[r][t];
                     }
                 }
                 __syncthreads();
-                if (p != j) {
-                    if (tid == tj) {
-#pragma unroll
-                        for (int r = 0; r < R; ++r) if (r == rj) {
-#pragma unroll
-                            for (int t = 0; t < S; ++t) v[r][t] = prow[t];
-                        }
-                    }
-                    if (tid == tp) {
-#pragma unroll
-                        for (int r = 0; r < R; ++r) if (r == rp_) {
-#pragma unroll
-                            for (int t = 0; t < S; ++t) v[r][t] = jrow[t];
-                        }
-                    }
-                }
-                // ---- scale column j and rank-1 update of the sub-panel's remaining columns
+                // winner among the NW warp candidates: lane l takes candidate l mod NW, two more redux.sync
+                const unsigned long long ck = reinterpret_cast<const unsigned long long*>(&sh.cand[par][lane % NW][5])[0];
+                const uint32_t chi = (uint32_t)(ck >> 32), clo = (uint32_t)ck;
+                const uint32_t whi = __reduce_max_sync(0xffffffffu, chi);
+                const uint32_t wlo = __reduce_max_sync(0xffffffffu, (chi == whi) ? clo : 0u);
+                const unsigned long long wkey = ((unsigned long long)whi << 32) | wlo;
+                const int wsel = (int)(wkey & 15ull);
+                const bool bad = (wkey >> 18) == 0ull || (uint32_t)(wkey >> 52) >= 0x7FFu;     // zero, NaN or Inf pivot
+                const int p = bad ? j : c0 + 16383 - (int)((wkey >> 4) & 0x3FFFull);
+                piv_reg[q] = bad ? -1 - j : p;
                 if (!bad) {
-                    const c128 rp = crecip(prow[q]);
+                    c128 prow[S];
+#pragma unroll
+                    for (int t = 0; t < S; ++t) prow[t] = sh.cand[par][wsel][t];
+                    const c128 rp = sh.cand[par][wsel][4];
+                    const int tp = (p - c0) % THREADS, rp_ = (p - c0) / THREADS;
+                    if (p != j) {
+                        if (tid == tp) {
+#pragma unroll
+                            for (int r = 0; r < R; ++r) if (r == rp_) {
+#pragma unroll
+                                for (int t = 0; t < S; ++t) v[r][t] = sh.jrow[par][t];
+                            }
+                        }
+                        if (tid == tj) {
+#pragma unroll
+                            for (int r = 0; r < R; ++r) if (r == rj) {
+#pragma unroll
+                                for (int t = 0; t < S; ++t) v[r][t] = prow[t];
+                            }
+                        }
+                    }
+                    // ---- scale column j and rank-1 update of the sub-panel's remaining columns
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
                         const int row = c0 + tid + r * THREADS;
@@ -143,6 +173,7 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
                 }
             }
         }
+        P_TOC(1);
         // ---- 3: store the sub-panel (rows above cs hold finished U entries and are unchanged), publish L11
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -157,6 +188,14 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             }
         }
         if (tid == 0) {
+#pragma unroll
+            for (int q = 0; q < S; ++q) {
+                if (q < sw) {
+                    const int pq = piv_reg[q] < 0 ? -1 - piv_reg[q] : piv_reg[q];
+                    spiv[q] = pq; pv[cs + q] = pq;
+                    if (piv_reg[q] < 0) atomicCAS(info, 0, cs + q + 1);
+                }
+            }
             // canon[i] = first step whose pivot row equals that of step i (rows below the sub-panel only)
             for (int i = 0; i < sw; ++i) {
                 int c = -1;
@@ -165,6 +204,7 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             }
         }
         __syncthreads();
+        P_TOC(2);
         // ---- 4: the other columns of the outer panel: interchanges (+ S x S solve for the inner panel's right part)
         const int nright = (c0 + w) - (cs + sw);          // inner-panel columns still to be updated
         if (tid < Wout) {
@@ -214,6 +254,7 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             }
         }
         __syncthreads();
+        P_TOC(3);
         // ---- 5: rank-sw update of the inner panel's remaining columns (rows below the sub-panel).
         // Software-pipelined over (column, row chunk): the loads of the next chunk are issued before the
         // current chunk is updated and stored, so that one L2 round trip is always in flight.
@@ -252,6 +293,7 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             }
         }
         __syncthreads();
+        P_TOC(4);
     }
     // ---- 6: U12 of the outer panel's columns to the RIGHT of this inner panel: solve the w x w unit-lower L11
     // against rows [c0, c0+w) of each such column (their interchanges were applied in step 4).  One thread per
@@ -275,6 +317,7 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             for (int i = 0; i < P2_MAXW; ++i) if (i < w) col[i] = x[i];
         }
     }
+    P_TOC(5);
 }
 
 }  // namespace lsms

@@ -148,7 +148,7 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
                 }
                 // ---- scale column j and rank-1 update of the sub-panel's remaining columns
                 if (!bad) {
-                    const c128 rp = crecip(prow[q]);
+                    const c128 rp = crecip_fast(prow[q]);
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
                         const int row = c0 + g0 + r * TT;
