@@ -44,7 +44,7 @@ static int bind_device(Ctx* c, int dev) {
     LSMS_CUDA_OK(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
     int rc;
     if ((rc = init_attrs_gemm()) || (rc = init_attrs_lu()) || (rc = init_attrs_assemble()) || (rc = init_attrs_fused()) ||
-        (rc = init_attrs_resident())) return rc;
+        (rc = init_attrs_resident()) || (rc = init_attrs_panel())) return rc;
     int lo = 0, hi = 0;
     LSMS_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
     LSMS_CUDA_OK(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
@@ -412,7 +412,8 @@ int lsms_set_option(lsms_handle_t c, int option, int value) {
         case LSMS_OPT_NB_OUTER: ok = value >= 0 && value <= 96 && value % 4 == 0; break;
         case LSMS_OPT_IB_INNER: ok = value >= 0 && value <= 16; break;
         case LSMS_OPT_LOOKAHEAD: ok = value >= 0 && value <= 2; break;
-        case LSMS_OPT_PANEL_THREADS: case LSMS_OPT_ALIGN_FIRST: ok = value == 0 || value == 1; break;
+        case LSMS_OPT_PANEL_THREADS: ok = value >= 0 && value <= 2; break;
+        case LSMS_OPT_ALIGN_FIRST: ok = value == 0 || value == 1; break;
         case LSMS_OPT_GROUPS: ok = value >= 0 && value <= MAX_GROUPS; break;
         case LSMS_OPT_PANEL_CLUSTER: ok = value == 0 || value == 1 || value == 2 || value == 4 || value == 8; break;
         case LSMS_OPT_SMALL_MODE: ok = value >= 0 && value <= 7; break;

@@ -50,6 +50,7 @@ int init_attrs_lu();
 int init_attrs_assemble();
 int init_attrs_fused();
 int init_attrs_resident();
+int init_attrs_panel();
 
 // assemble.cu
 size_t gaunt_table_bytes(int lmax);

@@ -55,9 +55,18 @@ struct PanelShared {
 // applies its interchanges / triangular solves to the outer panel [J, J+Wout).  pv = the matrix's pivot vector,
 // info = the matrix's status word.  Callers: k_panel_reg (one CTA per matrix, lock-step schedule) and the
 // small-matrix kernel of fused.cu.  Ends with the CTA's threads NOT synchronised (global stores may be pending).
-template <int THREADS, int R, int S>
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src_gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// DEPTH > 0: step 5 streams the columns it updates through `stage` (DEPTH slots of R*THREADS complex numbers of shared
+// memory) with per-thread asynchronous copies, DEPTH columns ahead -- the step is bound by the bytes a CTA keeps in
+// flight towards L2/HBM, and registers hold one column only.  DEPTH = 0: the register-pipelined loop (one column ahead).
+template <int THREADS, int R, int S, int DEPTH = 0>
 __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, int Wout, int c0, int w, int ne,
-                                           int* __restrict__ pv, int* __restrict__ info, PanelShared& sh) {
+                                           int* __restrict__ pv, int* __restrict__ info, PanelShared& sh, c128* stage = nullptr) {
     constexpr int NW = THREADS / 32;
     static_assert(S <= 4 && NW <= 16, "PanelShared is sized for S <= 4 and <= 16 warps");
     c128* L11 = sh.L11; c128* Us = sh.Us;
@@ -258,7 +267,42 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
         // ---- 5: rank-sw update of the inner panel's remaining columns (rows below the sub-panel).
         // Software-pipelined over (column, row chunk): the loads of the next chunk are issued before the
         // current chunk is updated and stored, so that one L2 round trip is always in flight.
-        if (nright > 0) {
+        if (nright > 0 && DEPTH > 0) {
+            // every thread copies, updates and stores its own rows only: no barrier inside the loop; a slot is refilled
+            // after the stores that consumed it have been issued
+            auto issue = [&](int c) {
+                if (c < nright) {
+                    c128* dst = stage + (size_t)(c % (DEPTH > 0 ? DEPTH : 1)) * (R * THREADS) + tid;
+                    const c128* src = A + (size_t)(cs + sw + c) * n + c0 + tid;
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const int row = c0 + tid + r * THREADS;
+                        if (row >= cs + sw && row < n) cp_async16(dst + r * THREADS, src + r * THREADS);
+                    }
+                }
+                cp_async_commit();
+            };
+            for (int d = 0; d < DEPTH; ++d) issue(d);
+            for (int c = 0; c < nright; ++c) {
+                cp_async_wait<(DEPTH > 0 ? DEPTH - 1 : 0)>();
+                const c128* src = stage + (size_t)(c % (DEPTH > 0 ? DEPTH : 1)) * (R * THREADS) + tid;
+                c128 u[S];
+#pragma unroll
+                for (int q = 0; q < S; ++q) u[q] = (q < sw) ? Us[q * P2_MAXW + c] : zero;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int row = c0 + tid + r * THREADS;
+                    if (row >= cs + sw && row < n) {
+                        c128 x = src[r * THREADS];
+#pragma unroll
+                        for (int q = 0; q < S; ++q) if (q < sw) cfms(x, v[r][q], u[q]);
+                        A[row + (size_t)(cs + sw + c) * n] = x;
+                    }
+                }
+                issue(c + DEPTH);
+            }
+            cp_async_wait<0>();
+        } else if (nright > 0) {
             constexpr int RC = (R % 5 == 0) ? 5 : ((R % 4 == 0) ? 4 : R);      // rows per chunk (R in {1,2,5,10,20,32})
             constexpr int NCH = R / RC;
             c128 cur[RC], nxt[RC];
