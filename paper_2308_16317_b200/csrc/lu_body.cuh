@@ -118,27 +118,37 @@ __device__ __forceinline__ void final_inverse_body(const c128* __restrict__ A, i
     for (int e = tid; e < k * k; e += THREADS) out[e] = S[e];
 }
 
-// K5 for a SMALL block (k*k <= 4*THREADS, e.g. k = 16 or 32 with 512 threads), trimmed for latency: one thread per
-// element (up to four), every thread finds the pivot of column j for itself (k broadcast reads, no exchange), the new
-// value of each element is computed from the OLD matrix, then written: two CTA barriers per elimination step instead
-// of six plus a serial section.  Same in-place Gauss-Jordan arithmetic and pivot rule as final_inverse_body.
+// K5 for a SMALL block (k <= 32, k*k <= 4*THREADS), trimmed for latency: one thread per element (up to four); every WARP
+// finds the pivot of column j for itself (lane i takes row i: two redux.sync on a 64-bit key, the reciprocal of every
+// candidate computed under the reduction and fetched from the winner by shuffles), the new value of each element is
+// computed from the OLD matrix, then written: two CTA barriers per elimination step instead of six plus a serial
+// section.  Same in-place Gauss-Jordan arithmetic as final_inverse_body; pivot = largest |re|+|im| (ties, up to 2^-47,
+// to the lowest row).
 template <int THREADS>
 __device__ __forceinline__ void final_inverse_small(const c128* __restrict__ A, int n, int k, c128* __restrict__ out,
                                                     int* __restrict__ info, c128* S, int* cpiv) {
-    const int ne = n - k, tid = threadIdx.x, kk = k * k;
+    const int ne = n - k, tid = threadIdx.x, lane = tid & 31, kk = k * k;
     for (int e = tid; e < kk; e += THREADS) { const int r = e % k, c = e / k; S[e] = A[(ne + r) + (size_t)(ne + c) * n]; }
     __syncthreads();
     bool failed = false;
     for (int j = 0; j < k; ++j) {
-        double bv = -1.0; int p = j;
-        for (int i = j; i < k; ++i) { const double a = cabs1(S[i + j * k]); if (a > bv) { bv = a; p = i; } }
-        if (!(bv > 0.0) || !(bv < 1.0e300 * 1.0e300)) {            // the same for every thread
+        const bool elig = lane >= j && lane < k;
+        const c128 cand = elig ? S[lane + j * k] : cmake(0.0, 0.0);
+        const c128 rinv = crecip_fast(cand);
+        const unsigned long long kb = elig ? ((((unsigned long long)__double_as_longlong(cabs1(cand))) & ~31ull) | (unsigned long long)(31 - lane)) : 0ull;
+        const uint32_t khi = (uint32_t)(kb >> 32), klo = (uint32_t)kb;
+        const uint32_t mhi = __reduce_max_sync(0xffffffffu, khi);
+        const uint32_t mlo = __reduce_max_sync(0xffffffffu, (khi == mhi) ? klo : 0u);
+        const unsigned long long wkey = ((unsigned long long)mhi << 32) | mlo;
+        if ((wkey >> 5) == 0ull || (uint32_t)(wkey >> 52) >= 0x7FFu) {       // zero, NaN or Inf pivot; the same in every thread
             if (tid == 0) atomicCAS(info, 0, ne + j + 1);
             failed = true;
             break;
         }
+        const int p = 31 - (int)(wkey & 31ull);
+        c128 rp;
+        rp.x = __shfl_sync(0xffffffffu, rinv.x, p); rp.y = __shfl_sync(0xffffffffu, rinv.y, p);
         if (tid == 0) cpiv[j] = p;
-        const c128 rp = crecip_fast(S[p + j * k]);
         c128 nv[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {

@@ -414,7 +414,7 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
     if (ncl > 1) { __threadfence(); rs_cluster_sync(); } else __syncthreads();
     if (rank == 0) {
         c128* S = reinterpret_cast<c128*>(rsm + 8192);
-        if (k * k <= 4 * RS_T) final_inverse_small<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, reinterpret_cast<int*>(rsm));
+        if (k <= 32 && k * k <= 4 * RS_T) final_inverse_small<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, reinterpret_cast<int*>(rsm));
         else final_inverse_body<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, *reinterpret_cast<K5Shared*>(rsm));
     }
     R_TOC(0);
