@@ -44,7 +44,8 @@ static int bind_device(Ctx* c, int dev) {
     LSMS_CUDA_OK(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
     int rc;
     if ((rc = init_attrs_gemm()) || (rc = init_attrs_lu()) || (rc = init_attrs_assemble()) || (rc = init_attrs_fused()) ||
-        (rc = init_attrs_resident()) || (rc = init_attrs_panel())) return rc;
+        (rc = init_attrs_resident()) || (rc = init_attrs_panel()) ||
+        (rc = init_attrs_panel_cluster())) return rc;
     int lo = 0, hi = 0;
     LSMS_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
     LSMS_CUDA_OK(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));

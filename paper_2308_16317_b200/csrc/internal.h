@@ -51,6 +51,7 @@ int init_attrs_assemble();
 int init_attrs_fused();
 int init_attrs_resident();
 int init_attrs_panel();
+int init_attrs_panel_cluster();
 
 // assemble.cu
 size_t gaunt_table_bytes(int lmax);

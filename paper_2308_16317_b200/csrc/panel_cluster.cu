@@ -7,14 +7,17 @@
 // rows c0 + g + r*CL*THREADS), so the sub-panel stays 4 columns wide and CL times as many SMs pull the panel
 // through their load/store units.  Same algorithm and arithmetic as k_panel_reg; what crosses CTAs goes through
 // distributed shared memory, every CTA keeping a full copy of the small shared state:
-//   * arg-max: each warp writes its candidate into slot [rank][warp] of EVERY CTA, one cluster barrier, then every
-//     thread reduces the CL*NW candidates itself (same result everywhere, no broadcast step);
-//   * pivot row / row j, L11, the rows of U: written by their owner into every CTA's copy;
+//   * column step: each warp finds its arg-max candidate (two redux.sync on a 64-bit key, as in panel_body.cuh) and
+//     writes the candidate's ROW, the reciprocal of its would-be pivot and the key into slot [rank][warp] of EVERY
+//     CTA; the owner of row j writes that row into every CTA; ONE cluster barrier; then every thread reduces the
+//     CL*NW keys itself (same result everywhere) and has the pivot row in its own shared memory;
+//   * L11, the rows of U: written by their owner into every CTA's copy;
 //   * the interchanges of the outer panel's other columns and the final w x w solve are done by rank 0.
-// Barriers per column step: two cluster barriers (arrive.release / wait.acquire, which also order the global-memory
-// traffic between the CTAs of the cluster).
+// Cluster barriers (arrive.release / wait.acquire, which also order the global-memory traffic between the CTAs of the
+// cluster): one per column step, three more per sub-panel.
 #include "common.cuh"
 #include "internal.h"
+#include "panel_body.cuh"
 
 namespace lsms {
 
@@ -35,23 +38,27 @@ __device__ __forceinline__ uint32_t pc_map(const void* p, uint32_t rank) {
 __device__ __forceinline__ void pc_st_c128(uint32_t addr, c128 v) {
     asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
 }
+__device__ __forceinline__ void pc_st_u64(uint32_t addr, unsigned long long v) { asm volatile("st.shared::cluster.u64 [%0], %1;" ::"r"(addr), "l"(v) : "memory"); }
 __device__ __forceinline__ void pc_st_f64(uint32_t addr, double v) { asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
 __device__ __forceinline__ void pc_st_s32(uint32_t addr, int v) { asm volatile("st.shared::cluster.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
 // store v into the copy of *p held by every CTA of the cluster (including this one)
 __device__ __forceinline__ void pc_bcast_c128(c128* p, c128 v, uint32_t ncl) { for (uint32_t k = 0; k < ncl; ++k) pc_st_c128(pc_map(p, k), v); }
 
-template <int THREADS, int R, int S>
+template <int THREADS, int R, int S, int DEPTH>
 __global__ void __launch_bounds__(THREADS, (THREADS <= 256) ? 2 : 1)
 k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int c0, int w, int ne,
             int* __restrict__ piv, int* __restrict__ info) {
     constexpr int NW = THREADS / 32;
+    extern __shared__ __align__(16) unsigned char pc_stage[];
+    c128* stage = reinterpret_cast<c128*>(pc_stage);
     const uint32_t rank = pc_rank(), ncl = pc_nranks();
     const int item = blockIdx.x / ncl;
     c128* A = base + (size_t)item * stride;
     int* pv = piv + (size_t)item * n;
-    __shared__ double red_v[PC_MAXCL * NW];
-    __shared__ int red_i[PC_MAXCL * NW];
-    __shared__ c128 prow[S], jrow[S];
+    // column-step exchange, double-buffered by the parity of the column: per (CTA, warp) the candidate's row (S entries),
+    // the reciprocal of its would-be pivot and the arg-max key; the row that stands at the pivot position
+    __shared__ c128 cand[2][PC_MAXCL * NW][S + 2];
+    __shared__ c128 jrow[2][S];
     __shared__ c128 L11[S * S];                 // L11[i*S + q] = multiplier of row cs+i, column cs+q (q < i)
     __shared__ c128 Us[S * PC_MAXW];            // Us[q*PC_MAXW + c] = U(cs+q, cs+sw+c)
     __shared__ int spiv[S], canon[S];
@@ -73,82 +80,94 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
 #pragma unroll
             for (int q = 0; q < S; ++q) v[r][q] = (row < n && q < sw) ? A[row + (size_t)(cs + q) * n] : zero;
         }
-        // ---- 2: column steps
+        // ---- 2: column steps, one cluster barrier each.  Arg-max key of a row: the bits of |re|+|im| with the low 23
+        // mantissa bits replaced by (65535 - (row - c0), candidate slot): one unsigned 64-bit maximum picks the largest
+        // magnitude and, among (nearly) equal ones, the lowest row; 0 = not eligible.
+        int piv_reg[S];
 #pragma unroll
         for (int q = 0; q < S; ++q) {
+            piv_reg[q] = cs + q;
             if (q < sw) {
-                const int j = cs + q;
-                double bv = -1.0; int bi = 0x7fffffff;
+                const int j = cs + q, par = q & 1;
+                const int myslot = (int)rank * NW + warp;
+                unsigned long long key = 0ull; int rb = 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const int row = c0 + g0 + r * TT;
-                    const double a = cabs1(v[r][q]);
-                    if (row >= j && row < ne && a > bv) { bv = a; bi = row; }
-                }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-                    const double ov = __shfl_xor_sync(0xffffffffu, bv, o); const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-                }
-                // every warp publishes its candidate in every CTA's table: lane k < ncl writes to CTA k
-                if (lane < (int)ncl) {
-                    pc_st_f64(pc_map(&red_v[rank * NW + warp], lane), bv);
-                    pc_st_s32(pc_map(&red_i[rank * NW + warp], lane), bi);
-                }
-                pc_sync();
-                bv = -1.0; bi = 0x7fffffff;
-                for (int e = lane; e < ncand; e += 32) {
-                    const double ov = red_v[e]; const int oi = red_i[e];
-                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-                }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-                    const double ov = __shfl_xor_sync(0xffffffffu, bv, o); const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-                }
-                const bool bad = !(bv > 0.0) || !(bv < 1.0e300 * 1.0e300);     // zero, NaN or Inf pivot
-                const int p = bad ? j : bi;
-                if (tid == 0) {
-                    spiv[q] = p;
-                    if (rank == 0) { pv[j] = p; if (bad) atomicCAS(&info[item], 0, j + 1); }
-                }
-                // ---- pivot row and row j into every CTA's copy
-                const int gj = (j - c0) % TT, rj = (j - c0) / TT;
-                const int gp = (p - c0) % TT, rp_ = (p - c0) / TT;
-                if (g0 == gp) {
-#pragma unroll
-                    for (int r = 0; r < R; ++r) if (r == rp_) {
-#pragma unroll
-                        for (int t = 0; t < S; ++t) pc_bcast_c128(&prow[t], v[r][t], ncl);
+                    if (row >= j && row < ne) {
+                        const unsigned long long kk = ((unsigned long long)__double_as_longlong(cabs1(v[r][q])) & ~0x7FFFFFull) |
+                                                      ((unsigned long long)(65535 - (row - c0)) << 7) | (unsigned long long)myslot;
+                        if (kk > key) { key = kk; rb = r; }
                     }
                 }
-                if (p != j && g0 == gj) {
+                c128 cr_[S];
+#pragma unroll
+                for (int t = 0; t < S; ++t) cr_[t] = v[0][t];
+#pragma unroll
+                for (int r = 1; r < R; ++r) if (r == rb) {
+#pragma unroll
+                    for (int t = 0; t < S; ++t) cr_[t] = v[r][t];
+                }
+                const c128 rinv = crecip_fast(cr_[q]);
+                const uint32_t khi = (uint32_t)(key >> 32), klo = (uint32_t)key;
+                const uint32_t mhi = __reduce_max_sync(0xffffffffu, khi);
+                const uint32_t mlo = __reduce_max_sync(0xffffffffu, (khi == mhi) ? klo : 0u);
+                if (key != 0ull && khi == mhi && klo == mlo) {
+                    for (uint32_t kc = 0; kc < ncl; ++kc) {
+                        const uint32_t dst = pc_map(&cand[par][myslot][0], kc);
+#pragma unroll
+                        for (int t = 0; t < S; ++t) pc_st_c128(dst + t * (uint32_t)sizeof(c128), cr_[t]);
+                        pc_st_c128(dst + S * (uint32_t)sizeof(c128), rinv);
+                    }
+                }
+                if (lane < (int)ncl)
+                    pc_st_u64(pc_map(&cand[par][myslot][S + 1], lane), ((unsigned long long)mhi << 32) | mlo);
+                const int gj = (j - c0) % TT, rj = (j - c0) / TT;
+                if (g0 == gj) {
 #pragma unroll
                     for (int r = 0; r < R; ++r) if (r == rj) {
 #pragma unroll
-                        for (int t = 0; t < S; ++t) pc_bcast_c128(&jrow[t], v[r][t], ncl);
+                        for (int t = 0; t < S; ++t) pc_bcast_c128(&jrow[par][t], v[r][t], ncl);
                     }
                 }
                 pc_sync();
-                if (p != j) {
-                    if (g0 == gj) {
-#pragma unroll
-                        for (int r = 0; r < R; ++r) if (r == rj) {
-#pragma unroll
-                            for (int t = 0; t < S; ++t) v[r][t] = prow[t];
-                        }
-                    }
-                    if (g0 == gp) {
-#pragma unroll
-                        for (int r = 0; r < R; ++r) if (r == rp_) {
-#pragma unroll
-                            for (int t = 0; t < S; ++t) v[r][t] = jrow[t];
-                        }
-                    }
+                // winner among the CL*NW candidates: every lane takes the slots lane, lane+32, ..., two more redux.sync
+                unsigned long long ck = 0ull;
+                for (int e = lane; e < ncand; e += 32) {
+                    const unsigned long long ok = reinterpret_cast<const unsigned long long*>(&cand[par][e][S + 1])[0];
+                    ck = ok > ck ? ok : ck;
                 }
-                // ---- scale column j and rank-1 update of the sub-panel's remaining columns
+                const uint32_t chi = (uint32_t)(ck >> 32), clo = (uint32_t)ck;
+                const uint32_t whi = __reduce_max_sync(0xffffffffu, chi);
+                const uint32_t wlo = __reduce_max_sync(0xffffffffu, (chi == whi) ? clo : 0u);
+                const unsigned long long wkey = ((unsigned long long)whi << 32) | wlo;
+                const int wsel = (int)(wkey & 127ull);
+                const bool bad = (wkey >> 23) == 0ull || (uint32_t)(wkey >> 52) >= 0x7FFu;     // zero, NaN or Inf pivot
+                const int p = bad ? j : c0 + 65535 - (int)((wkey >> 7) & 0xFFFFull);
+                piv_reg[q] = bad ? -1 - j : p;
                 if (!bad) {
-                    const c128 rp = crecip_fast(prow[q]);
+                    c128 prow[S];
+#pragma unroll
+                    for (int t = 0; t < S; ++t) prow[t] = cand[par][wsel][t];
+                    const c128 rp = cand[par][wsel][S];
+                    const int gp = (p - c0) % TT, rp_ = (p - c0) / TT;
+                    if (p != j) {
+                        if (g0 == gp) {
+#pragma unroll
+                            for (int r = 0; r < R; ++r) if (r == rp_) {
+#pragma unroll
+                                for (int t = 0; t < S; ++t) v[r][t] = jrow[par][t];
+                            }
+                        }
+                        if (g0 == gj) {
+#pragma unroll
+                            for (int r = 0; r < R; ++r) if (r == rj) {
+#pragma unroll
+                                for (int t = 0; t < S; ++t) v[r][t] = prow[t];
+                            }
+                        }
+                    }
+                    // ---- scale column j and rank-1 update of the sub-panel's remaining columns
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
                         const int row = c0 + g0 + r * TT;
@@ -176,6 +195,14 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
             }
         }
         if (tid == 0) {
+#pragma unroll
+            for (int q = 0; q < S; ++q) {
+                if (q < sw) {
+                    const int pq = piv_reg[q] < 0 ? -1 - piv_reg[q] : piv_reg[q];
+                    spiv[q] = pq;
+                    if (rank == 0) { pv[cs + q] = pq; if (piv_reg[q] < 0) atomicCAS(&info[item], 0, cs + q + 1); }
+                }
+            }
             // canon[i] = first step whose pivot row equals that of step i (rows below the sub-panel only)
             for (int i = 0; i < sw; ++i) {
                 int c = -1;
@@ -233,40 +260,41 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
             }
         }
         pc_sync();           // interchanged columns (global) and the rows of U (shared) visible to the whole cluster
-        // ---- 5: rank-sw update of the inner panel's remaining columns (rows below the sub-panel), software-pipelined
+        // ---- 5: rank-sw update of the inner panel's remaining columns (rows below the sub-panel): the columns stream
+        // through shared memory with per-thread asynchronous copies, DEPTH columns ahead (as in panel_body.cuh)
         if (nright > 0) {
-            constexpr int RC = (R % 5 == 0) ? 5 : ((R % 4 == 0) ? 4 : R);      // rows per chunk
-            constexpr int NCH = R / RC;
-            c128 cur[RC], nxt[RC];
+            auto issue = [&](int c) {
+                if (c < nright) {
+                    c128* dst = stage + (size_t)(c % DEPTH) * (R * THREADS) + tid;
+                    const c128* src = A + (size_t)(cs + sw + c) * n + c0 + g0;
 #pragma unroll
-            for (int i = 0; i < RC; ++i) {
-                const int row = c0 + g0 + i * TT;
-                cur[i] = (row >= cs + sw && row < n) ? A[row + (size_t)(cs + sw) * n] : zero;
-            }
-            for (int c = 0; c < nright; ++c) {
-#pragma unroll
-                for (int ch = 0; ch < NCH; ++ch) {
-                    const int nch = (ch + 1 == NCH) ? 0 : ch + 1;
-                    const int nc = c + ((ch + 1 == NCH) ? 1 : 0);
-#pragma unroll
-                    for (int i = 0; i < RC; ++i) {
-                        const int row = c0 + g0 + (nch * RC + i) * TT;
-                        nxt[i] = (nc < nright && row >= cs + sw && row < n) ? A[row + (size_t)(cs + sw + nc) * n] : zero;
-                    }
-#pragma unroll
-                    for (int i = 0; i < RC; ++i) {
-                        const int r = ch * RC + i;
+                    for (int r = 0; r < R; ++r) {
                         const int row = c0 + g0 + r * TT;
-                        if (row >= cs + sw && row < n) {
-#pragma unroll
-                            for (int q = 0; q < S; ++q) if (q < sw) cfms(cur[i], v[r][q], Us[q * PC_MAXW + c]);
-                            A[row + (size_t)(cs + sw + c) * n] = cur[i];
-                        }
+                        if (row >= cs + sw && row < n) cp_async16(dst + r * THREADS, src + (size_t)r * TT);
                     }
-#pragma unroll
-                    for (int i = 0; i < RC; ++i) cur[i] = nxt[i];
                 }
+                cp_async_commit();
+            };
+            for (int d = 0; d < DEPTH; ++d) issue(d);
+            for (int c = 0; c < nright; ++c) {
+                cp_async_wait<DEPTH - 1>();
+                const c128* src = stage + (size_t)(c % DEPTH) * (R * THREADS) + tid;
+                c128 u[S];
+#pragma unroll
+                for (int q = 0; q < S; ++q) u[q] = (q < sw) ? Us[q * PC_MAXW + c] : zero;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int row = c0 + g0 + r * TT;
+                    if (row >= cs + sw && row < n) {
+                        c128 x = src[r * THREADS];
+#pragma unroll
+                        for (int q = 0; q < S; ++q) if (q < sw) cfms(x, v[r][q], u[q]);
+                        A[row + (size_t)(cs + sw + c) * n] = x;
+                    }
+                }
+                issue(c + DEPTH);
             }
+            cp_async_wait<0>();
         }
         pc_sync();           // updated columns visible before the next sub-panel is loaded by other owners' neighbours
     }
@@ -292,20 +320,33 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
     }
 }
 
-template <int THREADS, int R, int S>
+template <int THREADS, int R, int DEPTH> constexpr size_t pc_stage_bytes() { return (size_t)DEPTH * R * THREADS * sizeof(c128); }
+
+template <int THREADS, int R, int S, int DEPTH>
 static int launch_clu(c128* base, size_t stride, int n, int J, int Wout, int c0, int w, int ne, int batch, int* piv, int* info,
                       int cl, cudaStream_t st) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(batch * cl), 1, 1);
     cfg.blockDim = dim3(THREADS, 1, 1);
-    cfg.dynamicSmemBytes = 0;
+    cfg.dynamicSmemBytes = pc_stage_bytes<THREADS, R, DEPTH>();
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    LSMS_CUDA_OK(cudaLaunchKernelEx(&cfg, k_panel_clu<THREADS, R, S>, base, stride, n, J, Wout, c0, w, ne, piv, info));
+    LSMS_CUDA_OK(cudaLaunchKernelEx(&cfg, k_panel_clu<THREADS, R, S, DEPTH>, base, stride, n, J, Wout, c0, w, ne, piv, info));
     LSMS_LAUNCH_CHECK();
+    return 0;
+}
+
+// (THREADS, R rows per thread, S sub-panel width, DEPTH columns in flight in step 5)
+#define LSMS_PC_LIST(X) X(256, 1, 4, 4) X(256, 2, 4, 4) X(512, 2, 4, 4) X(512, 5, 4, 4) X(512, 10, 2, 2)
+
+int init_attrs_panel_cluster() {
+#define LSMS_PC_ATTR(T, R, S, D) \
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_panel_clu<T, R, S, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pc_stage_bytes<T, R, D>()));
+    LSMS_PC_LIST(LSMS_PC_ATTR)
+#undef LSMS_PC_ATTR
     return 0;
 }
 
@@ -314,12 +355,12 @@ int launch_panel_cluster(c128* base, size_t stride, int n, int J, int Wout, int 
                          int cl, cudaStream_t st) {
     if (w < 1 || w > PC_MAXW || Wout > PC_MAXOUT || cl < 2 || cl > PC_MAXCL) return -1;
     const int m = (n - c0 + cl - 1) / cl;
-#define LSMS_PC(T, R, S) return launch_clu<T, R, S>(base, stride, n, J, Wout, c0, w, ne, batch, piv, info, cl, st)
-    if (m <= 256) LSMS_PC(256, 1, 4);
-    if (m <= 512) LSMS_PC(256, 2, 4);
-    if (m <= 1024) LSMS_PC(512, 2, 4);
-    if (m <= 2560) LSMS_PC(512, 5, 4);
-    if (m <= 5120) LSMS_PC(512, 10, 2);
+#define LSMS_PC(T, R, S, D) return launch_clu<T, R, S, D>(base, stride, n, J, Wout, c0, w, ne, batch, piv, info, cl, st)
+    if (m <= 256) LSMS_PC(256, 1, 4, 4);
+    if (m <= 512) LSMS_PC(256, 2, 4, 4);
+    if (m <= 1024) LSMS_PC(512, 2, 4, 4);
+    if (m <= 2560) LSMS_PC(512, 5, 4, 4);
+    if (m <= 5120) LSMS_PC(512, 10, 2, 2);
 #undef LSMS_PC
     return -1;
 }
