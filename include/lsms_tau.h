@@ -73,7 +73,8 @@ enum {
     LSMS_OPT_GROUPS = 3,        /* batch groups on separate streams, forked from and joined into the caller's stream:
                                    0 (default) chosen per shape, 1..8 forced                                               */
     LSMS_OPT_PANEL_THREADS = 4, /* panel kernel (K2): 1 (default) 512 threads for panels taller than 1280 rows, 256 below;
-                                   0: 256 threads throughout (half an SM)                                                  */
+                                   0: 256 threads throughout (half an SM); 2: 128 threads (a quarter SM, the footprint of one
+                                   Schur-update CTA) for panels of up to 1024 rows                                         */
     LSMS_OPT_PANEL_CLUSTER = 5, /* CTAs per matrix in the panel kernel (thread-block cluster, rows dealt round-robin,
                                    exchange through distributed shared memory): 0 (default) chosen per shape, 1 never,
                                    2 / 4 / 8 forced                                                                        */
