@@ -108,22 +108,20 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
                         if (kk > key) { key = kk; rb = r; }
                     }
                 }
-                c128 cr_[S];
+                c128 vq = v[0][q];
 #pragma unroll
-                for (int t = 0; t < S; ++t) cr_[t] = v[0][t];
-#pragma unroll
-                for (int r = 1; r < R; ++r) if (r == rb) {
-#pragma unroll
-                    for (int t = 0; t < S; ++t) cr_[t] = v[r][t];
-                }
-                const c128 rinv = crecip_fast(cr_[q]);
+                for (int r = 1; r < R; ++r) if (r == rb) vq = v[r][q];
+                const c128 rinv = crecip_fast(vq);
                 const uint32_t khi = (uint32_t)(key >> 32), klo = (uint32_t)key;
                 const uint32_t mhi = __reduce_max_sync(0xffffffffu, khi);
                 const uint32_t mlo = __reduce_max_sync(0xffffffffu, (khi == mhi) ? klo : 0u);
                 c128* slot = sh.cand[par][warp];
                 if (key != 0ull && khi == mhi && klo == mlo) {
 #pragma unroll
-                    for (int t = 0; t < S; ++t) slot[t] = cr_[t];
+                    for (int r = 0; r < R; ++r) if (r == rb) {
+#pragma unroll
+                        for (int t = 0; t < S; ++t) slot[t] = v[r][t];
+                    }
                     slot[4] = rinv;
                 }
                 if (lane == 0) reinterpret_cast<unsigned long long*>(slot + 5)[0] = ((unsigned long long)mhi << 32) | mlo;
