@@ -532,6 +532,29 @@ def test_small_mode_is_chosen_for_the_small_configs_and_matches_the_oracle(lt, h
     assert not infob.any() and lt.lsms_last_schedule(h) == 0
 
 
+def test_scheduler_leaves_the_on_chip_mode_when_the_batch_needs_many_waves_of_clusters(lt, h):
+    """The on-chip kernel holds a cluster of SMs per matrix for the whole elimination: by default it is used while the
+    batch needs at most ~3.5 waves of clusters (here 208^2: 4 SMs each, <= 129 matrices on 148 SMs) and the lock-step
+    schedule beyond; forced (small_mode = 7) it runs any batch, wave after wave, with the same results."""
+    n_sites, kmax, B = 13, 16, 160
+    A = sl.random_dense_matrices(B, n_sites * kmax, seed=4242)
+    tau_ls, info = lt.lsms_tau00_batched(h, torch.from_numpy(A).cuda(), n_sites, kmax, False, B)
+    torch.cuda.synchronize()
+    assert lt.lsms_last_schedule(h) == 0 and not info.cpu().numpy().any()
+    tau_few, info = lt.lsms_tau00_batched(h, torch.from_numpy(A[:100]).cuda(), n_sites, kmax, False, 100)
+    torch.cuda.synchronize()
+    assert lt.lsms_last_schedule(h) == 104 and not info.cpu().numpy().any()
+    h.set("small_mode", 7)
+    tau_oc, info = lt.lsms_tau00_batched(h, torch.from_numpy(A).cuda(), n_sites, kmax, False, B)
+    torch.cuda.synchronize()
+    assert lt.lsms_last_schedule(h) == 104 and not info.cpu().numpy().any()
+    tau_ls, tau_few, tau_oc = (t.cpu().numpy().transpose(0, 2, 1) for t in (tau_ls, tau_few, tau_oc))
+    assert np.array_equal(tau_few, tau_oc[:100])                 # the same kernel on the same matrices, whatever the batch
+    for b in range(0, B, 7):
+        check_tau(tau_oc[b], tau_ls[b], 1e-11, ("on chip vs lock-step", b))
+        check_tau(tau_oc[b], lapack_tau00(A[b], kmax), 1e-11, ("on chip vs LAPACK", b))
+
+
 # ------------------------------------------------------------------ boundary: re-entrancy and input validation
 
 def test_two_host_threads_two_handles_two_streams(lt):
