@@ -188,7 +188,7 @@ static int eliminate_prio(const Ctx* c, c128* M, int n, int k, int batch, const 
     for (int J = 0, W = W0; J < ne && !rc; J += W, W = (ne - J < NB) ? ne - J : NB) {
         const int Jend = J + W;
         { ProfScope ps(6, ax); rc = launch_row_permute(M, stride, n, J, W, Jend, n, batch, ws.perm, ws.tperm, (size_t)NB * n, NB, ax); } if (rc) break;
-        GemmShape t; t.batch = batch; t.beta0 = 1;
+        GemmShape t; t.batch = batch; t.beta0 = 1; t.triA = 1;
         t.A = ws.ninv; t.strideA = (size_t)NB * NB; t.ldA = NB;
         t.B = ws.tperm + (size_t)Jend * NB; t.strideB = (size_t)NB * n; t.ldB = NB;
         t.C = M + (size_t)J + (size_t)Jend * n; t.strideC = stride; t.ldC = n;
@@ -231,7 +231,7 @@ static int eliminate(const Ctx* c, c128* M, int n, int k, int batch, const TauWs
     for (int J = 0, W = W0; J < ne; J += W, W = (ne - J < NB) ? ne - J : NB) {
         const int Jend = J + W;                               // Jend <= ne < n
         { ProfScope ps(6, st); rc = launch_row_permute(M, stride, n, J, W, Jend, n, batch, ws.perm, ws.tperm, (size_t)NB * n, NB, st); } if (rc) return rc;
-        GemmShape t; t.batch = batch; t.beta0 = 1;
+        GemmShape t; t.batch = batch; t.beta0 = 1; t.triA = 1;
         t.A = ws.ninv; t.strideA = (size_t)NB * NB; t.ldA = NB;
         t.B = ws.tperm + (size_t)Jend * NB; t.strideB = (size_t)NB * n; t.ldB = NB;
         t.C = M + (size_t)J + (size_t)Jend * n; t.strideC = stride; t.ldC = n;

@@ -14,7 +14,7 @@
 
 namespace lsms {
 
-template <int STAGES, int BN>
+template <int STAGES, int BN, bool TRI>
 __global__ void __launch_bounds__(BN * 4, 512 / (BN * 4))
 k_schur_gemm(GemmShape g, int tiles_m) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -32,10 +32,10 @@ k_schur_gemm(GemmShape g, int tiles_m) {
     }
     __syncthreads();
     uint32_t cc = 0;
-    gemm_tile<STAGES, BN>(g, A, B, C, mvalid, nvalid, ring, full, cc);
+    gemm_tile<STAGES, BN, TRI>(g, A, B, C, mvalid, nvalid, ring, full, cc);
 }
 
-template <int STAGES, int BN>
+template <int STAGES, int BN, bool TRI>
 static int launch_classic(const GemmShape& g, cudaStream_t st) {
     const int tiles_m = (g.Mr + BM - 1) / BM, tiles_n = (g.Nc + BN - 1) / BN;
     for (int b0 = 0; b0 < g.batch; b0 += 65535) {
@@ -43,7 +43,7 @@ static int launch_classic(const GemmShape& g, cudaStream_t st) {
         h.A = g.A + (size_t)b0 * g.strideA; h.B = g.B + (size_t)b0 * g.strideB; h.C = g.C + (size_t)b0 * g.strideC;
         h.batch = g.batch - b0 < 65535 ? g.batch - b0 : 65535;
         dim3 grid((unsigned)(tiles_m * tiles_n), (unsigned)h.batch);
-        k_schur_gemm<STAGES, BN><<<grid, BN * 4, gemm_smem<STAGES, BN>(), st>>>(h, tiles_m);
+        k_schur_gemm<STAGES, BN, TRI><<<grid, BN * 4, gemm_smem<STAGES, BN>(), st>>>(h, tiles_m);
         LSMS_LAUNCH_CHECK();
     }
     return 0;
@@ -59,15 +59,17 @@ static int launch_classic(const GemmShape& g, cudaStream_t st) {
 // (31.7 TFLOP/s, bank-conflicted LDS.64) and a persistent one-CTA-per-SM variant with the next C tile prefetched
 // into shared memory (23.3 TFLOP/s).
 int init_attrs_gemm() {
-    LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<1, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<1, 32>()));
-    LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<2, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<2, 32>()));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<1, 32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<1, 32>()));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<2, 32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<2, 32>()));
+    LSMS_CUDA_OK(cudaFuncSetAttribute(k_schur_gemm<2, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemm_smem<2, 32>()));
     return 0;
 }
 
 int launch_schur_gemm(const GemmShape& g, cudaStream_t st) {
     if (g.Mr <= 0 || g.Nc <= 0 || g.K <= 0 || g.batch <= 0) return 0;
-    if (g.K <= KS) return launch_classic<1, 32>(g, st);
-    return launch_classic<2, 32>(g, st);
+    if (g.K <= KS) return launch_classic<1, 32, false>(g, st);
+    if (g.triA && g.Mr <= BM) return launch_classic<2, 32, true>(g, st);
+    return launch_classic<2, 32, false>(g, st);
 }
 
 }  // namespace lsms

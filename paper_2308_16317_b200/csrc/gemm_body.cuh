@@ -67,7 +67,10 @@ __device__ __forceinline__ void issue_chunk(const GemmShape& g, const c128* A, c
 // ring since its mbarriers were initialised (slot = cc % STAGES, parity = (cc / STAGES) & 1), so that a persistent
 // CTA can call this for tile after tile; the caller separates two calls by a __syncthreads() (ring reuse).
 // Used by k_schur_gemm (one tile per CTA, cc = 0) and by the small-matrix kernel of fused.cu.
-template <int STAGES, int BN>
+// TRI: A is LOWER TRIANGULAR with its diagonal at the tile's origin (the triangular solve as a GEMM, U12 = -(Ninv * T) with
+// Ninv = -(L11^-1), one tile row): the 8-row fragment blocks of A that lie wholly above the diagonal are exact zeros and
+// their DMMAs are skipped (56 % of the dense count at 64 rows); the result is unchanged.
+template <int STAGES, int BN, bool TRI = false>
 __device__ __forceinline__ void gemm_tile(const GemmShape& g, const c128* __restrict__ A, const c128* __restrict__ B,
                                           c128* __restrict__ C, int mvalid, int nvalid, c128* ring, uint64_t* full, uint32_t& cc) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -101,6 +104,28 @@ __device__ __forceinline__ void gemm_tile(const GemmShape& g, const c128* __rest
 #pragma unroll 1
         for (int ks = 0; ks < nfull; ++ks) {
             const int k0 = ks * 4;
+            if (TRI) {
+                // rows wm + mt*8 .. +7 of A are zero in columns > row: block mt is live iff its last row >= first column
+                const int kglob = kc * KS + k0;
+                if (wm + 31 < kglob) continue;                       // the whole 32-row warp tile lies above the diagonal
+                c128 b[2];
+#pragma unroll
+                for (int nt = 0; nt < 2; ++nt) b[nt] = Bs[(wn + nt * 8 + gq) * LDB_S + k0 + q];
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    if (wm + mt * 8 + 7 >= kglob) {
+                        const c128 a = As[(k0 + q) * LDA_S + wm + mt * 8 + gq];
+#pragma unroll
+                        for (int nt = 0; nt < 2; ++nt) {
+                            dmma884(cr[mt][nt][0], cr[mt][nt][1], a.x, -b[nt].x);
+                            dmma884(ci[mt][nt][0], ci[mt][nt][1], a.x, -b[nt].y);
+                            dmma884(cr[mt][nt][0], cr[mt][nt][1], a.y, b[nt].y);
+                            dmma884(ci[mt][nt][0], ci[mt][nt][1], a.y, -b[nt].x);
+                        }
+                    }
+                }
+                continue;
+            }
             c128 a[4], b[2];
 #pragma unroll
             for (int mt = 0; mt < 4; ++mt) a[mt] = As[(k0 + q) * LDA_S + wm + mt * 8 + gq];

@@ -68,6 +68,7 @@ struct GemmShape {
     int ldA, ldB, ldC;
     int Mr, Nc, K;
     int beta0;                               // 0: C -= A*B ;  1: C = -(A*B)  (C is not read)
+    int triA = 0;                            // 1: A is lower triangular, Mr <= 64 (one tile row): zero blocks are skipped
     int batch;
 };
 int launch_schur_gemm(const GemmShape& g, cudaStream_t st);
