@@ -14,9 +14,10 @@
 //         with that row's entries and the reciprocal of the would-be pivot, so the winner's row is already in shared
 //         memory when the barrier opens); rows never move between threads, each thread tracks the position of its
 //         row in the pivoted arrangement; result -> the owner's panel buffer
-//     R2  cluster barrier (all CTAs are done with the previous panel), then the panel buffer is sent to the other
-//         CTAs by the TMA engine: bulk copies shared -> remote shared (cp.async.bulk.shared::cluster.shared::cta),
-//         completion counted on an mbarrier of the RECEIVING CTA -- no second cluster barrier
+//     R2  the panel buffer is sent to the other CTAs by the TMA engine: bulk copies shared -> remote shared
+//         (cp.async.bulk.shared::cluster.shared::cta), completion counted on an mbarrier of the RECEIVING CTA; a
+//         receiver declares its panel buffer free by a release-store of a flag into the next owner's shared memory,
+//         which the owner polls before it copies -- no cluster-wide barrier inside the loop
 //     R3  every CTA, its own trailing columns: the panel's interchanges and the 8 x 8 unit-lower solve, one thread per
 //         column (rows of U -> a small operand buffer and, for the verification export, to global memory)
 //     R4  rank-8 update of its trailing columns on the FP64 tensor pipe (DMMA.8x8x4 from shared memory; operand
@@ -57,7 +58,7 @@ __host__ __device__ inline ResLayout res_layout(int n, int ncl) {
     L.off_piv = o; o += 32 * sizeof(c128);       // net row permutation of the panel (96 B, bulk-copied) + slack for tile over-reads
     L.off_U = o; o += (size_t)L.ncols_max * RS_LDU * sizeof(c128);
     L.off_red = o; o += 2 * RS_RED_PAR;
-    L.off_bar = o; o += 64;
+    L.off_bar = o; o += 128;                    // two mbarriers + the per-CTA 'panel buffer free' flags
     L.total = o;
     return L;
 }
@@ -90,6 +91,12 @@ __device__ __forceinline__ uint32_t rs_mapa(uint32_t addr, uint32_t rank) {
 __device__ __forceinline__ void rs_cluster_sync() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+__device__ __forceinline__ void rs_st_release_remote(uint32_t addr_cluster, int v) {
+    asm volatile("st.release.cluster.shared::cluster.s32 [%0], %1;" ::"r"(addr_cluster), "r"(v) : "memory");
+}
+__device__ __forceinline__ int rs_ld_acquire(const int* p) {
+    int v; asm volatile("ld.acquire.cluster.shared::cta.s32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory"); return v;
+}
 // shared (this CTA) -> shared of another CTA of the cluster, by the TMA engine; completion on the receiver's mbarrier
 __device__ __forceinline__ void rs_bulk_s2r(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
     asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -108,6 +115,7 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
     unsigned char* red = rsm + L.off_red;
     uint64_t* bar_load = reinterpret_cast<uint64_t*>(rsm + L.off_bar);
     uint64_t* bar_full = bar_load + 1;
+    int* ready = reinterpret_cast<int*>(bar_load + 2);   // ready[r], written by CTA r: r's panel buffer may receive panel ready[r]
     const int ld = L.ld, ldp = L.ldp;
 
     const int item = blockIdx.x / ncl;
@@ -121,6 +129,7 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
     const int my_cols = my_blocks * RW;                       // local columns incl. the padding of a ragged last block
     auto gcol = [&](int lc) { return ((lc / RW) * ncl + rank) * RW + lc % RW; };
 
+    if (tid < 8) ready[tid] = 0;
     if (tid == 0) {
         mbar_init(bar_load, 1); mbar_init(bar_full, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -341,7 +350,17 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
         }
     };
 
+    // this CTA has finished reading panel q-1 from its panel buffer: arm the mbarrier for panel q and tell q's owner
+    auto declare_free = [&](int q) {
+        if (q < np && q % ncl != rank && tid == 0) {
+            const int mq = n - q * RW;
+            mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * mq * sizeof(c128) + 3 * RW * sizeof(int)));
+            rs_st_release_remote(rs_mapa(smem_u32(&ready[rank]), (uint32_t)(q % ncl)), q);
+        }
+    };
     if (np > 0 && rank == 0) panel_factor(0);            // the first panel has nothing to hide behind
+    if (np > 0 && rank != 0 && tid == 0) mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * n * sizeof(c128) + 3 * RW * sizeof(int)));
+    if (ncl > 1) rs_cluster_sync();                      // every receiver is armed for panel 0 (ready[] = 0 everywhere)
     for (int p = 0; p < np; ++p) {
         const int m = n - p * RW;
         const int owner = p % ncl;
@@ -351,28 +370,23 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
             __syncthreads();
             R_TOC(1);
             R_STAMP(p, 0);
-        } else if (tid == 0) {
-            mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * m * sizeof(c128) + 3 * RW * sizeof(int)));
-        }
-        // ================= R2: every CTA has finished the previous panel's update; ship the panel
-        if (ncl > 1) {
-            rs_cluster_sync();
-            if (rank == owner) {
-                // the CTA that owns the NEXT panel is served first: its step is the critical path
-                if (tid < RW + 1) {
-                    const int c = tid;
-                    for (int d = 1; d < ncl; ++d) {
-                        const uint32_t dst = (uint32_t)((rank + d) % ncl);
-                        const uint32_t rbar = rs_mapa(smem_u32(bar_full), dst);
-                        if (c < RW) rs_bulk_s2r(rs_mapa(smem_u32(Lbuf + (size_t)c * ldp), dst), smem_u32(Lbuf + (size_t)c * ldp), (uint32_t)(m * sizeof(c128)), rbar);
-                        else rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv), (uint32_t)(3 * RW * sizeof(int)), rbar);
-                    }
+            // ================= R2: ship the panel -- to each CTA as soon as IT has declared its panel buffer free (a flag
+            // it stores, with release semantics, into this CTA's shared memory): no cluster-wide barrier on the critical
+            // path.  The CTA that owns the NEXT panel is served first.
+            if (ncl > 1 && tid < RW + 1) {
+                const int c = tid;
+                for (int d = 1; d < ncl; ++d) {
+                    const uint32_t dst = (uint32_t)((rank + d) % ncl);
+                    while (rs_ld_acquire(&ready[dst]) < p) {}
+                    const uint32_t rbar = rs_mapa(smem_u32(bar_full), dst);
+                    if (c < RW) rs_bulk_s2r(rs_mapa(smem_u32(Lbuf + (size_t)c * ldp), dst), smem_u32(Lbuf + (size_t)c * ldp), (uint32_t)(m * sizeof(c128)), rbar);
+                    else rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv), (uint32_t)(3 * RW * sizeof(int)), rbar);
                 }
-            } else {
-                mbar_wait(bar_full, full_parity); full_parity ^= 1;
-                if ((p + 1) % ncl == rank) R_STAMP(p, 2);
             }
-            if (rank == owner) R_STAMP(p, 1);
+            R_STAMP(p, 1);
+        } else {
+            mbar_wait(bar_full, full_parity); full_parity ^= 1;
+            if ((p + 1) % ncl == rank) R_STAMP(p, 2);
         }
         if (rank == owner) panel_export(p);
         R_TOC(2);
@@ -404,6 +418,7 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
             rank8_update(p, tl0, my_cols, 0, RS_T / 32);
         }
         __syncthreads();
+        declare_free(p + 1);
         R_TOC(3);
     }
     // ================= K5: the trailing k x k block -> global memory, inverted by rank 0
