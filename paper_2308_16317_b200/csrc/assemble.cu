@@ -53,7 +53,11 @@ __host__ __device__ inline void l_m_of(int L, int& l, int& m) { l = 0; while ((l
 
 // Table entry t (0..lmax) of the pair (L,L'), stored at [(t*kmax + L')*kmax + L]:
 //   coef = -4 pi i * i^{l-l'+l''} * C(L,L',L''),  idx = L'' = l''(l''+1) + m' - m,  l'' = |l-l'| + 2t.
-__global__ void k_gaunt_table(int lmax, c128* __restrict__ coef, int* __restrict__ idx) {
+__device__ __forceinline__ void legendre_table_block(int l2, double* __restrict__ leg);
+
+// The LAST block of the grid fills the Legendre recurrence table (below) instead: one launch for both tables.
+__global__ void k_gaunt_table(int lmax, c128* __restrict__ coef, int* __restrict__ idx, double* __restrict__ leg) {
+    if (blockIdx.x == gridDim.x - 1) { legendre_table_block(2 * lmax, leg); return; }
     int kmax = (lmax + 1) * (lmax + 1), nt = lmax + 1;
     int e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= kmax * kmax * nt) return;
@@ -126,7 +130,7 @@ __global__ void k_tinv(const c128* __restrict__ delta, const int* __restrict__ s
 // Fully normalised recurrence  Pbar_lm = a_lm (x Pbar_{l-1,m} - b_lm Pbar_{l-2,m}),
 // Pbar_mm = d_m sin(theta) Pbar_{m-1,m-1}; a, b, d tabulated once so that K1 has no sqrt/div inside.
 //   leg[0*S + l*(l2+1)+m] = a_lm, leg[1*S + ...] = b_lm, leg[2*S + m] = d_m,  S = (l2+1)^2
-__global__ void k_legendre_table(int l2, double* __restrict__ leg) {
+__device__ __forceinline__ void legendre_table_block(int l2, double* __restrict__ leg) {
     const int S = (l2 + 1) * (l2 + 1);
     for (int e = threadIdx.x; e < S; e += blockDim.x) {
         const int l = e / (l2 + 1), m = e % (l2 + 1);
@@ -327,9 +331,7 @@ int launch_assemble(const c128* tinv, const double* site_pos, const double* mome
     c128* coef = (c128*)ws;
     int* idx = (int*)((char*)ws + al256(e * sizeof(c128)));
     double* leg = (double*)((char*)ws + al256(e * sizeof(c128)) + al256(e * sizeof(int)));
-    k_gaunt_table<<<(unsigned)((e + 127) / 128), 128, 0, st>>>(lmax, coef, idx);
-    LSMS_LAUNCH_CHECK();
-    k_legendre_table<<<1, 128, 0, st>>>(l2, leg);
+    k_gaunt_table<<<(unsigned)((e + 127) / 128) + 1, 128, 0, st>>>(lmax, coef, idx, leg);
     LSMS_LAUNCH_CHECK();
     // row-site chunks: per-R tables of a chunk fit in ~52 KB: four CTAs (32 warps) per SM hide the gather and
     // table latencies better than two with bigger chunks (measured on workload P: 3.7 ms vs 4.8 ms)
