@@ -15,7 +15,7 @@
 namespace lsms {
 
 template <int STAGES, int BN, bool TRI>
-__global__ void __launch_bounds__(BN * 4, 512 / (BN * 4))
+__global__ void __launch_bounds__(BN * 4, (STAGES == 1 ? 6 : 4) * 128 / (BN * 4))
 k_schur_gemm(GemmShape g, int tiles_m) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c128* ring = reinterpret_cast<c128*>(smem_raw);
@@ -55,7 +55,9 @@ static int launch_classic(const GemmShape& g, cudaStream_t st) {
 // full (measured: 8 warps per SM reach 21.8 of 36.9 TFLOP/s, 16 warps 34.1).  With two 8-warp CTAs per SM the pipe
 // therefore starves whenever one of them loads or stores its C tile (92 % DMMA-active); with four 4-warp CTAs three
 // are still in their main loop: 34.6 TFLOP/s.  K <= 16 (rank-IB updates inside an outer panel, bound by the C-tile
-// traffic): the same 64 x 32 tiles with one ring stage (6.2 -> 4.9 ms per P step against 64 x 64 tiles).  Tried and dropped: a one-DMMA-per-accumulator loop body with operands picked by 64-bit loads
+// traffic): the same 64 x 32 tiles with one ring stage (6.2 -> 4.9 ms per P step against 64 x 64 tiles) and SIX CTAs per
+// SM (80 registers, 27 KB): each CTA is one load -> 4 k-steps -> store chain, so more of them in flight hide more of the
+// C-tile latency (4.9 -> 4.4 ms per P step, 9.6 -> 8.9 on C).  Tried and dropped: a one-DMMA-per-accumulator loop body with operands picked by 64-bit loads
 // (31.7 TFLOP/s, bank-conflicted LDS.64) and a persistent one-CTA-per-SM variant with the next C tile prefetched
 // into shared memory (23.3 TFLOP/s).
 int init_attrs_gemm() {
