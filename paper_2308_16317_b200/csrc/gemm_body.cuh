@@ -104,7 +104,7 @@ __device__ __forceinline__ void gemm_tile(const GemmShape& g, const c128* __rest
 #pragma unroll 1
         for (int ks = 0; ks < nfull; ++ks) {
             const int k0 = ks * 4;
-            if (TRI) {
+            if constexpr (TRI) {
                 // rows wm + mt*8 .. +7 of A are zero in columns > row: block mt is live iff its last row >= first column
                 const int kglob = kc * KS + k0;
                 if (wm + 31 < kglob) continue;                       // the whole 32-row warp tile lies above the diagonal
@@ -124,21 +124,21 @@ __device__ __forceinline__ void gemm_tile(const GemmShape& g, const c128* __rest
                         }
                     }
                 }
-                continue;
-            }
-            c128 a[4], b[2];
+            } else {
+                c128 a[4], b[2];
 #pragma unroll
-            for (int mt = 0; mt < 4; ++mt) a[mt] = As[(k0 + q) * LDA_S + wm + mt * 8 + gq];
+                for (int mt = 0; mt < 4; ++mt) a[mt] = As[(k0 + q) * LDA_S + wm + mt * 8 + gq];
 #pragma unroll
-            for (int nt = 0; nt < 2; ++nt) b[nt] = Bs[(wn + nt * 8 + gq) * LDB_S + k0 + q];
+                for (int nt = 0; nt < 2; ++nt) b[nt] = Bs[(wn + nt * 8 + gq) * LDB_S + k0 + q];
 #pragma unroll
-            for (int nt = 0; nt < 2; ++nt) {
+                for (int nt = 0; nt < 2; ++nt) {
 #pragma unroll
-                for (int mt = 0; mt < 4; ++mt) {
-                    dmma884(cr[mt][nt][0], cr[mt][nt][1], a[mt].x, -b[nt].x);
-                    dmma884(ci[mt][nt][0], ci[mt][nt][1], a[mt].x, -b[nt].y);
-                    dmma884(cr[mt][nt][0], cr[mt][nt][1], a[mt].y, b[nt].y);
-                    dmma884(ci[mt][nt][0], ci[mt][nt][1], a[mt].y, -b[nt].x);
+                    for (int mt = 0; mt < 4; ++mt) {
+                        dmma884(cr[mt][nt][0], cr[mt][nt][1], a[mt].x, -b[nt].x);
+                        dmma884(ci[mt][nt][0], ci[mt][nt][1], a[mt].x, -b[nt].y);
+                        dmma884(cr[mt][nt][0], cr[mt][nt][1], a[mt].y, b[nt].y);
+                        dmma884(ci[mt][nt][0], ci[mt][nt][1], a[mt].y, -b[nt].x);
+                    }
                 }
             }
         }
