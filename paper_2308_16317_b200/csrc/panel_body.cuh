@@ -125,13 +125,10 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
                     slot[4] = rinv;
                 }
                 if (lane == 0) reinterpret_cast<unsigned long long*>(slot + 5)[0] = ((unsigned long long)mhi << 32) | mlo;
-                const int tj = (j - c0) % THREADS, rj = (j - c0) / THREADS;
+                const int tj = j - c0;                      // row j belongs to thread j - c0 (< w <= 16 <= THREADS), its first row
                 if (tid == tj) {
 #pragma unroll
-                    for (int r = 0; r < R; ++r) if (r == rj) {
-#pragma unroll
-                        for (int t = 0; t < S; ++t) sh.jrow[par][t] = v[r][t];
-                    }
+                    for (int t = 0; t < S; ++t) sh.jrow[par][t] = v[0][t];
                 }
                 __syncthreads();
                 // winner among the NW warp candidates: lane l takes candidate l mod NW, two more redux.sync
@@ -160,10 +157,7 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
                         }
                         if (tid == tj) {
 #pragma unroll
-                            for (int r = 0; r < R; ++r) if (r == rj) {
-#pragma unroll
-                                for (int t = 0; t < S; ++t) v[r][t] = prow[t];
-                            }
+                            for (int t = 0; t < S; ++t) v[0][t] = prow[t];
                         }
                     }
                     // ---- scale column j and rank-1 update of the sub-panel's remaining columns

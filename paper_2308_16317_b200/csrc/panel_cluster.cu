@@ -100,35 +100,31 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
                         if (kk > key) { key = kk; rb = r; }
                     }
                 }
-                c128 cr_[S];
+                c128 vq = v[0][q];
 #pragma unroll
-                for (int t = 0; t < S; ++t) cr_[t] = v[0][t];
-#pragma unroll
-                for (int r = 1; r < R; ++r) if (r == rb) {
-#pragma unroll
-                    for (int t = 0; t < S; ++t) cr_[t] = v[r][t];
-                }
-                const c128 rinv = crecip_fast(cr_[q]);
+                for (int r = 1; r < R; ++r) if (r == rb) vq = v[r][q];
+                const c128 rinv = crecip_fast(vq);
                 const uint32_t khi = (uint32_t)(key >> 32), klo = (uint32_t)key;
                 const uint32_t mhi = __reduce_max_sync(0xffffffffu, khi);
                 const uint32_t mlo = __reduce_max_sync(0xffffffffu, (khi == mhi) ? klo : 0u);
                 if (key != 0ull && khi == mhi && klo == mlo) {
+#pragma unroll 1
                     for (uint32_t kc = 0; kc < ncl; ++kc) {
                         const uint32_t dst = pc_map(&cand[par][myslot][0], kc);
 #pragma unroll
-                        for (int t = 0; t < S; ++t) pc_st_c128(dst + t * (uint32_t)sizeof(c128), cr_[t]);
+                        for (int r = 0; r < R; ++r) if (r == rb) {
+#pragma unroll
+                            for (int t = 0; t < S; ++t) pc_st_c128(dst + t * (uint32_t)sizeof(c128), v[r][t]);
+                        }
                         pc_st_c128(dst + S * (uint32_t)sizeof(c128), rinv);
                     }
                 }
                 if (lane < (int)ncl)
                     pc_st_u64(pc_map(&cand[par][myslot][S + 1], lane), ((unsigned long long)mhi << 32) | mlo);
-                const int gj = (j - c0) % TT, rj = (j - c0) / TT;
+                const int gj = j - c0;                      // row j belongs to cluster thread j - c0 (< 16 <= TT), its first row
                 if (g0 == gj) {
 #pragma unroll
-                    for (int r = 0; r < R; ++r) if (r == rj) {
-#pragma unroll
-                        for (int t = 0; t < S; ++t) pc_bcast_c128(&jrow[par][t], v[r][t], ncl);
-                    }
+                    for (int t = 0; t < S; ++t) pc_bcast_c128(&jrow[par][t], v[0][t], ncl);
                 }
                 pc_sync();
                 // winner among the CL*NW candidates: every lane takes the slots lane, lane+32, ..., two more redux.sync
@@ -161,10 +157,7 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
                         }
                         if (g0 == gj) {
 #pragma unroll
-                            for (int r = 0; r < R; ++r) if (r == rj) {
-#pragma unroll
-                                for (int t = 0; t < S; ++t) v[r][t] = prow[t];
-                            }
+                            for (int t = 0; t < S; ++t) v[0][t] = prow[t];
                         }
                     }
                     // ---- scale column j and rank-1 update of the sub-panel's remaining columns
