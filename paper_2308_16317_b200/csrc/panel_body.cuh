@@ -98,16 +98,18 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             piv_reg[q] = cs + q;
             if (q < sw) {
                 const int j = cs + q, par = q & 1;
-                unsigned long long key = 0ull; int rb = 0;
+                // local best row by magnitude (ascending rows, strict >: the lowest row among equal ones), then ONE key
+                double ba = -1.0; int rb = 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const int row = c0 + tid + r * THREADS;
-                    if (row >= j && row < ne) {
-                        const unsigned long long kk = ((unsigned long long)__double_as_longlong(cabs1(v[r][q])) & ~0x3FFFFull) |
-                                                      ((unsigned long long)(16383 - (row - c0)) << 4) | (unsigned long long)warp;
-                        if (kk > key) { key = kk; rb = r; }
-                    }
+                    const double a = cabs1(v[r][q]);
+                    if (row >= j && row < ne && (a > ba || a != a)) { ba = a; rb = r; }   // a NaN entry is taken, kept and flagged
                 }
+                unsigned long long key = 0ull;
+                if (ba >= 0.0 || ba != ba)
+                    key = ((unsigned long long)__double_as_longlong(ba) & ~0x3FFFFull) |
+                          ((unsigned long long)(16383 - (tid + rb * THREADS)) << 4) | (unsigned long long)warp;
                 c128 vq = v[0][q];
 #pragma unroll
                 for (int r = 1; r < R; ++r) if (r == rb) vq = v[r][q];

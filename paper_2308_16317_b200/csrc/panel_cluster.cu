@@ -90,16 +90,18 @@ k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int 
             if (q < sw) {
                 const int j = cs + q, par = q & 1;
                 const int myslot = (int)rank * NW + warp;
-                unsigned long long key = 0ull; int rb = 0;
+                // local best row by magnitude (ascending rows, strict >: the lowest row among equal ones), then ONE key
+                double ba = -1.0; int rb = 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const int row = c0 + g0 + r * TT;
-                    if (row >= j && row < ne) {
-                        const unsigned long long kk = ((unsigned long long)__double_as_longlong(cabs1(v[r][q])) & ~0x7FFFFFull) |
-                                                      ((unsigned long long)(65535 - (row - c0)) << 7) | (unsigned long long)myslot;
-                        if (kk > key) { key = kk; rb = r; }
-                    }
+                    const double a = cabs1(v[r][q]);
+                    if (row >= j && row < ne && (a > ba || a != a)) { ba = a; rb = r; }   // a NaN entry is taken, kept and flagged
                 }
+                unsigned long long key = 0ull;
+                if (ba >= 0.0 || ba != ba)
+                    key = ((unsigned long long)__double_as_longlong(ba) & ~0x7FFFFFull) |
+                          ((unsigned long long)(65535 - (g0 + rb * TT)) << 7) | (unsigned long long)myslot;
                 c128 vq = v[0][q];
 #pragma unroll
                 for (int r = 1; r < R; ++r) if (r == rb) vq = v[r][q];
