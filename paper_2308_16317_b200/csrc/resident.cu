@@ -18,8 +18,9 @@
 //         (cp.async.bulk.shared::cluster.shared::cta), completion counted on an mbarrier of the RECEIVING CTA; a
 //         receiver declares its panel buffer free by a release-store of a flag into the next owner's shared memory,
 //         which the owner polls before it copies -- no cluster-wide barrier inside the loop
-//     R3  every CTA, its own trailing columns: the panel's interchanges and the 8 x 8 unit-lower solve, one thread per
-//         column (rows of U -> a small operand buffer and, for the verification export, to global memory)
+//     R3  every CTA, its own trailing columns: the panel's interchanges as ONE net row permutation (eight threads per
+//         column) and the 8 x 8 unit-lower solve (rows of U -> a small operand buffer and, for the verification
+//         export, to global memory)
 //     R4  rank-8 update of its trailing columns on the FP64 tensor pipe (DMMA.8x8x4 from shared memory; operand
 //         strides chosen conflict-free: ld = 1, ldp = 2, ldu = 4 (mod 8) complex units)
 //   K5  the trailing k x k block goes to global memory and rank 0 inverts it (final_inverse_small).
