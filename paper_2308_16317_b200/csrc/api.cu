@@ -376,7 +376,7 @@ using namespace lsms;
 
 extern "C" {
 
-const char* lsms_version(void) { return "lsms_tau 0.2 (sm_100a; DMMA.8x8x4 Schur update, TMA-staged; small-matrix mode)"; }
+const char* lsms_version(void) { return "lsms_tau 0.3 (sm_100a; DMMA.8x8x4 Schur update, TMA-staged; on-chip cluster mode for small matrices)"; }
 
 int lsms_create(lsms_handle_t* handle_out) {
     if (!handle_out) return -1;
