@@ -99,9 +99,12 @@ k_panel_post(const c128* __restrict__ base, size_t stride, int n, int J, int W, 
 // ---------------------------------------------------------------- K3b: apply the net row permutation
 // to the trailing columns [col_lo, col_hi): the new top block (rows J..J+W) goes, packed with ld = nbmax,
 // to tperm (the B operand of the TRSM-GEMM that writes U12 back into the matrix); displaced original top
-// rows are scattered to their final rows below.  One CTA per strip of PERM_TN columns.
-constexpr int PERM_TN = 16, PERM_THREADS = 256;
+// rows are scattered to their final rows below.  One CTA per strip of PERM_TN columns: 16 for matrices of up to ~4000
+// rows, 8 for taller ones, whose scattered row accesses of a strip span more DRAM pages (measured, K3a + K3b per step:
+// H (6750 rows) 26.5 -> 24.0 ms with 8 columns; M (880) 2.9 -> 3.2 and P (2160) 5.8 -> 5.8, so those keep 16).
+constexpr int PERM_THREADS = 256;
 
+template <int PERM_TN>
 __global__ void __launch_bounds__(PERM_THREADS)
 k_row_permute(c128* __restrict__ base, size_t stride, int n, int J, int W, int col_lo, int col_hi,
               const int* __restrict__ perm_all, c128* __restrict__ tperm_all, size_t tperm_stride, int nbmax) {
@@ -206,12 +209,17 @@ int launch_panel_post(const c128* base, size_t stride, int n, int J, int W, int 
 int launch_row_permute(c128* base, size_t stride, int n, int J, int W, int col_lo, int col_hi, int batch, const int* perm,
                        c128* tperm, size_t tperm_stride, int nbmax, cudaStream_t st) {
     if (col_hi <= col_lo) return 0;
-    size_t smem = (size_t)PERM_TN * W * sizeof(c128) + (1 + 3 * (size_t)W) * sizeof(int);
+    const int tn = n > 4000 ? 8 : 16;
+    size_t smem = (size_t)tn * W * sizeof(c128) + (1 + 3 * (size_t)W) * sizeof(int);
     for (int b0 = 0; b0 < batch; b0 += 65535) {
         int nb = batch - b0 < 65535 ? batch - b0 : 65535;
-        dim3 grid((col_hi - col_lo + PERM_TN - 1) / PERM_TN, nb);
-        k_row_permute<<<grid, PERM_THREADS, smem, st>>>(base + (size_t)b0 * stride, stride, n, J, W, col_lo, col_hi,
-                                                       perm + (size_t)b0 * (4 + 3 * nbmax), tperm + (size_t)b0 * tperm_stride, tperm_stride, nbmax);
+        dim3 grid((col_hi - col_lo + tn - 1) / tn, nb);
+        if (tn == 8)
+            k_row_permute<8><<<grid, PERM_THREADS, smem, st>>>(base + (size_t)b0 * stride, stride, n, J, W, col_lo, col_hi,
+                                                              perm + (size_t)b0 * (4 + 3 * nbmax), tperm + (size_t)b0 * tperm_stride, tperm_stride, nbmax);
+        else
+            k_row_permute<16><<<grid, PERM_THREADS, smem, st>>>(base + (size_t)b0 * stride, stride, n, J, W, col_lo, col_hi,
+                                                               perm + (size_t)b0 * (4 + 3 * nbmax), tperm + (size_t)b0 * tperm_stride, tperm_stride, nbmax);
         LSMS_LAUNCH_CHECK();
     }
     return 0;
