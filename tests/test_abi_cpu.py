@@ -44,6 +44,10 @@ def test_handle_options_and_workspace_queries():
     assert L.lsms_set_option(h.ptr, lt.LSMS_OPT_NB_OUTER, 63) == -3 and L.lsms_set_option(h.ptr, lt.LSMS_OPT_IB_INNER, 17) == -3
     assert L.lsms_set_option(h.ptr, 99, 0) == -2 and L.lsms_set_option(None, 0, 0) == -1
     assert L.lsms_set_option(h.ptr, lt.LSMS_OPT_PANEL_CLUSTER, 3) == -3 and L.lsms_set_option(h.ptr, lt.LSMS_OPT_GROUPS, 9) == -3
+    assert L.lsms_set_option(h.ptr, lt.LSMS_OPT_SMALL_MODE, 8) == -3 and L.lsms_set_option(h.ptr, lt.LSMS_OPT_PANEL_THREADS, 3) == -3
+    h.set("small_mode", 7).set("panel_threads", 2)                       # on-chip mode forced; quarter-SM panel kernel
+    assert h.get("small_mode") == 7 and h.get("panel_threads") == 2
+    h.set("small_mode", 0).set("panel_threads", 1)
     w64 = lt.lsms_workspace_bytes(h, 135, 3, False, 128)
     assert w64 >= 128 * 2160 * 4
     h.set("nb_outer", 32)
