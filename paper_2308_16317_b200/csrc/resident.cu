@@ -13,19 +13,23 @@
 //         each (every warp publishes its arg-max candidate -- found by two redux.sync on a 64-bit key -- TOGETHER
 //         with that row's entries and the reciprocal of the would-be pivot, so the winner's row is already in shared
 //         memory when the barrier opens); rows never move between threads, each thread tracks the position of its
-//         row in the pivoted arrangement; result -> the owner's panel buffer
-//     R2  the panel buffer is sent to the other CTAs by the TMA engine: bulk copies shared -> remote shared
-//         (cp.async.bulk.shared::cluster.shared::cta), completion counted on an mbarrier of the RECEIVING CTA; a
-//         receiver declares its panel buffer free by a release-store of a flag into the next owner's shared memory,
-//         which the owner polls before it copies -- no cluster-wide barrier inside the loop
+//         row in the pivoted arrangement; result -> staged in the panel's own (now dead) columns of the matrix
+//     R2  the staged panel is sent to the other CTAs' panel buffers by the TMA engine: bulk copies shared -> remote
+//         shared (cp.async.bulk.shared::cluster.shared::cta), completion counted on an mbarrier of the RECEIVING CTA.
+//         A receiver declares its panel buffer free by a release-store of a flag into the next owner's shared memory;
+//         the owner's warp 15 (the "shipper") polls the flags and serves each CTA as soon as it is free, the next
+//         owner first -- no cluster-wide barrier inside the loop, and nobody waits for a CTA that is behind
 //     R3  every CTA, its own trailing columns: the panel's interchanges as ONE net row permutation (eight threads per
 //         column) and the 8 x 8 unit-lower solve (rows of U -> a small operand buffer and, for the verification
 //         export, to global memory)
 //     R4  rank-8 update of its trailing columns on the FP64 tensor pipe (DMMA.8x8x4 from shared memory; operand
 //         strides chosen conflict-free: ld = 1, ldp = 2, ldu = 4 (mod 8) complex units)
 //   K5  the trailing k x k block goes to global memory and rank 0 inverts it (final_inverse_small).
-// LOOK-AHEAD: the CTA that owns panel p+1 updates that block first (R3, R4 on its 8 columns), then half of its warps
-// factor panel p+1 (R1) while the other half -- and the other CTAs -- finish step p.
+// LOOK-AHEAD: the CTA that owns panel p+1 updates that block first (R3, R4 on its 8 columns) and factors panel p+1 (R1)
+// at once, with its SM to itself, while the other CTAs finish step p.  It catches up on step p for its other columns
+// only after panel p+1 is on its way (its own panel buffer still holds panel p): warps 0-14 do that while warp 15 ships
+// -- off the critical path, while the next owner works.  Measured chain per panel (208^2, first -> last): ship 1.0 ->
+// 0.65 us, block update 1.7 -> 1.45, R1 3.6 -> 2.8, staging 0.7 -> 0.55: 7.0 -> 5.5 us.
 //
 // Global traffic: the matrix is read once (TMA bulk loads, one per column); U and the final block are written once.
 #include "common.cuh"
@@ -112,11 +116,12 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
     c128* Aloc = reinterpret_cast<c128*>(rsm);
     c128* Lbuf = reinterpret_cast<c128*>(rsm + L.off_L);
     int* spiv = reinterpret_cast<int*>(rsm + L.off_piv);
+    int* spiv2 = spiv + 32;                              // staging copy of the next panel's permutation
     c128* Ubuf = reinterpret_cast<c128*>(rsm + L.off_U);
     unsigned char* red = rsm + L.off_red;
     uint64_t* bar_load = reinterpret_cast<uint64_t*>(rsm + L.off_bar);
     uint64_t* bar_full = bar_load + 1;
-    int* ready = reinterpret_cast<int*>(bar_load + 2);   // ready[r], written by CTA r: r's panel buffer may receive panel ready[r]
+    int* ready = reinterpret_cast<int*>(bar_load + 2);   // ready[r] (written by CTA r): r's panel buffer may receive panel ready[r]
     const int ld = L.ld, ldp = L.ldp;
 
     const int item = blockIdx.x / ncl;
@@ -138,6 +143,7 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
     // padding columns of a ragged last block and the U buffer start as zeros
     for (int lc = tid; lc < my_cols; lc += RS_T) if (gcol(lc) >= n) for (int r = 0; r < ld; ++r) Aloc[(size_t)lc * ld + r] = cmake(0.0, 0.0);
     for (int e = tid; e < L.ncols_max * RS_LDU; e += RS_T) Ubuf[e] = cmake(0.0, 0.0);
+    for (int e = tid; e < RW * ldp + 32; e += RS_T) Lbuf[e] = cmake(0.0, 0.0);      // incl. the permutation ints and the slack behind them
     asm volatile("fence.proxy.async;" ::: "memory");
     __syncthreads();
     // ---- the CTA's column blocks -> shared memory: one TMA bulk copy per column
@@ -250,17 +256,26 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
         const int c0 = p * RW, wv = min(RW, ne - c0), m = n - c0;
         const int lcp = (p / ncl) * RW;
         if (tid < m) {
+            // staging area = the panel's own columns of the matrix (dead once they are in registers); columns beyond wv
+            // of a ragged last panel hold live central entries: they are not part of L and are stored where they belong
 #pragma unroll
-            for (int c = 0; c < RW; ++c) {
-                Lbuf[(size_t)c * ldp + pos] = (c < wv) ? v[c] : cmake(0.0, 0.0);
-                if (c >= wv) Aloc[(size_t)(lcp + c) * ld + c0 + pos] = v[c];
-            }
-            if (pos < wv) spiv[RW + pos] = c0 + tid;
+            for (int c = 0; c < RW; ++c) Aloc[(size_t)(lcp + c) * ld + c0 + pos] = v[c];
+            if (pos < wv) spiv2[RW + pos] = c0 + tid;
             if (tid < RW) {
-                spiv[2 * RW + tid] = (tid < wv && pos >= wv) ? c0 + pos : -1;
-                if (tid >= wv) spiv[RW + tid] = c0 + tid;          // positions of a ragged last panel that are no pivots
+                spiv2[2 * RW + tid] = (tid < wv && pos >= wv) ? c0 + pos : -1;
+                if (tid >= wv) spiv2[RW + tid] = c0 + tid;         // positions of a ragged last panel that are no pivots
             }
         }
+    };
+    // staged panel -> this CTA's own panel buffer (the other CTAs get it by bulk copy)
+    auto panel_to_lbuf = [&](int p) {
+        const int c0 = p * RW, wv = min(RW, ne - c0), m = n - c0;
+        const int lcp = (p / ncl) * RW;
+        for (int e = tid; e < RW * m; e += RS_T) {
+            const int c = e / m, r = e % m;
+            Lbuf[(size_t)c * ldp + r] = (c < wv) ? Aloc[(size_t)(lcp + c) * ld + c0 + r] : cmake(0.0, 0.0);
+        }
+        if (tid < 3 * RW) spiv[tid] = spiv2[tid];
     };
     // ... -> global memory (off the critical path: after the panel has been shipped): pivot vector, status, and the rows
     // of U held by this block for the verification export (k_backsolve_central reads U11, U12)
@@ -351,75 +366,89 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
         }
     };
 
-    // this CTA has finished reading panel q-1 from its panel buffer: arm the mbarrier for panel q and tell q's owner
+    // ship panel p (staged in its own columns) to the CTAs rank+d_lo .. rank+d_hi-1 (mod ncl), each as soon as IT has
+    // declared its panel buffer free -- no cluster-wide barrier: the next owner, which is served first, never waits for
+    // a CTA that is still catching up
+    auto ship = [&](int p, int d_lo, int d_hi) {
+        const int c0 = p * RW, wv = min(RW, ne - c0), m = n - c0, lcp = (p / ncl) * RW;
+        if (tid >= RS_T - 32 && tid < RS_T - 32 + RW + 1) {          // the shipper: warp 15
+            const int c = tid - (RS_T - 32);
+            for (int d = d_lo; d < d_hi; ++d) {
+                const uint32_t dst = (uint32_t)((rank + d) % ncl);
+                while (rs_ld_acquire(&ready[dst]) < p) {}
+                const uint32_t rbar = rs_mapa(smem_u32(bar_full), dst);
+                if (c < wv) rs_bulk_s2r(rs_mapa(smem_u32(Lbuf + (size_t)c * ldp), dst), smem_u32(Aloc + (size_t)(lcp + c) * ld + c0), (uint32_t)(m * sizeof(c128)), rbar);
+                else if (c == RW) rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv2), (uint32_t)(3 * RW * sizeof(int)), rbar);
+            }
+        }
+    };
+    // this CTA is done with the panel buffer's content: arm the mbarrier for panel q and tell q's owner
     auto declare_free = [&](int q) {
         if (q < np && q % ncl != rank && tid == 0) {
-            const int mq = n - q * RW;
-            mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * mq * sizeof(c128) + 3 * RW * sizeof(int)));
+            const int mq = n - q * RW, wq = min(RW, ne - q * RW);
+            mbar_expect_tx(bar_full, (uint32_t)((size_t)wq * mq * sizeof(c128) + 3 * RW * sizeof(int)));
             rs_st_release_remote(rs_mapa(smem_u32(&ready[rank]), (uint32_t)(q % ncl)), q);
         }
     };
+
     if (np > 0 && rank == 0) panel_factor(0);            // the first panel has nothing to hide behind
-    if (np > 0 && rank != 0 && tid == 0) mbar_expect_tx(bar_full, (uint32_t)((size_t)RW * n * sizeof(c128) + 3 * RW * sizeof(int)));
-    if (ncl > 1) rs_cluster_sync();                      // every receiver is armed for panel 0 (ready[] = 0 everywhere)
+    if (np > 0 && rank != 0 && tid == 0) {               // (ready[] = 0 everywhere since before the start-up cluster barrier)
+        const int wq = min(RW, ne);
+        mbar_expect_tx(bar_full, (uint32_t)((size_t)wq * n * sizeof(c128) + 3 * RW * sizeof(int)));
+    }
+    if (ncl > 1) rs_cluster_sync();                      // every receiver is armed for panel 0
     for (int p = 0; p < np; ++p) {
-        const int m = n - p * RW;
         const int owner = p % ncl;
+        const int lcp = (p / ncl) * RW;
         if (rank == owner) {
             panel_publish(p);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncthreads();
             R_TOC(1);
             R_STAMP(p, 0);
-            // ================= R2: ship the panel -- to each CTA as soon as IT has declared its panel buffer free (a flag
-            // it stores, with release semantics, into this CTA's shared memory): no cluster-wide barrier on the critical
-            // path.  The CTA that owns the NEXT panel is served first.
-            if (ncl > 1 && tid < RW + 1) {
-                const int c = tid;
-                for (int d = 1; d < ncl; ++d) {
-                    const uint32_t dst = (uint32_t)((rank + d) % ncl);
-                    while (rs_ld_acquire(&ready[dst]) < p) {}
-                    const uint32_t rbar = rs_mapa(smem_u32(bar_full), dst);
-                    if (c < RW) rs_bulk_s2r(rs_mapa(smem_u32(Lbuf + (size_t)c * ldp), dst), smem_u32(Lbuf + (size_t)c * ldp), (uint32_t)(m * sizeof(c128)), rbar);
-                    else rs_bulk_s2r(rs_mapa(smem_u32(spiv), dst), smem_u32(spiv), (uint32_t)(3 * RW * sizeof(int)), rbar);
-                }
+            // ================= R2 and, off the critical path, the catch-up: warp 15 ships the panel -- next owner first, each
+            // CTA as soon as it has declared its panel buffer free -- while warps 0-14 do the part of the PREVIOUS step that
+            // this CTA put off while it factored panel p (panel p-1 through its columns right of block p); then panel p goes
+            // into this CTA's own panel buffer
+            if (warp == RS_T / 32 - 1) {
+                if (ncl > 1) ship(p, 1, ncl);
+            } else if (p > 0) {
+                swap_solve(p - 1, lcp + RW, my_cols, 0, RS_T - 32);
+                asm volatile("bar.sync 5, %0;" ::"r"(RS_T - 32) : "memory");
+                rank8_update(p - 1, lcp + RW, my_cols, 0, RS_T / 32 - 1);
             }
             R_STAMP(p, 1);
+            __syncthreads();
+            panel_to_lbuf(p);
+            panel_export(p);
+            __syncthreads();
         } else {
             mbar_wait(bar_full, full_parity); full_parity ^= 1;
             if ((p + 1) % ncl == rank) R_STAMP(p, 2);
         }
-        if (rank == owner) panel_export(p);
         R_TOC(2);
         const int tl0 = (p >= rank) ? ((p - rank) / ncl + 1) * RW : 0;          // first local column right of block p
         if (p + 1 < np && (p + 1) % ncl == rank) {
             // ---- LOOK-AHEAD: this CTA owns the next panel, whose factorisation is the critical path (8 dependent pivot
-            // steps).  Warps 0-7 bring its block (local columns [tl0, tl0+8)) up to date and factor it while warps 8-15
-            // take panel p through the CTA's other columns.
-            if (tid < RS_PT) {
-                swap_solve(p, tl0, tl0 + RW, 0, RS_PT);
-                asm volatile("bar.sync 3, %0;" ::"r"(RS_PT) : "memory");
-                rank8_update(p, tl0, tl0 + RW, 0, RS_PT / 32);
-                asm volatile("bar.sync 3, %0;" ::"r"(RS_PT) : "memory");
-                R_TOC(4);
-                R_STAMP(p, 3);
-                panel_factor(p + 1);
-                R_STAMP(p, 4);
-            } else {
-                swap_solve(p, tl0 + RW, my_cols, RS_PT, RS_T - RS_PT);
-                asm volatile("bar.sync 2, %0;" ::"r"(RS_T - RS_PT) : "memory");
-                rank8_update(p, tl0 + RW, my_cols, RS_PT / 32, (RS_T - RS_PT) / 32);
-            }
-            R_TOC(5);
+            // steps): it brings that block (local columns [tl0, tl0+8)) up to date and factors it at once, with the SM to
+            // itself; panel p's update of its other columns waits until panel p+1 has been shipped (above).
+            swap_solve(p, tl0, tl0 + RW, 0, RS_T);
             __syncthreads();
-            R_TOC(6);
+            rank8_update(p, tl0, tl0 + RW, 0, RS_T / 32);
+            __syncthreads();
+            R_TOC(4);
+            R_STAMP(p, 3);
+            panel_factor(p + 1);
+            R_STAMP(p, 4);
+            R_TOC(5);
         } else {
             swap_solve(p, tl0, my_cols, 0, RS_T);
             __syncthreads();
             rank8_update(p, tl0, my_cols, 0, RS_T / 32);
+            __syncthreads();
+            declare_free(p + 1);
         }
         __syncthreads();
-        declare_free(p + 1);
         R_TOC(3);
     }
     // ================= K5: the trailing k x k block -> global memory, inverted by rank 0
