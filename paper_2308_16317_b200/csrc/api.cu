@@ -322,9 +322,10 @@ static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
     const int rcl = resident_cluster_size(n, k);
     if (sm == 7) return rcl > 0 ? -rcl : 0;
     // Default for matrices that fit on chip (n <= ~216 with 4 SMs each), while the batch needs at most ~3.5 waves of
-    // clusters: the on-chip kernel is built for latency (208^2 x 32: 0.25 ms against 0.56 ms through L2 and 0.85 ms in
+    // clusters: the on-chip kernel is built for latency (208^2 x 32: 0.20 ms against 0.56 ms through L2 and 0.85 ms in
     // lock-step), but it holds 4 SMs per matrix for the whole elimination, and from ~150 matrices of 208^2 on the
-    // lock-step schedule has the higher throughput (1024 matrices: 3.5 ms against 6.4 ms on chip).
+    // lock-step schedule has the higher throughput (128 matrices: 0.71 ms on chip, 0.78 lock-step; 192: 1.05 / 0.90;
+    // 512: 2.72 / 1.64).
     if (sm == 0 && rcl > 0 && 2LL * batch * rcl <= 7LL * c->sms) return -rcl;
     if (sm == 0) return 0;
     if (!fused_supported(n, k, eff_nb(c), eff_ib(c))) return 0;
