@@ -555,6 +555,30 @@ def test_scheduler_leaves_the_on_chip_mode_when_the_batch_needs_many_waves_of_cl
         check_tau(tau_oc[b], lapack_tau00(A[b], kmax), 1e-11, ("on chip vs LAPACK", b))
 
 
+def test_on_chip_mode_repeated_launches_are_bitwise_reproducible(lt, h):
+    """The on-chip kernel synchronises its CTAs with flags, mbarriers and a polling "shipper" warp instead of cluster
+    barriers: many launches in a row, batches of one wave and of several, cluster sizes 1 / 2 / 4 / 8 -- every launch
+    must return, and return the same bits (the schedule inside the cluster must not leak into the arithmetic)."""
+    h.set("small_mode", 7)
+    for n_sites, kmax, canted, B in ((13, 16, False, 32), (13, 16, False, 150), (7, 9, False, 64), (33, 4, False, 40),
+                                     (27, 4, True, 20), (2, 25, True, 9), (16, 1, False, 300)):
+        k = kmax * (2 if canted else 1)
+        A = sl.random_dense_matrices(B, n_sites * k, seed=77 + n_sites)
+        M0 = torch.from_numpy(A).cuda()
+        first = None
+        for rep in range(25):
+            tau, info = lt.lsms_tau00_batched(h, M0.clone(), n_sites, kmax, canted, B)
+            if first is None:
+                first = tau.clone()
+            else:
+                assert torch.equal(torch.view_as_real(tau), torch.view_as_real(first)), (n_sites, kmax, rep)
+        torch.cuda.synchronize()
+        assert lt.lsms_last_schedule(h) > 100 and not info.cpu().numpy().any()
+        t = first.cpu().numpy().transpose(0, 2, 1)
+        for b in range(0, B, max(1, B // 5)):
+            check_tau(t[b], lapack_tau00(A[b], k), 1e-11, (n_sites, kmax, b))
+
+
 # ------------------------------------------------------------------ boundary: re-entrancy and input validation
 
 def test_two_host_threads_two_handles_two_streams(lt):
