@@ -19,7 +19,8 @@
  *   - Rydberg atomic units: kappa = sqrt(z), Im kappa >= 0, lengths in Bohr
  *
  * State and threads ("the library owns nothing persistent ... re-entrant on different
- * streams").  There is NO process-wide state.  Everything a call needs beyond its arguments lives in an opaque
+ * streams").  There is NO process-wide state (one exception, described where it is declared: the built-in scratch
+ * array of lsms_tau00_onchip_static_scratch).  Everything a call needs beyond its arguments lives in an opaque
  * handle the caller creates and destroys: the scheduler options and the auxiliary streams and events of the batch
  * scheduler (look-ahead and batch-group streams).  A handle is bound to the device that is current at its first call
  * that enqueues work; a later call made while another device is current returns cudaErrorInvalidDevice (101).  One handle serves
@@ -27,7 +28,8 @@
  * host threads on different streams (the paper's callers are many MPI ranks sharing a GPU).
  *
  * Pointers are DEVICE pointers unless the name ends in _host.  The caller owns every buffer, including the
- * workspace; the library allocates no device memory.  All device work is ordered after what is already enqueued
+ * workspace; the library allocates no device memory (its device image holds one fixed 256 KB array, see
+ * lsms_tau00_onchip_static_scratch).  All device work is ordered after what is already enqueued
  * on `cuda_stream` (a cudaStream_t passed as void*), later work on `cuda_stream` is ordered after it, and the calls
  * return without synchronising (the *_host entry point synchronises the stream before returning because it hands
  * results back in host memory).
@@ -170,6 +172,38 @@ int lsms_build_M_shared_g0_batched(lsms_handle_t handle, const lsms_c128* tinv_d
 int lsms_tau00_batched(lsms_handle_t handle, lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
                        lsms_c128* tau00_out, int* info,
                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* tau^{00} of a batch of SMALL matrices for a caller that cannot give the library any device workspace and cannot
+ * allocate one (eq. (4), :62; the on-chip schedule of lsms_tau00_batched, LSMS_OPT_SMALL_MODE = 7).
+ *
+ * For whom: the paper's callers are Fortran MPI ranks that go through a C interface and share a GPU (PAPER.md:88-92,
+ * :110).  A rank that sized all of its device buffers at start-up has no spare memory inside the energy loop; a
+ * cudaMalloc there can fail because the other ranks hold the rest of the GPU, and it stalls the device for all of them.
+ * Likewise a host code whose device memory belongs to another runtime (OpenACC / OpenMP data regions, a pool) can pass
+ * matrices and result blocks but has no way to ask for workspace.  This call needs none: it takes no handle and no
+ * workspace, and it calls no cudaMalloc / cudaFree and creates no stream or event.  The one piece of global memory the
+ * kernel needs beyond its arguments -- a pivot word per matrix row -- is a fixed array of LSMS_STATIC_SCRATCH_WORDS
+ * 32-bit words (256 KB) built into the library, which every GPU that loads the library holds until the process exits.
+ *
+ *   M         [batch][n*n]  column-major, OVERWRITTEN (factorised in place), n = n_sites*k, k = kmax*(1+spin_canted);
+ *                           n must fit the on-chip kernel: n <= 256 and the matrix within the shared memory of 8 SMs
+ *                           (n <= ~216 for complex128), else LSMS_ERR_NOT_ON_CHIP
+ *   batch                   batch * n <= LSMS_STATIC_SCRATCH_WORDS, else LSMS_ERR_STATIC_SCRATCH_TOO_SMALL
+ *   tau00_out [batch][k*k]  column-major (out);   info [batch] (out) as for lsms_tau00_batched
+ * Both size limits are checked on the host before any CUDA call.  Results are those of lsms_tau00_batched in on-chip
+ * mode (same kernel, same launch shape).
+ * First call on a device: it looks up the array's address on that device and opts the kernel into its shared-memory
+ * size (once per device, remembered inside the library, thread-safe).  Make that first call outside any stream capture.
+ * Sharing: every call on a device uses the same array, whatever the stream or host thread.  Calls that overlap on the
+ * GPU overwrite each other's pivot words -- order them (one stream, or events).  The array keeps the last call's
+ * contents; nothing in it needs clearing, the kernel writes a matrix's pivot words before anything reads them.
+ * Errors: -1 M, -2 n_sites, -3 kmax, -5 batch, -6 tau00_out, -7 info (null or not 16-byte aligned where complex),
+ * LSMS_ERR_NOT_ON_CHIP, LSMS_ERR_STATIC_SCRATCH_TOO_SMALL; >0 CUDA error code.                                  */
+#define LSMS_STATIC_SCRATCH_WORDS 65536
+#define LSMS_ERR_NOT_ON_CHIP (-20)
+#define LSMS_ERR_STATIC_SCRATCH_TOO_SMALL (-21)
+int lsms_tau00_onchip_static_scratch(lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
+                                     lsms_c128* tau00_out, int* info, void* cuda_stream);
 
 /* Verification only (not on the timed path): the whole central block column X = M^{-1} E,
  * E = last k columns of I_n, for the residual test ||M X - E|| ("solving X'X = I").

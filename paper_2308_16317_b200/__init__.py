@@ -25,6 +25,7 @@ EXPORTS = (
     "lsms_workspace_bytes", "lsms_solve_workspace_bytes", "lsms_host_call_scratch_bytes",
     "lsms_tinv_from_phase_shifts", "lsms_build_M_batched", "lsms_build_M_shared_g0_batched", "lsms_tau00_batched",
     "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_contour_sum_batched",
+    "lsms_tau00_onchip_static_scratch",
     # include/lsms_tau_diag.h -- measurement and debugging
     "lsms_last_launch_count", "lsms_last_schedule", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe",
     "lsms_schur_update_batched", "lsms_debug_gaunt_closed_form",
@@ -71,6 +72,7 @@ def lib() -> ctypes.CDLL:
         L.lsms_build_M_shared_g0_batched.argtypes = [vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, vp, vp, vp, sz, vp]
         L.lsms_tau00_batched.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp, vp, sz, vp]
         L.lsms_solve_central_column_batched.argtypes = [vp, vp, ci, ci, ci, ci, vp, vp, vp, sz, vp]
+        L.lsms_tau00_onchip_static_scratch.argtypes = [vp, ci, ci, ci, ci, vp, vp, vp]
         L.lsms_tau00_from_host.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, vp, vp, vp, sz, vp,
                                            ctypes.POINTER(sz), ctypes.POINTER(sz)]
         L.lsms_contour_sum_batched.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp]
@@ -294,6 +296,33 @@ def lsms_tau00_batched(handle: Handle, M, n_sites, kmax, spin_canted, batch, tau
         workspace = _workspace(lsms_workspace_bytes(handle, n_sites, max(lmax, 0), spin_canted, batch), M.device)
     _check(lib().lsms_tau00_batched(handle.ptr, _ptr(M), n_sites, kmax, int(bool(spin_canted)), batch, _ptr(tau00_out),
                                     _ptr(info), _ptr(workspace), workspace.numel(), _stream(stream)), "lsms_tau00_batched")
+    return tau00_out, info
+
+
+LSMS_STATIC_SCRATCH_WORDS = 65536            # include/lsms_tau.h
+LSMS_ERR_NOT_ON_CHIP, LSMS_ERR_STATIC_SCRATCH_TOO_SMALL = -20, -21
+
+
+def lsms_tau00_onchip_static_scratch(M, n_sites, kmax, spin_canted, batch, tau00_out, info, stream=None):
+    """tau00 of a batch of small matrices for callers that cannot allocate device memory (ranks that share a GPU and
+    sized their buffers at start-up; host codes whose device memory another runtime owns): no handle, no workspace.
+    The pivot scratch is a fixed 256 KB array inside the library, so batch * n <= LSMS_STATIC_SCRATCH_WORDS and the
+    matrix must fit the on-chip kernel (n <= ~216).  Nothing is allocated here either: M (overwritten), tau00_out
+    [batch, k, k] and info [batch] are the caller's tensors.  All calls on a device share the scratch array: do not let
+    two of them overlap on the GPU.  Make the first call on a device outside any stream capture."""
+    for name, t in (("M", M), ("tau00_out", tau00_out), ("info", info)):
+        if t is None:
+            raise LsmsError(f"lsms_tau00_onchip_static_scratch: {name} must be given (this call allocates nothing)")
+    rc = lib().lsms_tau00_onchip_static_scratch(_ptr(M), n_sites, kmax, int(bool(spin_canted)), batch, _ptr(tau00_out),
+                                                _ptr(info), _stream(stream))
+    k = kmax * (2 if spin_canted else 1)
+    if rc == LSMS_ERR_NOT_ON_CHIP:
+        raise LsmsError(f"lsms_tau00_onchip_static_scratch: a {n_sites * k} x {n_sites * k} matrix does not fit the on-chip "
+                        "kernel (n <= ~216); use lsms_tau00_batched with a workspace")
+    if rc == LSMS_ERR_STATIC_SCRATCH_TOO_SMALL:
+        raise LsmsError(f"lsms_tau00_onchip_static_scratch: batch * n = {batch * n_sites * k} exceeds the built-in scratch of "
+                        f"{LSMS_STATIC_SCRATCH_WORDS} words; split the batch or use lsms_tau00_batched with a workspace")
+    _check(rc, "lsms_tau00_onchip_static_scratch")
     return tau00_out, info
 
 
