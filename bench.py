@@ -469,7 +469,7 @@ class Bench:
                                      f"{16.0 * n * n * B / 1e6:.1f} MB of M per step: L2-resident by design (small-matrix mode); M is re-assembled every step"),
                        "parallelism": f"batch sharded by central atom over {world} GPU(s), no data-path collective; "
                                       f"{gathered} tau00 blocks gathered after the timed region"},
-            "tflops": tflops, "tflops_convention": "8/3 n^3 per matrix",
+            "n": n, "batch": B, "tflops": tflops, "tflops_convention": "8/3 n^3 per matrix",
             "frac_fp64_peak": tflops / peak_fp64 if peak_fp64 else None,
             "schedule": {"mode": ("on-chip small-matrix mode, cluster of %d CTA(s) (SMs) per matrix, one launch" % (schedule_used - 100)) if schedule_used > 100
                          else ("small-matrix mode through L2, %d CTA(s) per matrix, one launch" % schedule_used) if schedule_used > 0
@@ -487,7 +487,9 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="P,C,M,T", help="comma-separated workloads; the first is the top-level JSON line")
+    ap.add_argument("--workload", default="P,C,M,T,H,N,NC",
+                    help="comma-separated workloads; the first is the top-level JSON line, the others go under per_workload; "
+                         "every one of them appears in the compact `summary` that ends the line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--nb", type=int, default=0, help="outer panel width override (0 = library default)")
     ap.add_argument("--ib", type=int, default=0, help="inner panel width override")
@@ -512,12 +514,29 @@ def main() -> None:
 
     bench = Bench(args)
     results = {}
+    steps = args.steps
     for i, key in enumerate(keys):
+        # secondary lines of the tall workloads (H, N, NC: 0.5 - 2 s per step): at most five timed steps each, so that the
+        # default run stays within a few minutes; every line states its own "steps"
+        args.steps = min(steps, 5) if (i > 0 and sl.CONFIGS[key].n > 5000) else steps
         results[key] = bench.run(key, with_cpu_baseline=not args.no_cpu_baseline)
+    args.steps = steps
     if bench.rank == 0:
         line = dict(results[keys[0]])
         if len(keys) > 1:
             line["per_workload"] = {k: results[k] for k in keys[1:]}
+        # the LAST key of the line: one compact record per workload (a reader that keeps only the tail of stdout still
+        # sees every configuration: ms per step, tau00/s, whole-step and dominant-kernel fractions of the FP64 tensor
+        # peak, K1's fraction of the HBM copy rate, end-to-end ms, parity of the timed run)
+        def compact(r):
+            par, roof = r["parity"] or {}, r["roofline"] or {}
+            rnd = lambda v, d: None if v is None else round(v, d)
+            sci = lambda v: None if v is None else float(f"{v:.1e}")
+            return {"ms": rnd(r["ms_per_step"], 3), "tau00_s": rnd(r["value"], 2),
+                    "frac_peak": rnd(r["frac_fp64_peak"], 3), "k_frac": rnd(roof.get("frac"), 3),
+                    "k1_hbm": rnd(roof.get("k1_assembly_frac_of_hbm"), 3), "e2e_ms": rnd(r["e2e"]["ms_per_step"], 3),
+                    "parity_ok": par.get("ok"), "rel_fro": sci(par.get("max_rel_fro")), "res": sci(par.get("residual_max"))}
+        line["summary"] = {k: compact(results[k]) for k in keys}
         print(json.dumps(line))
         bad = [k for k in keys if results[k]["parity"] and not results[k]["parity"]["ok"]]
         if bad:

@@ -168,7 +168,13 @@ int lsms_build_M_shared_g0_batched(lsms_handle_t handle, const lsms_c128* tinv_d
  *   M         [batch][n*n]  OVERWRITTEN (factorised in place), n = n_sites*k, k = kmax*(1+spin_canted)
  *   tau00_out [batch][k*k]  column-major (out)
  *   info      [batch] (out) 0 ok; j>0 = zero or non-finite pivot met at elimination step j (1-based)
- * Errors: -1 handle, -2 M, -3 n_sites, -4 kmax, -6 batch, -7 tau00_out, -8 info, -9/-10 workspace.           */
+ * Size limit: n <= 16384 rows; one or two matrices per call may have up to 40960 rows (their panels are factored by a
+ * cluster of CTAs) unless LSMS_OPT_PANEL_CLUSTER / LSMS_OPT_PANEL_THREADS or the device rule that out.  Beyond it this
+ * call, lsms_solve_central_column_batched and lsms_tau00_from_host return LSMS_ERR_PANEL_TOO_TALL before enqueueing
+ * anything, and the workspace queries return 0.
+ * Errors: -1 handle, -2 M, -3 n_sites, -4 kmax, -6 batch, -7 tau00_out, -8 info, -9/-10 workspace,
+ * LSMS_ERR_PANEL_TOO_TALL.                                                                                    */
+#define LSMS_ERR_PANEL_TOO_TALL (-22)
 int lsms_tau00_batched(lsms_handle_t handle, lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
                        lsms_c128* tau00_out, int* info,
                        void* workspace, size_t workspace_bytes, void* cuda_stream);
@@ -200,7 +206,7 @@ int lsms_tau00_batched(lsms_handle_t handle, lsms_c128* M, int n_sites, int kmax
  * Errors: -1 M, -2 n_sites, -3 kmax, -5 batch, -6 tau00_out, -7 info (null or not 16-byte aligned where complex),
  * LSMS_ERR_NOT_ON_CHIP, LSMS_ERR_STATIC_SCRATCH_TOO_SMALL; >0 CUDA error code.                                  */
 #define LSMS_STATIC_SCRATCH_WORDS 65536
-#define LSMS_ERR_NOT_ON_CHIP (-20)
+#define LSMS_ERR_NOT_ON_CHIP (-20)              /* codes below -19 name a condition, not an argument position */
 #define LSMS_ERR_STATIC_SCRATCH_TOO_SMALL (-21)
 int lsms_tau00_onchip_static_scratch(lsms_c128* M, int n_sites, int kmax, int spin_canted, int batch,
                                      lsms_c128* tau00_out, int* info, void* cuda_stream);

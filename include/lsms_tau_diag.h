@@ -23,6 +23,14 @@ int lsms_last_launch_count(lsms_handle_t handle);
  * in the distributed shared memory of a cluster of c CTAs.  -1 before the first call. */
 int lsms_last_schedule(lsms_handle_t handle);
 
+/* How many thread-block clusters of `cluster_size` (1, 2, 4, 8) CTAs of a cluster kernel fit on the handle's device at
+ * once -- as this process sees it, so under MPS / MIG the answer is for its SM partition (cudaOccupancyMaxActiveClusters at the
+ * kernel's largest shared-memory size, asked once when the handle is bound).  kernel: 0 on-chip elimination
+ * (k_lu_resident), 1 one-launch elimination through L2 (k_lu_fused / k_lu_tiny), 2 cluster panel kernel (k_panel_clu;
+ * cluster_size 1 gives 0).  0 means the scheduler never picks that kernel with that cluster size on this device and
+ * uses the lock-step / one-CTA schedule instead.  Binds the handle.  Errors: -1 handle, -2 kernel, -3 cluster_size, -4 count_host. */
+int lsms_max_active_clusters(lsms_handle_t handle, int kernel, int cluster_size, int* count_host);
+
 /* Per-kernel-class timing.  Between lsms_profile_begin and lsms_profile_end every kernel enqueued through the
  * handle is bracketed by CUDA events on the stream it is launched on (the events belong to the handle and are
  * created on demand).  lsms_profile_end synchronises those events and returns, per class, the summed device time

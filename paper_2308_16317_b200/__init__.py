@@ -27,7 +27,7 @@ EXPORTS = (
     "lsms_solve_central_column_batched", "lsms_tau00_from_host", "lsms_contour_sum_batched",
     "lsms_tau00_onchip_static_scratch",
     # include/lsms_tau_diag.h -- measurement and debugging
-    "lsms_last_launch_count", "lsms_last_schedule", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe",
+    "lsms_last_launch_count", "lsms_last_schedule", "lsms_max_active_clusters", "lsms_profile_begin", "lsms_profile_end", "lsms_fp64_peak_probe",
     "lsms_schur_update_batched", "lsms_debug_gaunt_closed_form",
 )
 
@@ -78,6 +78,7 @@ def lib() -> ctypes.CDLL:
         L.lsms_contour_sum_batched.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp]
         L.lsms_last_launch_count.argtypes = [vp]
         L.lsms_last_schedule.argtypes = [vp]
+        L.lsms_max_active_clusters.argtypes = [vp, ci, ci, ctypes.POINTER(ci)]
         L.lsms_profile_begin.argtypes = [vp]
         L.lsms_profile_end.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_double)]
         L.lsms_fp64_peak_probe.argtypes = [vp, ci, ci, vp, ctypes.POINTER(ctypes.c_double), vp]
@@ -88,7 +89,13 @@ def lib() -> ctypes.CDLL:
     return _lib
 
 
+LSMS_ERR_PANEL_TOO_TALL = -22
+
+
 def _check(rc: int, what: str) -> None:
+    if rc == LSMS_ERR_PANEL_TOO_TALL:
+        raise LsmsError(f"{what}: the matrix has more rows than the panel kernels cover for this batch and these options "
+                        "(16384; 40960 for one or two matrices per call)")
     if rc != 0:
         raise LsmsError(f"{what} returned {rc} "
                         f"({'argument %d invalid' % -rc if rc < 0 else 'CUDA error code'})")
@@ -185,6 +192,13 @@ def lsms_last_schedule(handle: Handle) -> int:
     return int(lib().lsms_last_schedule(handle.ptr))
 
 
+def lsms_max_active_clusters(handle: Handle, kernel: int, cluster_size: int) -> int:
+    """kernel: 0 on-chip elimination, 1 one-launch elimination through L2, 2 cluster panel kernel."""
+    out = ctypes.c_int(-1)
+    _check(lib().lsms_max_active_clusters(handle.ptr, kernel, cluster_size, ctypes.byref(out)), "lsms_max_active_clusters")
+    return out.value
+
+
 KERNEL_CLASSES = ("K1_assemble", "K2_panel", "small_mode_lu", "K4_inner_gemm", "K4_schur_gemm", "K5_final_inverse",
                   "K3_permute_ninv", "K4_trsm_gemm")
 
@@ -215,14 +229,27 @@ def lsms_fp64_peak_probe(handle: Handle, which: int, iters: int = 20000, sink=No
     return out.value
 
 
-def _workspace(nbytes: int, device):
+def _empty(shape, dtype, device, stream=None):
+    """Buffers this module allocates on the caller's behalf (omitted outputs, the workspace) are allocated with `stream`
+    current -- the stream the library call runs on.  torch's caching allocator ties a block to the stream that was
+    current when it was allocated: a workspace dropped when the (asynchronous) call returns may then only be reused by
+    work ordered after the call on that same stream, never by another stream's work while the kernels still use it.
+    (The scheduler's own streams are forked from and joined back into `stream` inside the call.)"""
     import torch
-    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+    if stream is None:
+        return torch.empty(shape, dtype=dtype, device=device)
+    with torch.cuda.stream(stream):
+        return torch.empty(shape, dtype=dtype, device=device)
 
 
-def _info(batch, device):
+def _workspace(nbytes: int, device, stream=None):
     import torch
-    return torch.empty((batch,), dtype=torch.int32, device=device)
+    return _empty(max(int(nbytes), 256), torch.uint8, device, stream)
+
+
+def _info(batch, device, stream=None):
+    import torch
+    return _empty((batch,), torch.int32, device, stream)
 
 
 def lsms_tinv_from_phase_shifts(handle: Handle, delta, species, z, lmax, n_sites, spin_canted, n_species, batch,
@@ -232,11 +259,11 @@ def lsms_tinv_from_phase_shifts(handle: Handle, delta, species, z, lmax, n_sites
     import torch
     nspin = 2 if spin_canted else 1
     if tinv_diag is None:
-        tinv_diag = torch.empty((batch, n_sites, nspin, lmax + 1), dtype=torch.complex128, device=z.device)
+        tinv_diag = _empty((batch, n_sites, nspin, lmax + 1), torch.complex128, z.device, stream)
     if kappa is None:
-        kappa = torch.empty((batch,), dtype=torch.complex128, device=z.device)
+        kappa = _empty((batch,), torch.complex128, z.device, stream)
     if info is None:
-        info = _info(batch, z.device)
+        info = _info(batch, z.device, stream)
     _check(lib().lsms_tinv_from_phase_shifts(handle.ptr, _ptr(delta), _ptr(species), _ptr(z), lmax, n_sites,
                                              int(bool(spin_canted)), n_species, batch, _ptr(tinv_diag), _ptr(kappa),
                                              _ptr(info), _stream(stream)), "lsms_tinv_from_phase_shifts")
@@ -250,11 +277,11 @@ def lsms_build_M_batched(handle: Handle, tinv_diag, site_pos, moment_dir, kappa,
     k = (lmax + 1) ** 2 * (2 if spin_canted else 1)
     n = n_sites * k
     if M_out is None:
-        M_out = torch.empty((batch, n, n), dtype=torch.complex128, device=kappa.device)
+        M_out = _empty((batch, n, n), torch.complex128, kappa.device, stream)
     if info is None:
-        info = _info(batch, kappa.device)
+        info = _info(batch, kappa.device, stream)
     if workspace is None:
-        workspace = _workspace(lsms_workspace_bytes(handle, n_sites, lmax, spin_canted, batch), kappa.device)
+        workspace = _workspace(lsms_workspace_bytes(handle, n_sites, lmax, spin_canted, batch), kappa.device, stream)
     _check(lib().lsms_build_M_batched(handle.ptr, _ptr(tinv_diag), _ptr(site_pos), _ptr(moment_dir), _ptr(kappa), lmax,
                                       n_sites, int(bool(spin_canted)), batch, _ptr(M_out), _ptr(info), _ptr(workspace),
                                       workspace.numel(), _stream(stream)), "lsms_build_M_batched")
@@ -269,11 +296,11 @@ def lsms_build_M_shared_g0_batched(handle: Handle, tinv_diag, site_pos, moment_d
     n = n_sites * k
     batch = n_atoms * n_energies
     if M_out is None:
-        M_out = torch.empty((batch, n, n), dtype=torch.complex128, device=kappa.device)
+        M_out = _empty((batch, n, n), torch.complex128, kappa.device, stream)
     if info is None:
-        info = _info(batch, kappa.device)
+        info = _info(batch, kappa.device, stream)
     if workspace is None:
-        workspace = _workspace(lsms_workspace_bytes(handle, n_sites, lmax, spin_canted, batch), kappa.device)
+        workspace = _workspace(lsms_workspace_bytes(handle, n_sites, lmax, spin_canted, batch), kappa.device, stream)
     _check(lib().lsms_build_M_shared_g0_batched(handle.ptr, _ptr(tinv_diag), _ptr(site_pos), _ptr(moment_dir), _ptr(kappa),
                                                 lmax, n_sites, int(bool(spin_canted)), n_atoms, n_energies, _ptr(M_out),
                                                 _ptr(info), _ptr(workspace), workspace.numel(), _stream(stream)),
@@ -289,11 +316,11 @@ def lsms_tau00_batched(handle: Handle, M, n_sites, kmax, spin_canted, batch, tau
     k = kmax * (2 if spin_canted else 1)
     lmax = int(round(kmax ** 0.5)) - 1
     if tau00_out is None:
-        tau00_out = torch.empty((batch, k, k), dtype=torch.complex128, device=M.device)
+        tau00_out = _empty((batch, k, k), torch.complex128, M.device, stream)
     if info is None:
-        info = _info(batch, M.device)
+        info = _info(batch, M.device, stream)
     if workspace is None:
-        workspace = _workspace(lsms_workspace_bytes(handle, n_sites, max(lmax, 0), spin_canted, batch), M.device)
+        workspace = _workspace(lsms_workspace_bytes(handle, n_sites, max(lmax, 0), spin_canted, batch), M.device, stream)
     _check(lib().lsms_tau00_batched(handle.ptr, _ptr(M), n_sites, kmax, int(bool(spin_canted)), batch, _ptr(tau00_out),
                                     _ptr(info), _ptr(workspace), workspace.numel(), _stream(stream)), "lsms_tau00_batched")
     return tau00_out, info
@@ -333,11 +360,11 @@ def lsms_solve_central_column_batched(handle: Handle, M, n_sites, kmax, spin_can
     k = kmax * (2 if spin_canted else 1)
     n = n_sites * k
     if X_out is None:
-        X_out = torch.empty((batch, k, n), dtype=torch.complex128, device=M.device)
+        X_out = _empty((batch, k, n), torch.complex128, M.device, stream)
     if info is None:
-        info = _info(batch, M.device)
+        info = _info(batch, M.device, stream)
     if workspace is None:
-        workspace = _workspace(lsms_solve_workspace_bytes(handle, n_sites, kmax, spin_canted, batch), M.device)
+        workspace = _workspace(lsms_solve_workspace_bytes(handle, n_sites, kmax, spin_canted, batch), M.device, stream)
     _check(lib().lsms_solve_central_column_batched(handle.ptr, _ptr(M), n_sites, kmax, int(bool(spin_canted)), batch,
                                                    _ptr(X_out), _ptr(info), _ptr(workspace), workspace.numel(),
                                                    _stream(stream)), "lsms_solve_central_column_batched")
@@ -347,7 +374,7 @@ def lsms_solve_central_column_batched(handle: Handle, M, n_sites, kmax, spin_can
 def lsms_contour_sum_batched(handle: Handle, tau00, weights, n_atoms, n_energies, k, out=None, stream=None):
     import torch
     if out is None:
-        out = torch.empty((n_atoms, k, k), dtype=torch.complex128, device=tau00.device)
+        out = _empty((n_atoms, k, k), torch.complex128, tau00.device, stream)
     _check(lib().lsms_contour_sum_batched(handle.ptr, _ptr(tau00), _ptr(weights), n_atoms, n_energies, k, _ptr(out),
                                           _stream(stream)), "lsms_contour_sum_batched")
     return out

@@ -3,6 +3,7 @@
 #include <math.h>
 #include <stdint.h>
 #include <string.h>
+#include <algorithm>
 #include <new>
 #include <vector>
 #include "../../include/lsms_tau.h"
@@ -46,6 +47,14 @@ static int bind_device(Ctx* c, int dev) {
     if ((rc = init_attrs_gemm()) || (rc = init_attrs_lu()) || (rc = init_attrs_assemble()) || (rc = init_attrs_fused()) ||
         (rc = init_attrs_resident()) || (rc = init_attrs_panel()) ||
         (rc = init_attrs_panel_cluster())) return rc;
+    // How many clusters of 1 / 2 / 4 / 8 CTAs of each cluster kernel this device -- or the SM partition this process has been
+    // given of it (MPS / MIG: the paper's ranks share a GPU) -- can hold at once; 0 = such a cluster cannot
+    // be launched here at all, and the scheduler then keeps to the schedules that need none.
+    for (int i = 0; i < 4; ++i) {
+        c->res_clusters[i] = resident_max_active_clusters(1 << i);
+        c->fused_clusters[i] = fused_max_active_clusters(1 << i);
+        c->pclu_clusters[i] = i ? panel_cluster_max_active_clusters(1 << i) : 0;
+    }
     int lo = 0, hi = 0;
     LSMS_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
     LSMS_CUDA_OK(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
@@ -89,6 +98,16 @@ static TauWs tau_ws_layout(void* base, int NB, int n, int k, int batch) {
     w.total = (size_t)(p - (char*)base);
     return w;
 }
+// the same layout seen from item b0 on
+static TauWs tau_ws_offset(const TauWs& ws, int NB, int n, int k, int b0) {
+    TauWs w = ws;
+    w.piv = ws.piv + (size_t)b0 * n;
+    w.perm = ws.perm + (size_t)b0 * (4 + 3 * NB);
+    w.ninv = ws.ninv + (size_t)b0 * NB * NB;
+    w.tperm = ws.tperm + (size_t)b0 * NB * n;
+    w.k5 = (char*)ws.k5 + (final_inverse_ws_bytes(k, 1) ? (size_t)b0 * k * k * sizeof(c128) : 0);
+    return w;
+}
 static size_t tau_ws_bytes(const Ctx* c, int n, int k, int batch) { return tau_ws_layout(nullptr, eff_nb(c), n, k, batch).total; }
 
 // Blocked right-looking elimination of the first ne = n-k columns of every item, in lock-step over
@@ -116,6 +135,7 @@ static size_t tau_ws_bytes(const Ctx* c, int n, int k, int batch) { return tau_w
 // under look-ahead it waits for the Schur update to drain instead of running beneath it and whole steps of batches
 // >= 4 got SLOWER (NC 1897 -> 1928 ms, H 629 -> 654, C 440 -> 465, P 121 -> 129).  It pays when there is next to
 // nothing to overlap with: one or two tall matrices (rank 12450, batch 1: 369 -> 223 ms; rank 4320: 36.9 -> 32.5 ms).
+static inline int ilog2(int cl) { return cl >= 8 ? 3 : cl >= 4 ? 2 : cl >= 2 ? 1 : 0; }
 static int panel_cluster_size(const Ctx* c, int m, int batch) {
     const int pc = c->opt[LSMS_OPT_PANEL_CLUSTER];
     if (c->opt[LSMS_OPT_PANEL_THREADS] < 1) return 1;
@@ -125,7 +145,15 @@ static int panel_cluster_size(const Ctx* c, int m, int batch) {
     else if (batch <= 2 && m >= 4096) cl = 8;
     else if (batch <= 2 && m >= 2048) cl = 4;
     if (cl > 1 && (m + cl - 1) / cl > 5120) cl = 1;         // taller than the cluster instances cover: one-CTA kernel
+    if (cl > 1 && c->pclu_clusters[ilog2(cl)] < 1) cl = 1;  // such a cluster cannot be co-scheduled on this device / partition
     return cl;
+}
+
+// Tallest panel the lock-step schedule can factor: the first one, n rows.  The one-CTA panel kernels cover 16384 rows,
+// the cluster kernel 8 x 5120 (picked for one or two matrices only, see above); later panels are shorter and covered
+// whenever the first is.  Checked by every entry point before anything is enqueued (LSMS_ERR_PANEL_TOO_TALL).
+static bool rows_supported(const Ctx* c, int n, int batch) {
+    return n <= 16384 || panel_cluster_size(c, n, batch) > 1;
 }
 
 // factor the outer panel [J, J+W) on stream st: inner panels of width <= IB
@@ -166,51 +194,6 @@ static int schur_update(c128* M, int n, int batch, int J, int W, int c_lo, int c
     g.C = M + (size_t)Jend + (size_t)c_lo * n;
     ProfScope ps(4, st, 8.0 * g.Mr * g.Nc * g.K * batch);
     return launch_schur_gemm(g, st);
-}
-
-// Look-ahead variant 2: EVERYTHING except the big Schur update runs on the group's high-priority stream (interchanges,
-// triangular solve, the next panel's slice of the update, the panel factorisation); the group's main stream carries only
-// the updates of the remaining columns.  With two batch groups the block scheduler then hands freed SM resources to one
-// group's latency- and bandwidth-bound kernels first while the other group's update CTAs fill the rest.
-static int eliminate_prio(const Ctx* c, c128* M, int n, int k, int batch, const TauWs& ws, int* info, cudaStream_t st, const GroupStreams& gs) {
-    const int ne = n - k;
-    const int NB = eff_nb(c), IB = eff_ib(c);
-    const size_t stride = (size_t)n * n;
-    int* piv = ws.piv;
-    if (ne <= 0) return 0;
-    int W0 = ne < NB ? ne : NB;
-    if (c->opt[LSMS_OPT_ALIGN_FIRST] && NB % 64 == 0 && n % 64 != 0 && n % 64 < W0) W0 = n % 64;
-    cudaStream_t ax = gs.aux;
-    LSMS_CUDA_OK(cudaEventRecord(gs.join, st));
-    LSMS_CUDA_OK(cudaStreamWaitEvent(ax, gs.join, 0));
-    int rc = factor_panel(c, M, n, batch, 0, W0, ne, IB, piv, info, ax);
-    if (!rc) { ProfScope ps(6, ax); rc = launch_panel_post(M, stride, n, 0, W0, batch, piv, ws.perm, ws.ninv, NB, ax); }
-    for (int J = 0, W = W0; J < ne && !rc; J += W, W = (ne - J < NB) ? ne - J : NB) {
-        const int Jend = J + W;
-        { ProfScope ps(6, ax); rc = launch_row_permute(M, stride, n, J, W, Jend, n, batch, ws.perm, ws.tperm, (size_t)NB * n, NB, ax); } if (rc) break;
-        GemmShape t; t.batch = batch; t.beta0 = 1; t.triA = 1;
-        t.A = ws.ninv; t.strideA = (size_t)NB * NB; t.ldA = NB;
-        t.B = ws.tperm + (size_t)Jend * NB; t.strideB = (size_t)NB * n; t.ldB = NB;
-        t.C = M + (size_t)J + (size_t)Jend * n; t.strideC = stride; t.ldC = n;
-        t.Mr = W; t.Nc = n - Jend; t.K = W;
-        { ProfScope ps(7, ax, 8.0 * t.Mr * t.Nc * t.K * batch); rc = launch_schur_gemm(t, ax); } if (rc) break;
-        const int W2 = (Jend < ne) ? ((ne - Jend < NB) ? ne - Jend : NB) : 0;
-        if (W2 > 0) { rc = schur_update(M, n, batch, J, W, Jend, Jend + W2, ax); if (rc) break; }
-        if (cudaEventRecord(gs.fork, ax) != cudaSuccess || cudaStreamWaitEvent(st, gs.fork, 0) != cudaSuccess) { rc = (int)cudaGetLastError(); break; }
-        rc = schur_update(M, n, batch, J, W, Jend + W2, n, st); if (rc) break;
-        if (cudaEventRecord(gs.join, st) != cudaSuccess) { rc = (int)cudaGetLastError(); break; }
-        if (W2 > 0) {
-            rc = factor_panel(c, M, n, batch, Jend, W2, ne, IB, piv, info, ax); if (rc) break;
-            { ProfScope ps(6, ax); rc = launch_panel_post(M, stride, n, Jend, W2, batch, piv, ws.perm, ws.ninv, NB, ax); } if (rc) break;
-        }
-        if (cudaStreamWaitEvent(ax, gs.join, 0) != cudaSuccess) { rc = (int)cudaGetLastError(); break; }
-    }
-    // the auxiliary stream is joined back even when a launch failed
-    cudaError_t e1 = cudaEventRecord(gs.fork, ax);
-    cudaError_t e2 = cudaStreamWaitEvent(st, gs.fork, 0);
-    if (rc) return rc;
-    LSMS_CUDA_OK(e1); LSMS_CUDA_OK(e2);
-    return 0;
 }
 
 // one batch group [0, batch) of items (pointers already offset to the group's first item)
@@ -290,13 +273,8 @@ static int eliminate_groups(Ctx* c, c128* M, int n, int k, int batch, const TauW
         if (b1 <= b0) continue;
         cudaStream_t gst = (g == 0) ? st : c->gs[g].main;
         if (g > 0) { rc = (int)cudaStreamWaitEvent(gst, c->ev_start, 0); if (rc) break; }
-        TauWs w = ws;
-        w.piv = ws.piv + (size_t)b0 * n;
-        w.perm = ws.perm + (size_t)b0 * (4 + 3 * NB);
-        w.ninv = ws.ninv + (size_t)b0 * NB * NB;
-        w.tperm = ws.tperm + (size_t)b0 * NB * n;
-        w.k5 = (char*)ws.k5 + (final_inverse_ws_bytes(k, 1) ? (size_t)b0 * k * k * sizeof(c128) : 0);
-        rc = (c->opt[LSMS_OPT_LOOKAHEAD] == 2 ? eliminate_prio : eliminate)(c, M + (size_t)b0 * stride, n, k, b1 - b0, w, info + b0, gst, c->gs[g]);
+        const TauWs w = tau_ws_offset(ws, NB, n, k, b0);
+        rc = eliminate(c, M + (size_t)b0 * stride, n, k, b1 - b0, w, info + b0, gst, c->gs[g]);
         if (!rc) {
             ProfScope ps(5, gst);
             rc = launch_final_inverse(M + (size_t)b0 * stride, stride, n, k, b1 - b0, tau + (size_t)b0 * k * k, info + b0, w.k5, gst);
@@ -319,17 +297,21 @@ static int eliminate_groups(Ctx* c, c128* M, int n, int k, int batch, const TauW
 static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
     const int sm = c->opt[LSMS_OPT_SMALL_MODE];
     if (sm == 1) return 0;
-    const int rcl = resident_cluster_size(n, k);
+    int rcl = resident_cluster_size(n, k);
+    // clusters of rcl CTAs that can be resident at once (0: the cluster cannot be launched on this device / partition)
+    const int ract = rcl > 0 ? std::min(c->res_clusters[ilog2(rcl)], c->sms / rcl) : 0;
+    if (ract < 1) rcl = 0;
     if (sm == 7) return rcl > 0 ? -rcl : 0;
     // Default for matrices that fit on chip (n <= ~216 with 4 SMs each), while the batch needs at most ~3.5 waves of
     // clusters: the on-chip kernel is built for latency (208^2 x 32: 0.20 ms against 0.56 ms through L2 and 0.85 ms in
     // lock-step), but it holds 4 SMs per matrix for the whole elimination, and from ~150 matrices of 208^2 on the
     // lock-step schedule has the higher throughput (128 matrices: 0.71 ms on chip, 0.78 lock-step; 192: 1.05 / 0.90;
     // 512: 2.72 / 1.64).
-    if (sm == 0 && rcl > 0 && 2LL * batch * rcl <= 7LL * c->sms) return -rcl;
+    if (sm == 0 && rcl > 0 && 2LL * batch <= 7LL * ract) return -rcl;
     if (sm == 0) return 0;
     if (!fused_supported(n, k, eff_nb(c), eff_ib(c))) return 0;
-    if (sm >= 3) return 1 << (sm - 3);
+    if (sm >= 3) return c->fused_clusters[sm - 3] > 0 ? 1 << (sm - 3) : 0;
+    if (c->fused_clusters[0] < 1) return 0;
     // sm == 2: the one-launch mode through L2 (fused.cu).  CTAs per matrix: a CTA is a quarter of an SM, so few matrices
     // get a cluster each until the chip is covered.  Tiny matrices: at most 4 -- their panel chain is serial, rank 0
     // factors under the other ranks' updates, and a third to seventh helper only adds barrier traffic (208^2 x 32:
@@ -339,7 +321,7 @@ static int pick_small_mode(const Ctx* c, int n, int k, int batch) {
     const long long slots = 4LL * c->sms;
     const int cl_max = fused_is_tiny(n) ? 4 : 8;
     int cl = 1;
-    while (cl < cl_max && (long long)batch * cl * 2 <= slots) cl *= 2;
+    while (cl < cl_max && (long long)batch * cl * 2 <= slots && c->fused_clusters[ilog2(cl * 2)] > 0) cl *= 2;
     return cl;
 }
 
@@ -348,8 +330,16 @@ static int tau00_impl(Ctx* c, c128* M, int n, int k, int batch, c128* tau, int* 
     const int cl = pick_small_mode(c, n, k, batch);
     c->last_schedule = cl < 0 ? 100 - cl : cl;
     if (cl < 0) {
-        ProfScope ps(2, st, 8.0 / 3.0 * (double)n * n * n * batch);
-        return launch_lu_resident(M, (size_t)n * n, n, k, batch, -cl, ws.piv, tau, info, st);
+        int done = 0, rc;
+        { ProfScope ps(2, st, 8.0 / 3.0 * (double)n * n * n * batch);
+          rc = launch_lu_resident(M, (size_t)n * n, n, k, batch, -cl, ws.piv, tau, info, st, &done); }
+        if (rc <= 0) return rc;
+        // The cluster launch was refused although bind_device found it feasible (the SMs available to this process can
+        // change under it).  A refused launch enqueues nothing and its error code has been taken off the thread: the
+        // items not yet enqueued go through the lock-step schedule, which needs no cluster.
+        c->last_schedule = 0;
+        return eliminate_groups(c, M + (size_t)done * n * n, n, k, batch - done, tau_ws_offset(ws, eff_nb(c), n, k, done),
+                                tau + (size_t)done * k * k, info + done, st);
     }
     if (cl > 0) {
         ProfScope ps(2, st, 8.0 / 3.0 * (double)n * n * n * batch);
@@ -362,7 +352,7 @@ static size_t workspace_bytes_impl(const Ctx* c, int n_sites, int lmax, int spin
     if (n_sites < 1 || lmax < 0 || lmax > 8 || batch < 1) return 0;
     int kmax = (lmax + 1) * (lmax + 1), k = kmax * (spin_canted ? 2 : 1);
     size_t n = (size_t)n_sites * k;
-    if (n > 46340) return 0;
+    if (n > 46340 || !rows_supported(c, (int)n, batch)) return 0;
     size_t a = align256(gaunt_table_bytes(lmax));
     size_t t = tau_ws_bytes(c, (int)n, k, batch);
     return a > t ? a : t;
@@ -413,7 +403,7 @@ int lsms_set_option(lsms_handle_t c, int option, int value) {
     switch (option) {
         case LSMS_OPT_NB_OUTER: ok = value >= 0 && value <= 96 && value % 4 == 0; break;
         case LSMS_OPT_IB_INNER: ok = value >= 0 && value <= 16; break;
-        case LSMS_OPT_LOOKAHEAD: ok = value >= 0 && value <= 2; break;
+        case LSMS_OPT_LOOKAHEAD: ok = value == 0 || value == 1; break;
         case LSMS_OPT_PANEL_THREADS: ok = value >= 0 && value <= 2; break;
         case LSMS_OPT_ALIGN_FIRST: ok = value == 0 || value == 1; break;
         case LSMS_OPT_GROUPS: ok = value >= 0 && value <= MAX_GROUPS; break;
@@ -443,7 +433,7 @@ size_t lsms_solve_workspace_bytes(lsms_handle_t c, int n_sites, int kmax, int sp
     if (!c || n_sites < 1 || kmax < 1 || batch < 1) return 0;
     int k = kmax * (spin_canted ? 2 : 1);
     size_t n = (size_t)n_sites * k;
-    if (n > 46340) return 0;
+    if (n > 46340 || !rows_supported(c, (int)n, batch)) return 0;
     return align256((size_t)batch * n * n * sizeof(c128)) + align256((size_t)batch * k * k * sizeof(c128)) + tau_ws_bytes(c, (int)n, k, batch);
 }
 
@@ -528,6 +518,7 @@ int lsms_tau00_batched(lsms_handle_t h, lsms_c128* M, int n_sites, int kmax, int
     const long long nll = (long long)n_sites * k;
     if (nll > 46340) return -3;
     const int n = (int)nll;
+    if (!rows_supported(h, n, batch)) return LSMS_ERR_PANEL_TOO_TALL;
     if (!workspace || !aligned16(workspace)) return -9;
     if (workspace_bytes < tau_ws_bytes(h, n, k, batch)) return -10;
     LSMS_BIND(h);
@@ -547,7 +538,7 @@ int lsms_solve_central_column_batched(lsms_handle_t h, const lsms_c128* M, int n
     if (!info) return -8;
     if (!workspace || !aligned16(workspace)) return -9;
     const size_t need = lsms_solve_workspace_bytes(h, n_sites, kmax, spin_canted, batch);
-    if (need == 0) return -3;
+    if (need == 0) return (long long)n_sites * kmax * (spin_canted ? 2 : 1) > 46340 ? -3 : LSMS_ERR_PANEL_TOO_TALL;
     if (workspace_bytes < need) return -10;
     LSMS_BIND(h);
     const int k = kmax * (spin_canted ? 2 : 1);
@@ -604,7 +595,7 @@ int lsms_tau00_from_host(lsms_handle_t h, const lsms_c128* delta_host, const int
     if (!info_host) return -14;
     if (!device_scratch || !aligned16(device_scratch)) return -15;
     const size_t need = lsms_host_call_scratch_bytes(h, n_sites, lmax, spin_canted, n_species, batch);
-    if (need == 0) return -8;
+    if (need == 0) return (long long)n_sites * (lmax + 1) * (lmax + 1) * (spin_canted ? 2 : 1) > 46340 ? -8 : LSMS_ERR_PANEL_TOO_TALL;
     if (scratch_bytes < need) return -16;
     LSMS_BIND(h);
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -672,6 +663,17 @@ int lsms_contour_sum_batched(lsms_handle_t h, const lsms_c128* tau00, const lsms
 
 int lsms_last_launch_count(lsms_handle_t h) { return h ? h->last_launches : -1; }
 int lsms_last_schedule(lsms_handle_t h) { return h ? h->last_schedule : -1; }
+
+int lsms_max_active_clusters(lsms_handle_t h, int kernel, int cluster_size, int* count_host) {
+    LSMS_ENTER(h);
+    if (kernel < 0 || kernel > 2) return -2;
+    if (cluster_size != 1 && cluster_size != 2 && cluster_size != 4 && cluster_size != 8) return -3;
+    if (!count_host) return -4;
+    LSMS_BIND(h);
+    const int i = ilog2(cluster_size);
+    *count_host = kernel == 0 ? h->res_clusters[i] : kernel == 1 ? h->fused_clusters[i] : h->pclu_clusters[i];
+    return 0;
+}
 
 int lsms_profile_begin(lsms_handle_t h) {
     if (!h) return -1;

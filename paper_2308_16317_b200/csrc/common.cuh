@@ -55,5 +55,8 @@ extern thread_local LaunchCounter g_launches;
 
 }  // namespace lsms
 
-#define LSMS_CUDA_OK(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return (int)e__; } while (0)
-#define LSMS_LAUNCH_CHECK() do { ++lsms::g_launches.n; cudaError_t e__ = cudaPeekAtLastError(); if (e__ != cudaSuccess) return (int)e__; } while (0)
+// A failed runtime call or launch leaves its code pending on the host thread; it is taken off there (cudaGetLastError)
+// before it is returned, so that it is reported once, by the call that caused it, and neither a later library call nor
+// the caller's own checks (torch's, say) trip over a stale code.
+#define LSMS_CUDA_OK(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { cudaGetLastError(); return (int)e__; } } while (0)
+#define LSMS_LAUNCH_CHECK() do { ++lsms::g_launches.n; cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return (int)e__; } while (0)

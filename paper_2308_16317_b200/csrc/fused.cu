@@ -454,6 +454,18 @@ int init_attrs_fused() {
     return 0;
 }
 
+int fused_max_active_clusters(int cl) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)cl); cfg.blockDim = dim3(FT); cfg.dynamicSmemBytes = F_SMEM;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = (unsigned)cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    int a = 0, b = 0;
+    if (cudaOccupancyMaxActiveClusters(&a, k_lu_fused, &cfg) != cudaSuccess ||
+        cudaOccupancyMaxActiveClusters(&b, k_lu_tiny, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return a < b ? a : b;
+}
+
 int launch_lu_fused(c128* base, size_t stride, int n, int k, int batch, int NB, int IB, int align_first, int cl,
                     int* piv, c128* tau, int* info, cudaStream_t st) {
     if (!fused_supported(n, k, NB, IB) || (cl != 1 && cl != 2 && cl != 4 && cl != 8)) return -1;

@@ -24,6 +24,12 @@ struct Ctx {
     int device = 0;
     int sms = 148;
     int opt[LSMS_OPT_COUNT];
+    // clusters of 1 / 2 / 4 / 8 CTAs that fit the device (or this process's SM partition) at once, per cluster kernel:
+    // on-chip elimination, one-launch elimination through L2, cluster panel kernel.  Filled by bind_device; an unbound
+    // handle (host-side size queries) assumes they all fit.
+    int res_clusters[4] = {1 << 20, 1 << 20, 1 << 20, 1 << 20};
+    int fused_clusters[4] = {1 << 20, 1 << 20, 1 << 20, 1 << 20};
+    int pclu_clusters[4] = {0, 1 << 20, 1 << 20, 1 << 20};
     GroupStreams gs[MAX_GROUPS];
     cudaEvent_t ev_start = nullptr;
     Prof prof;
@@ -44,7 +50,7 @@ struct ProfScope {
     ~ProfScope();
 };
 
-// one-time per-device opt-in to dynamic shared-memory sizes (called from lsms_create for the handle's device)
+// one-time per-device opt-in to dynamic shared-memory sizes (called from bind_device, at a handle's first enqueueing call)
 int init_attrs_gemm();
 int init_attrs_lu();
 int init_attrs_assemble();
@@ -96,7 +102,14 @@ int launch_lu_fused(c128* base, size_t stride, int n, int k, int batch, int NB, 
 
 // resident.cu -- small-matrix mode, on-chip variant: the matrix lives in the distributed shared memory of a cluster
 int resident_cluster_size(int n, int k);             // smallest cluster that holds an n x n matrix on chip (0: none)
-int launch_lu_resident(c128* base, size_t stride, int n, int k, int batch, int cl, int* piv, c128* tau, int* info, cudaStream_t st);
+// *enqueued (optional) receives the number of leading items whose launch was accepted, also when a launch is refused
+int launch_lu_resident(c128* base, size_t stride, int n, int k, int batch, int cl, int* piv, c128* tau, int* info, cudaStream_t st,
+                       int* enqueued = nullptr);
+// cudaOccupancyMaxActiveClusters of the cluster kernels for clusters of cl CTAs at their largest shared-memory size
+// (the minimum over a kernel family's instances); 0 when such a cluster cannot be launched on the current device
+int resident_max_active_clusters(int cl);
+int fused_max_active_clusters(int cl);
+int panel_cluster_max_active_clusters(int cl);
 
 // reduce.cu
 int launch_contour_sum(const c128* tau, const c128* w, int n_atoms, int n_e, int kk, c128* out, cudaStream_t st);

@@ -29,7 +29,13 @@ static int launch_one(c128* base, size_t stride, int n, int J, int Wout, int c0,
 // Instantiations (THREADS, R rows per thread, S sub-panel width, DEPTH columns in flight in step 5).  S <= 4: the column
 // threads of step 4 hold 2*S more values beside the sub-panel; R*S complex numbers per thread are the sub-panel.
 // DEPTH * R * THREADS * 16 B of shared memory per CTA: 160 KB for the 512-thread kernels (one CTA per SM), 80 KB for
-// the 256-thread ones (two per SM), <= 48 KB for the 128-thread ones (four per SM, the slot of one Schur-update CTA).
+// the 256-thread ones (two per SM), <= 32 KB for the 128-thread ones with R <= 4 (four per SM, the slot of one
+// Schur-update CTA); X(128, 8, 2, 3) stages 48 KB beside ~8.6 KB of static PanelShared, so THREE of those fit an SM.
+// GPU tests that reach each instance (tests/test_gpu_parity.py):
+//   128-thread row, 256-thread row, <512,5,4,4>, <512,10,2,2>: test_panel_kernel_variants_match_oracle[threads = 2 / 0 / 1]
+//   <512,20,1,0> (5121-10240 rows): test_tau00_full_size_against_stored_oracle_values[H_0, H_23, N_23; panel_cluster = 1],
+//                                   test_tau00_high_l_batch_of_three_as_bench_times_it (default handle, batch 3)
+//   <512,32,1,0> (> 10240 rows):    test_tau00_full_size_against_stored_oracle_values[NC_5; panel_cluster = 1]
 #define LSMS_P2_LIST(X)                                                                                     \
     X(128, 1, 4, 4) X(128, 2, 4, 4) X(128, 4, 4, 4) X(128, 8, 2, 3)                                         \
     X(256, 1, 4, 4) X(256, 2, 4, 4) X(256, 5, 4, 4) X(256, 10, 2, 2) X(256, 20, 1, 0)                       \

@@ -69,6 +69,7 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
                                            int* __restrict__ pv, int* __restrict__ info, PanelShared& sh, c128* stage = nullptr) {
     constexpr int NW = THREADS / 32;
     static_assert(S <= 4 && NW <= 16, "PanelShared is sized for S <= 4 and <= 16 warps");
+    static_assert(R * THREADS <= 16384, "arg-max key: 14 bits for the row offset within the panel (16383 - offset), 4 for the warp");
     c128* L11 = sh.L11; c128* Us = sh.Us;
     int* spiv = sh.spiv; int* canon = sh.canon;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;

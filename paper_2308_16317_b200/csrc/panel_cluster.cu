@@ -49,6 +49,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS <= 256) ? 2 : 1)
 k_panel_clu(c128* __restrict__ base, size_t stride, int n, int J, int Wout, int c0, int w, int ne,
             int* __restrict__ piv, int* __restrict__ info) {
     constexpr int NW = THREADS / 32;
+    static_assert(PC_MAXCL * R * THREADS <= 65536 && PC_MAXCL * NW <= 128,
+                  "arg-max key: 16 bits for the row offset within the panel (65535 - offset), 7 for the (CTA, warp) slot");
     extern __shared__ __align__(16) unsigned char pc_stage[];
     c128* stage = reinterpret_cast<c128*>(pc_stage);
     const uint32_t rank = pc_rank(), ncl = pc_nranks();
@@ -343,6 +345,29 @@ int init_attrs_panel_cluster() {
     LSMS_PC_LIST(LSMS_PC_ATTR)
 #undef LSMS_PC_ATTR
     return 0;
+}
+
+template <int THREADS, int R, int S, int DEPTH>
+static int active_clu(int cl) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)cl, 1, 1); cfg.blockDim = dim3(THREADS, 1, 1); cfg.dynamicSmemBytes = pc_stage_bytes<THREADS, R, DEPTH>();
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    int nclu = 0;
+    if (cudaOccupancyMaxActiveClusters(&nclu, k_panel_clu<THREADS, R, S, DEPTH>, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return nclu;
+}
+
+// the minimum over the instances: a panel walks through several of them as it gets shorter
+int panel_cluster_max_active_clusters(int cl) {
+    if (cl < 2 || cl > PC_MAXCL) return 0;
+    int best = 1 << 30;
+#define LSMS_PC_OCC(T, R, S, D) { const int a = active_clu<T, R, S, D>(cl); if (a < best) best = a; }
+    LSMS_PC_LIST(LSMS_PC_OCC)
+#undef LSMS_PC_OCC
+    return best;
 }
 
 // cl = CTAs per matrix (2, 4 or 8); rows per CTA = ceil((n - c0) / cl) picks the instance

@@ -44,6 +44,7 @@ constexpr int RS_PT = 256;           // panel threads = largest n
 constexpr int RW = 8;                // panel width = column-block width
 constexpr int RS_LDU = RW + 4;       // U operand buffer stride (complex), == 4 (mod 8)
 constexpr size_t RS_SMEM_MAX = 232448;
+static_assert(RS_PT <= 256 && RS_PT / 32 <= 8, "arg-max key of the panel step: 8 bits for the row position (255 - pos), 3 for the warp");
 
 struct ResLayout {
     int ld, ldp, ncols_max;
@@ -479,20 +480,36 @@ int init_attrs_resident() {
     return 0;
 }
 
-int launch_lu_resident(c128* base, size_t stride, int n, int k, int batch, int cl, int* piv, c128* tau, int* info, cudaStream_t st) {
+// cluster launch configuration shared by the launcher and the occupancy query
+static void cluster_config(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* at, unsigned grid, unsigned threads, size_t smem, int cl, cudaStream_t st) {
+    cfg = cudaLaunchConfig_t{};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = (unsigned)cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+}
+
+int resident_max_active_clusters(int cl) {
+    cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1];
+    cluster_config(cfg, at, (unsigned)cl, RS_T, RS_SMEM_MAX, cl, nullptr);
+    int nclu = 0;
+    if (cudaOccupancyMaxActiveClusters(&nclu, k_lu_resident, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return nclu;
+}
+
+int launch_lu_resident(c128* base, size_t stride, int n, int k, int batch, int cl, int* piv, c128* tau, int* info, cudaStream_t st,
+                       int* enqueued) {
+    if (enqueued) *enqueued = 0;
     const int cl_min = resident_cluster_size(n, k);
     if (cl_min == 0 || cl < cl_min || (cl != 1 && cl != 2 && cl != 4 && cl != 8)) return -1;
     const size_t smem = res_layout(n, cl).total;
     for (int b0 = 0; b0 < batch; b0 += 16384) {
         const int nb = batch - b0 < 16384 ? batch - b0 : 16384;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(nb * cl)); cfg.blockDim = dim3(RS_T); cfg.dynamicSmemBytes = smem; cfg.stream = st;
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = (unsigned)cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at; cfg.numAttrs = 1;
+        cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1];
+        cluster_config(cfg, at, (unsigned)(nb * cl), RS_T, smem, cl, st);
         LSMS_CUDA_OK(cudaLaunchKernelEx(&cfg, k_lu_resident, base + (size_t)b0 * stride, stride, n, k, piv + (size_t)b0 * n,
                                         tau + (size_t)b0 * k * k, info + b0));
         LSMS_LAUNCH_CHECK();
+        if (enqueued) *enqueued = b0 + nb;
     }
     return 0;
 }

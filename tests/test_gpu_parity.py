@@ -282,18 +282,52 @@ def read_golden(key, item):
     return n, k, ref
 
 
+@pytest.mark.parametrize("panel_cluster", [0, 1])
 @pytest.mark.parametrize("key,item", [("H", 0), ("H", 23), ("N", 23), ("C", 24), ("P", 24), ("NC", 5)])
-def test_tau00_full_size_against_stored_oracle_values(lt, h, key, item):
+def test_tau00_full_size_against_stored_oracle_values(lt, h, key, item, panel_cluster):
     """Element-wise parity at full size where the oracle needs minutes to an hour per item: tau00 of single items of
     the largest workloads (H item 0 is the worst-conditioned matrix of all configs, cond_1 ~ 1.6e6; NC is the paper's
     rank-12450 NiAu shape) against values the oracle wrote into tests/golden/ (tests/golden/make_golden_full_size.py:
-    oracle.assemble_M + FP64 LU with long-double iterative refinement; nothing there comes from the CUDA path)."""
+    oracle.assemble_M + FP64 LU with long-double iterative refinement; nothing there comes from the CUDA path).
+    panel_cluster = 0: what a one-matrix call gets by default, the CLUSTER panel kernel on panels of >= 2048 rows;
+    panel_cluster = 1: the ONE-CTA panel kernels that every batch of three or more matrices runs on -- the kernels
+    bench.py times H / N / NC on: k_panel_reg<512,20,1,0> (H, N: 5121-10240 rows), <512,32,1,0> (NC: > 10240 rows),
+    <512,10,2,2> (C), <512,5,4,4> (P), and the shorter instances as the panels shrink."""
     n, k, ref = read_golden(key, item)
     batch = sl.make_batch(key).select([item])
     assert batch.cfg.n == n and batch.cfg.k == k
+    h.set("panel_cluster", panel_cluster)
     tau, info, _ = lt.tau00_from_liz_batch(h, batch)
     assert not info.any()
-    check_tau(tau[0], ref, TAU_TOL, (key, item))
+    print(f"full-size parity {key}_{item} panel_cluster={panel_cluster}: rel. Frobenius {relF(tau[0], ref):.2e}")
+    check_tau(tau[0], ref, TAU_TOL, (key, item, panel_cluster))
+
+
+def test_tau00_high_l_batch_of_three_as_bench_times_it(lt, h):
+    """Workload H (6750 x 6750, spin-canted, l_max = 4) in the launch shape `bench.py --workload H` times: a batch of
+    more than two matrices through a DEFAULT handle -- lock-step schedule, look-ahead, one-CTA tall-panel kernel
+    k_panel_reg<512,20,1,0> (not the cluster kernel that one- and two-matrix calls get).  Items 0, 11, 23: the residual of
+    the central block column on every item, tau00 equal to that column's central block, and the two items with stored
+    oracle values (0: worst-conditioned of all configs; 23) element by element."""
+    items = [0, 11, 23]
+    batch = sl.make_batch("H").select(items)
+    cfg = batch.cfg
+    n, k = cfg.n, cfg.k
+    M, _, _ = gpu_M(lt, h, batch)
+    X, info = lt.lsms_solve_central_column_batched(h, M, cfg.n_sites, cfg.kmax, True, 3)
+    torch.cuda.synchronize()
+    assert lt.lsms_last_schedule(h) == 0 and h.get("panel_cluster") == 0 and not info.cpu().numpy().any()
+    res = device_residuals(M, X, n, k)
+    assert float(res.max()) < RES_TOL, res
+    tau, info2 = lt.lsms_tau00_batched(h, M, cfg.n_sites, cfg.kmax, True, 3)                  # overwrites M
+    torch.cuda.synchronize()
+    assert lt.lsms_last_schedule(h) == 0 and not info2.cpu().numpy().any()
+    assert float((X[:, :, n - k:] - tau).abs().max()) == 0.0
+    tau = tau.cpu().numpy().transpose(0, 2, 1)
+    for i, item in ((0, 0), (2, 23)):
+        _, _, ref = read_golden("H", item)
+        print(f"H item {item} in a batch of three (one-CTA tall panels): rel. Frobenius {relF(tau[i], ref):.2e}")
+        check_tau(tau[i], ref, TAU_TOL, ("H batch of 3", item))
 
 
 @pytest.mark.parametrize("key,item", [("N", 23), ("NC", 0)])
@@ -409,11 +443,22 @@ def test_lookahead_on_and_off_give_identical_results(lt, h):
     assert np.array_equal(tau0, tau1)
 
 
-@pytest.mark.parametrize("threads", [0, 1])
+@pytest.mark.parametrize("threads", [0, 1, 2])
 def test_panel_kernel_variants_match_oracle(lt, h, threads):
-    """Both K2 footprints (256 / 512 threads) against the oracle on a tiny LIZ, a ragged random matrix (w and
-    sub-panel tails) and a mid LIZ (several row chunks)."""
-    h.set("panel_threads", threads).set("small_mode", 1)
+    """The three K2 footprints (LSMS_OPT_PANEL_THREADS: 0 = 256 threads throughout, 1 = 512 threads on tall panels,
+    2 = 128 threads up to 1024 rows) against the oracle on a tiny LIZ, ragged random matrices (w and sub-panel tails), a
+    mid LIZ (several row chunks) and single items of P and C with stored oracle values, one-CTA panel kernel forced.
+    Which k_panel_reg instances that reaches (panel height m = n - c0 shrinks through the shorter ones):
+      threads = 2: <128,1,4,4> <128,2,4,4> (T, 207, 164 rows), <128,4,4,4> <128,8,2,3> (M: 880 rows), the 256-thread ones above
+      threads = 0: <256,1,4,4> <256,2,4,4> <256,5,4,4> (<= 1280 rows), <256,10,2,2> (P: 2160), <256,20,1,0> (C: 4320)
+      threads = 1: the same up to 1280 rows, <512,5,4,4> (P), <512,10,2,2> (C); the taller <512,20,1,0> / <512,32,1,0> are
+                   reached by test_tau00_full_size_against_stored_oracle_values[panel_cluster=1] and the H batch of three."""
+    h.set("panel_threads", threads).set("small_mode", 1).set("panel_cluster", 1)
+    for key, item in (("P", 24), ("C", 24)):
+        _, _, gold = read_golden(key, item)
+        t, i, _ = lt.tau00_from_liz_batch(h, sl.make_batch(key).select([item]))
+        assert not i.any()
+        check_tau(t[0], gold, TAU_TOL, (key, item, threads))
     batch = sl.make_batch("T").select([0, 17, 31])
     ref, _ = oracle.tau00_batched(batch, "long double")
     tau, info, _ = lt.tau00_from_liz_batch(h, batch)
@@ -555,6 +600,21 @@ def test_scheduler_leaves_the_on_chip_mode_when_the_batch_needs_many_waves_of_cl
         check_tau(tau_oc[b], lapack_tau00(A[b], kmax), 1e-11, ("on chip vs LAPACK", b))
 
 
+def test_cluster_capacity_is_known_to_the_scheduler(lt, h):
+    """The cluster kernels are only scheduled where the device (or the SM partition this process has) can hold such a
+    cluster: the capacities asked at bind time are plausible on a whole B200 (148 SMs; one CTA per SM for the on-chip and
+    the tall-panel cluster kernels, so at most 148 / cl clusters) and non-zero for every cluster size the scheduler uses."""
+    for cl in (1, 2, 4, 8):
+        res, fus = lt.lsms_max_active_clusters(h, 0, cl), lt.lsms_max_active_clusters(h, 1, cl)
+        assert 1 <= res <= 148 // cl, (cl, res)
+        assert 1 <= fus <= 4 * 148 // cl, (cl, fus)
+        if cl > 1:
+            pc = lt.lsms_max_active_clusters(h, 2, cl)
+            assert 1 <= pc <= 148 // cl, (cl, pc)
+    assert lt.lsms_max_active_clusters(h, 2, 1) == 0
+    assert lt.lsms_max_active_clusters(h, 0, 4) >= 30        # workload T: 32 clusters of 4 in one wave
+
+
 def test_on_chip_mode_repeated_launches_are_bitwise_reproducible(lt, h):
     """The on-chip kernel synchronises its CTAs with flags, mbarriers and a polling "shipper" warp instead of cluster
     barriers: many launches in a row, batches of one wave and of several, cluster sizes 1 / 2 / 4 / 8 -- every launch
@@ -618,6 +678,29 @@ def test_two_host_threads_two_handles_two_streams(lt):
         assert not serial[i][0][1].any() and not conc[i][0][1].any()
         assert np.array_equal(serial[i][0][0], conc[i][0][0])
     h0.destroy()
+
+
+def test_calls_on_a_side_stream_with_buffers_left_to_the_binding(lt, h):
+    """Every call takes the stream it runs on.  With outputs and workspace omitted the binding allocates them with that
+    stream current, so the caching allocator cannot hand the dropped workspace to other work while the kernels still use
+    it: the whole path on a side stream, repeated with allocator churn on the default stream, gives the bits of the
+    default-stream run."""
+    batch = sl.make_batch("T")
+    cfg, B = batch.cfg, batch.batch
+    delta, species, z, pos, mom = lt.device_inputs(batch)
+    ref, info, _ = lt.tau00_from_liz_batch(h, batch)
+    assert not info.any()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    for rep in range(5):
+        tinv, kappa, _ = lt.lsms_tinv_from_phase_shifts(h, delta, species, z, cfg.lmax, cfg.n_sites, False, 2, B, stream=side)
+        M, _ = lt.lsms_build_M_batched(h, tinv, pos, None, kappa, cfg.lmax, cfg.n_sites, False, B, stream=side)
+        tau, info = lt.lsms_tau00_batched(h, M, cfg.n_sites, cfg.kmax, False, B, stream=side)
+        junk = [torch.full((1 << 18,), float(rep), device="cuda") for _ in range(8)]      # default-stream allocations meanwhile
+        del junk
+        side.synchronize()
+        assert tau.is_cuda and not info.cpu().numpy().any()
+        assert np.array_equal(tau.cpu().numpy().transpose(0, 2, 1), ref), rep
 
 
 def test_illegal_input_values_are_flagged_per_item(lt, h):
