@@ -218,11 +218,19 @@ class Bench:
         self.local = int(os.environ.get("LOCAL_RANK", "0"))
         if not torch.cuda.is_available():
             raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
-        torch.cuda.set_device(self.local)
-        self.dev = f"cuda:{self.local}"
+        # --all-ranks-on-device D: every rank uses cuda:D (one-GPU boxes: the ranks share the GPU by time-slicing, which is
+        # fine here because no rank ever waits for another rank's kernel -- the path has no data-path collective); NCCL
+        # refuses two ranks on one device, hence gloo for the three small host-side collectives in that case
+        self.gpu = args.all_ranks_on_device if args.all_ranks_on_device >= 0 else self.local
+        torch.cuda.set_device(self.gpu)
+        self.dev = f"cuda:{self.gpu}"
+        self.coll_dev = self.dev if args.dist_backend == "nccl" else "cpu"     # where the collectives' tensors live
         if self.world > 1:
             os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-            dist.init_process_group("nccl", device_id=torch.device(self.dev))
+            if args.dist_backend == "nccl":
+                dist.init_process_group("nccl", device_id=torch.device(self.dev))
+            else:
+                dist.init_process_group("gloo")
         lt.lib()
         self.h = lt.lsms_create()
         self.set_schedule(False)
@@ -246,7 +254,7 @@ class Bench:
             self.dist.barrier()
 
     def max_over_ranks(self, x: float) -> float:
-        return self.shard.max_over_ranks(x, self.dev)
+        return self.shard.max_over_ranks(x, self.coll_dev)
 
     # ------------------------------------------------------------------------------------------------
     def run(self, key: str, with_cpu_baseline: bool) -> dict:
@@ -292,7 +300,7 @@ class Bench:
         assert not info.cpu().numpy().any(), "non-zero info in warm-up"
 
         # ---- timed region: device-resident path
-        sampler = ClockSampler(self.local)
+        sampler = ClockSampler(self.gpu)
         if rank == 0:
             sampler.start()
             time.sleep(0.25)
@@ -313,7 +321,12 @@ class Bench:
         tflops = value * flops_per_matrix(n) / 1e12
         tau_timed = tau.cpu().numpy().transpose(0, 2, 1).copy()          # [b, row, col] of the TIMED schedule's last step
         # N > 1: the k x k outputs of all ranks in global batch order (the only data that crosses GPUs, after the timed region)
-        gathered = int(self.shard.gather_tau00(tau, [B] * world).shape[0]) if world > 1 else B
+        gathered = B
+        if world > 1:
+            full = self.shard.gather_tau00(tau.to(self.coll_dev), [B] * world)
+            gathered = int(full.shape[0])
+            if rank == 0 and args.save_gathered:             # [world * B, k, k] as stored (column-major blocks), global batch order
+                np.save(args.save_gathered, full.cpu().numpy())
 
         # ---- per-kernel breakdown of one step + roofline of the dominant kernel (CUDA events on the launch stream).
         # The breakdown step runs the SERIAL schedule (one batch group, no look-ahead), so that every event pair
@@ -491,6 +504,11 @@ def main() -> None:
                     help="comma-separated workloads; the first is the top-level JSON line, the others go under per_workload; "
                          "every one of them appears in the compact `summary` that ends the line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="N > 1: backend of the barrier, the MAX over ranks and the gather of the k x k outputs after the timed region")
+    ap.add_argument("--all-ranks-on-device", type=int, default=-1, metavar="D",
+                    help="N > 1 on a box with fewer GPUs than ranks: every rank uses cuda:D (needs --dist-backend gloo)")
+    ap.add_argument("--save-gathered", default="", help="N > 1: rank 0 writes the gathered tau00 blocks of the last step (of the last workload run) to this .npy")
     ap.add_argument("--nb", type=int, default=0, help="outer panel width override (0 = library default)")
     ap.add_argument("--ib", type=int, default=0, help="inner panel width override")
     ap.add_argument("--no-lookahead", action="store_true", help="factor the next panel in front of, not under, the update")
@@ -507,6 +525,8 @@ def main() -> None:
         if w not in sl.CONFIGS:
             raise SystemExit(f"unknown workload {w}")
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.all_ranks_on_device >= 0 and args.dist_backend == "nccl" and int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("--all-ranks-on-device needs --dist-backend gloo (NCCL refuses two ranks on one device)")
 
     if args.impl == "reference":
         run_reference(args, sl.CONFIGS[keys[0]])

@@ -49,17 +49,6 @@ static_assert(sizeof(PanelShared) <= F_RING_BYTES, "panel state is aliased onto 
 static_assert(sizeof(K5Shared) + 16 <= 8192, "K5 state");
 static_assert((2 * 96 * F_MAXIB + F_MAXIB * F_MAXIB) * sizeof(c128) <= F_RING_BYTES, "tiny-mode strip staging");
 
-#ifdef LSMS_FUSED_TIMING
-// working aid (not compiled by default): per-phase nanoseconds summed over all CTAs, thread 0 of each CTA
-__device__ unsigned long long g_phase_ns[8];
-__device__ __forceinline__ unsigned long long f_now() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define F_TIC() unsigned long long t__ = f_now()
-#define F_TOC(i) do { if (threadIdx.x == 0) { unsigned long long n__ = f_now(); atomicAdd(&g_phase_ns[i], n__ - t__); t__ = n__; } } while (0)
-#else
-#define F_TIC() do {} while (0)
-#define F_TOC(i) do {} while (0)
-#endif
-
 __device__ __forceinline__ uint32_t f_cluster_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ uint32_t f_cluster_size() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
 
@@ -186,7 +175,6 @@ k_lu_fused(c128* __restrict__ base, size_t stride, int n, int k, int NB, int IB,
     phase_sync(ncl);
     uint32_t cc = 0;
 
-    F_TIC();
     for (int J = 0, W = W0; J < ne; J += W, W = min(NB, ne - J)) {
         const int Jend = J + W;
         // ---------------- inner panels
@@ -194,14 +182,12 @@ k_lu_fused(c128* __restrict__ base, size_t stride, int n, int k, int NB, int IB,
             const int w = min(IB, Jend - c0);
             if (rank == 0) panel_phase(A, n, J, W, c0, w, ne, pv, inf, psh);                                  // P1
             phase_sync(ncl);
-            F_TOC(1);
             const int rem = Jend - (c0 + w);
             if (rem > 0) {                                                                                     // P2
                 gemm_phase(A + (size_t)(c0 + w) + (size_t)c0 * n, A + (size_t)c0 + (size_t)(c0 + w) * n,
                            A + (size_t)(c0 + w) + (size_t)(c0 + w) * n, n, n - (c0 + w), rem, w, (int)rank, (int)ncl, ring, full, cc);
                 phase_sync(ncl);
             }
-            F_TOC(2);
         }
         const int ntrail = n - Jend;                               // > 0: Jend <= ne < n
         // ---------------- P3: net permutation of the outer panel's W interchanges (pv was written by rank 0 before the
@@ -209,7 +195,6 @@ k_lu_fused(c128* __restrict__ base, size_t stride, int n, int k, int NB, int IB,
         int* top_src = perm + 1; int* ddst = top_src + W; int* dsrc = ddst + W;
         if (tid < 32) net_permutation(pv + J, J, W, dsrc + W, dsrc + 2 * W, dsrc + 3 * W, perm, top_src, ddst, dsrc);
         __syncthreads();
-        F_TOC(3);
         const int nd = perm[0];
         // ---------------- P4: trailing columns [Jend, n): new top block gathered in place, displaced rows scattered
         {
@@ -239,7 +224,6 @@ k_lu_fused(c128* __restrict__ base, size_t stride, int n, int k, int NB, int IB,
             }
         }
         phase_sync(ncl);
-        F_TOC(4);
         // ---------------- P5: U12 = L11^{-1} A12 by IB-row blocks
         for (int c0 = J; c0 < Jend; c0 += IB) {
             const int w = min(IB, Jend - c0);
@@ -267,12 +251,10 @@ k_lu_fused(c128* __restrict__ base, size_t stride, int n, int k, int NB, int IB,
                 phase_sync(ncl);
             }
         }
-        F_TOC(5);
         // ---------------- P6: Schur update
         gemm_phase(A + (size_t)Jend + (size_t)J * n, A + (size_t)J + (size_t)Jend * n, A + (size_t)Jend + (size_t)Jend * n,
                    n, ntrail, ntrail, W, (int)rank, (int)ncl, ring, full, cc);
         phase_sync(ncl);
-        F_TOC(6);
     }
     // ---------------- K5: tau00 = inverse of the trailing k x k block
     if (rank == 0) {
@@ -373,14 +355,12 @@ k_lu_tiny(c128* __restrict__ base, size_t stride, int n, int k, int IB, int* __r
     phase_sync(ncl);
     uint32_t cc = 0;
     bool factored = false;                  // is the current panel already factored (by the previous iteration's look-ahead)?
-    F_TIC();
     for (int c0 = 0; c0 < ne; c0 += IB) {
         const int w = min(IB, ne - c0), cend = c0 + w, ntrail = n - cend;
         if (!factored) {
             if (rank == 0) panel_smem(A, n, c0, w, ne, pv, inf, ring, red_v, red_i);                         // T1
             phase_sync(ncl);
         }
-        F_TOC(0);
         int* top_src = perm + 1; int* ddst = top_src + w; int* dsrc = ddst + w;
         if (tid < 32) net_permutation(pv + c0, c0, w, dsrc + w, dsrc + 2 * w, dsrc + 3 * w, perm, top_src, ddst, dsrc);   // T2
         const int w2 = (cend < ne) ? min(IB, ne - cend) : 0;           // width of the next panel
@@ -391,24 +371,17 @@ k_lu_tiny(c128* __restrict__ base, size_t stride, int n, int k, int IB, int* __r
                 tiny_t3(A, n, c0, w, cend, cend + w2, ring, perm);
                 phase_sync(1);
                 gemm_phase(L21, A + (size_t)c0 + (size_t)cend * n, A + (size_t)cend + (size_t)cend * n, n, ntrail, w2, w, 0, 1, ring, full, cc);
-                F_TOC(1);
                 cluster_arrive();
                 panel_smem(A, n, cend, w2, ne, pv, inf, ring, red_v, red_i);
-                F_TOC(2);
                 cluster_wait();
                 cluster_arrive(); cluster_wait();
-                F_TOC(3);
             } else {
                 const int lo = cend + w2, rest = n - lo, nr = (int)ncl - 1, r1 = (int)rank - 1;
                 const int per = (rest + nr - 1) / nr;
                 tiny_t3(A, n, c0, w, min(n, lo + r1 * per), min(n, lo + (r1 + 1) * per), ring, perm);
-                F_TOC(1);
                 cluster_arrive(); cluster_wait();
-                F_TOC(2);
                 gemm_phase(L21, A + (size_t)c0 + (size_t)lo * n, A + (size_t)cend + (size_t)lo * n, n, ntrail, rest, w, r1, nr, ring, full, cc);
-                F_TOC(3);
                 cluster_arrive(); cluster_wait();
-                F_TOC(4);
             }
             factored = true;
         } else {
@@ -425,7 +398,6 @@ k_lu_tiny(c128* __restrict__ base, size_t stride, int n, int k, int IB, int* __r
         c128* S = reinterpret_cast<c128*>(fsm + 8192);
         final_inverse_body<FT>(A, n, k, tau + (size_t)item * k * k, inf, S, ksh);
     }
-    F_TOC(6);
     if (ncl > 1) phase_sync(ncl);
 }
 
@@ -436,14 +408,6 @@ bool fused_supported(int n, int k, int NB, int IB) {
     if (8192 + (size_t)k * k * sizeof(c128) > F_RING_BYTES) return false;
     return true;
 }
-
-#ifdef LSMS_FUSED_TIMING
-extern "C" int lsms_work_fused_phase_ns(unsigned long long* out_host, int reset) {
-    if (out_host) cudaMemcpyFromSymbol(out_host, g_phase_ns, sizeof(unsigned long long) * 8);
-    if (reset) { unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0}; cudaMemcpyToSymbol(g_phase_ns, z, sizeof(z)); }
-    return 0;
-}
-#endif
 
 // n for which the tiny kernel (panel on chip, single-level blocking) applies
 bool fused_is_tiny(int n) { return (size_t)n * F_MAXIB * sizeof(c128) <= F_RING_BYTES; }

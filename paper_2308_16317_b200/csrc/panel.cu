@@ -79,12 +79,4 @@ int launch_panel_reg(c128* base, size_t stride, int n, int J, int Wout, int c0, 
     return -1;
 }
 
-#ifdef LSMS_PANEL_TIMING
-extern "C" int lsms_work_panel_cycles(unsigned long long* out_host, int reset) {
-    if (out_host) cudaMemcpyFromSymbol(out_host, g_panel_cyc, sizeof(unsigned long long) * 8);
-    if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_panel_cyc, z, sizeof(z)); }
-    return 0;
-}
-#endif
-
 }  // namespace lsms

@@ -26,16 +26,6 @@
 
 namespace lsms {
 
-#ifdef LSMS_PANEL_TIMING
-// working aid (not compiled by default): per-phase cycles of thread 0 of CTA 0 of k_panel_reg
-static __device__ unsigned long long g_panel_cyc[8];
-#define P_TIC() long long pt__ = clock64()
-#define P_TOC(i) do { if (threadIdx.x == 0 && blockIdx.x == 0) { long long n__ = clock64(); atomicAdd(&g_panel_cyc[i], (unsigned long long)(n__ - pt__)); pt__ = clock64(); } } while (0)
-#else
-#define P_TIC() do {} while (0)
-#define P_TOC(i) do {} while (0)
-#endif
-
 constexpr int P2_MAXW = 16;       // inner panel width limit
 constexpr int P2_MAXOUT = 128;    // outer panel width limit (column threads of step 4)
 
@@ -75,7 +65,6 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const c128 zero = cmake(0.0, 0.0);
 
-    P_TIC();
     for (int s0 = 0; s0 < w; s0 += S) {
         const int cs = c0 + s0, sw = min(S, w - s0);
         // ---- 1: sub-panel -> registers
@@ -86,7 +75,6 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
 #pragma unroll
             for (int q = 0; q < S; ++q) v[r][q] = (row < n && q < sw) ? A[row + (size_t)(cs + q) * n] : zero;
         }
-        P_TOC(0);
         // ---- 2: column steps, ONE CTA barrier each.  Arg-max key of a row: the bits of |re|+|im| with the low 18
         // mantissa bits replaced by (16383 - (row - c0), warp), so that one unsigned 64-bit maximum picks the largest
         // magnitude and, among (nearly) equal ones, the lowest row (LAPACK's izamax up to 2^-34); 0 = not eligible.  Every warp
@@ -177,7 +165,6 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
                 }
             }
         }
-        P_TOC(1);
         // ---- 3: store the sub-panel (rows above cs hold finished U entries and are unchanged), publish L11
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -208,7 +195,6 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             }
         }
         __syncthreads();
-        P_TOC(2);
         // ---- 4: the other columns of the outer panel: interchanges (+ S x S solve for the inner panel's right part)
         const int nright = (c0 + w) - (cs + sw);          // inner-panel columns still to be updated
         if (tid < Wout) {
@@ -258,7 +244,6 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             }
         }
         __syncthreads();
-        P_TOC(3);
         // ---- 5: rank-sw update of the inner panel's remaining columns (rows below the sub-panel).
         // Software-pipelined over (column, row chunk): the loads of the next chunk are issued before the
         // current chunk is updated and stored, so that one L2 round trip is always in flight.
@@ -332,7 +317,6 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             }
         }
         __syncthreads();
-        P_TOC(4);
     }
     // ---- 6: U12 of the outer panel's columns to the RIGHT of this inner panel: solve the w x w unit-lower L11
     // against rows [c0, c0+w) of each such column (their interchanges were applied in step 4).  One thread per
@@ -356,7 +340,6 @@ __device__ __forceinline__ void panel_body(c128* __restrict__ A, int n, int J, i
             for (int i = 0; i < P2_MAXW; ++i) if (i < w) col[i] = x[i];
         }
     }
-    P_TOC(5);
 }
 
 }  // namespace lsms

@@ -69,26 +69,6 @@ __host__ __device__ inline ResLayout res_layout(int n, int ncl) {
     return L;
 }
 
-#ifdef LSMS_RES_TIMING
-// working aid (not compiled by default): per-phase cycles of thread 0 of CTA 0
-__device__ unsigned long long g_res_cyc[32];
-__device__ unsigned long long g_res_tl[64 * 8];
-__device__ __forceinline__ unsigned long long rs_gt() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define R_STAMP(p, i) do { if (threadIdx.x == 0 && blockIdx.x < 4 && (p) < 64) g_res_tl[(p) * 8 + (i)] = rs_gt(); } while (0)
-#define R_TIC() long long t__ = clock64()
-#define R_TOC(i) do { if (threadIdx.x == 0 && blockIdx.x < 4) { long long n__ = clock64(); atomicAdd(&g_res_cyc[blockIdx.x * 8 + ((i) & 7)], (unsigned long long)(n__ - t__)); t__ = clock64(); } } while (0)
-extern "C" int lsms_work_res_timeline(unsigned long long* out_host) { cudaMemcpyFromSymbol(out_host, g_res_tl, sizeof(unsigned long long) * 64 * 8); return 0; }
-extern "C" int lsms_work_res_cycles(unsigned long long* out_host, int reset) {
-    if (out_host) cudaMemcpyFromSymbol(out_host, g_res_cyc, sizeof(unsigned long long) * 32);
-    if (reset) { unsigned long long z[32] = {0}; cudaMemcpyToSymbol(g_res_cyc, z, sizeof(z)); }
-    return 0;
-}
-#else
-#define R_TIC() do {} while (0)
-#define R_STAMP(p, i) do {} while (0)
-#define R_TOC(i) do {} while (0)
-#endif
-
 __device__ __forceinline__ uint32_t rs_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ uint32_t rs_ncl() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ uint32_t rs_mapa(uint32_t addr, uint32_t rank) {
@@ -158,10 +138,8 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
             if (g < n) tma_bulk_g2s(Aloc + (size_t)lc * ld, A + (size_t)g * n, (uint32_t)(n * sizeof(c128)), bar_load);
         }
     }
-    R_TIC();
     rs_cluster_sync();                           // every CTA of the cluster is running and its mbarriers are initialised
     mbar_wait(bar_load, 0);
-    R_TOC(0);
     uint32_t full_parity = 0;
     const int np = (ne + RW - 1) / RW;
 
@@ -405,8 +383,6 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
             panel_publish(p);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncthreads();
-            R_TOC(1);
-            R_STAMP(p, 0);
             // ================= R2 and, off the critical path, the catch-up: warp 15 ships the panel -- next owner first, each
             // CTA as soon as it has declared its panel buffer free -- while warps 0-14 do the part of the PREVIOUS step that
             // this CTA put off while it factored panel p (panel p-1 through its columns right of block p); then panel p goes
@@ -418,16 +394,13 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
                 asm volatile("bar.sync 5, %0;" ::"r"(RS_T - 32) : "memory");
                 rank8_update(p - 1, lcp + RW, my_cols, 0, RS_T / 32 - 1);
             }
-            R_STAMP(p, 1);
             __syncthreads();
             panel_to_lbuf(p);
             panel_export(p);
             __syncthreads();
         } else {
             mbar_wait(bar_full, full_parity); full_parity ^= 1;
-            if ((p + 1) % ncl == rank) R_STAMP(p, 2);
         }
-        R_TOC(2);
         const int tl0 = (p >= rank) ? ((p - rank) / ncl + 1) * RW : 0;          // first local column right of block p
         if (p + 1 < np && (p + 1) % ncl == rank) {
             // ---- LOOK-AHEAD: this CTA owns the next panel, whose factorisation is the critical path (8 dependent pivot
@@ -437,11 +410,7 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
             __syncthreads();
             rank8_update(p, tl0, tl0 + RW, 0, RS_T / 32);
             __syncthreads();
-            R_TOC(4);
-            R_STAMP(p, 3);
             panel_factor(p + 1);
-            R_STAMP(p, 4);
-            R_TOC(5);
         } else {
             swap_solve(p, tl0, my_cols, 0, RS_T);
             __syncthreads();
@@ -450,7 +419,6 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
             declare_free(p + 1);
         }
         __syncthreads();
-        R_TOC(3);
     }
     // ================= K5: the trailing k x k block -> global memory, inverted by rank 0
     for (int e = tid; e < my_cols * k; e += RS_T) {
@@ -463,7 +431,6 @@ k_lu_resident(c128* __restrict__ base, size_t stride, int n, int k, int* __restr
         if (k <= 32 && k * k <= 4 * RS_T) final_inverse_small<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, reinterpret_cast<int*>(rsm));
         else final_inverse_body<RS_T>(A, n, k, tau + (size_t)item * k * k, inf, S, *reinterpret_cast<K5Shared*>(rsm));
     }
-    R_TOC(0);
     if (ncl > 1) rs_cluster_sync();             // no CTA leaves while its shared memory may still be a copy target
 }
 

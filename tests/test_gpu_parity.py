@@ -811,3 +811,40 @@ def test_host_entry_point_matches_device_path(lt, h):
         assert not i.numpy().any()
         out.append(t.numpy().copy())
     assert np.array_equal(out[0], out[1])
+
+
+# ------------------------------------------------------------------ f2: the N > 1 path of bench.py on a device
+
+def test_bench_two_ranks_share_one_gpu_and_gather_in_global_batch_order(lt, tmp_path):
+    """SURVEY 8(e)/(f) f2 (ranks spread over GPUs, each with its own atoms): bench.py's N > 1 branch --
+    process group, atoms sharded per rank, barrier + MAX-over-ranks timing, gather of the k x k blocks after the timed
+    region -- executed with real kernels.  This box has one GPU, so both ranks use cuda:0 (they never wait for each
+    other's kernels: there is no data-path collective) and the three small collectives go through gloo, NCCL refusing two
+    ranks on one device.  Checked: exit code, n_gpus, and all 2 x 32 gathered blocks against the oracle on the GLOBAL
+    batch (atom 0's energies, then atom 1's), i.e. every rank computed its own atoms and the gather kept the order."""
+    import json
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    out = str(tmp_path / "gathered.npy")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), "bench.py", "--gpus", "2", "--dist-backend", "gloo", "--all-ranks-on-device", "0",
+           "--workload", "T", "--steps", "2", "--warmup", "3", "--no-cpu-baseline", "--save-gathered", out]
+    r = subprocess.run(cmd, cwd=root, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, (r.stdout[-1500:], r.stderr[-3000:])
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                    # rank 0 alone prints
+    line = json.loads(lines[0])
+    cfg = sl.CONFIGS["T"]
+    assert line["n_gpus"] == 2 and line["scaling"] == "weak" and line["parity"]["ok"]
+    assert abs(line["value"] - 2 * cfg.batch / (line["ms_per_step"] * 1e-3)) < 1e-6 * line["value"]
+    full = np.load(out).transpose(0, 2, 1)                    # stored column-major -> [b, row, col]
+    glob = sl.make_batch(cfg, n_atoms=2)
+    assert full.shape == (2 * cfg.batch, cfg.k, cfg.k) and glob.batch == 2 * cfg.batch
+    ref, oinfo = oracle.tau00_batched(glob, "double")
+    assert not oinfo.any()
+    for b in range(glob.batch):
+        check_tau(full[b], ref[b], TAU_TOL, ("two ranks", b))
+    assert relF(full[cfg.batch], full[0]) > 1e-3              # atom 1 is not a copy of atom 0
