@@ -264,6 +264,8 @@ class Bench:
         # ---- inputs: every rank gets its own central atoms (weak scaling: per-GPU work fixed)
         atoms = self.shard.shard_atoms(world * cfg.n_atoms, world, rank)
         batch = sl.make_batch(cfg, atom_offset=atoms.start)
+        if args.batch_items > 0:                  # the (n, batch) plane: the first K items of the workload, assembled item by item
+            batch = batch.select(list(range(min(args.batch_items, batch.batch))))
         B, n, k = batch.batch, cfg.n, cfg.k
         n_species = batch.delta.shape[0]
         delta, species, z, pos, mom = lt.device_inputs(batch, dev)
@@ -274,7 +276,7 @@ class Bench:
         tau = torch.empty((B, k, k), dtype=torch.complex128, device=dev)
         info = torch.zeros((3, B), dtype=torch.int32, device=dev)          # one row per stage
         ws = torch.empty(lt.lsms_workspace_bytes(h, cfg.n_sites, cfg.lmax, cfg.spin_canted, B), dtype=torch.uint8, device=dev)
-        shared_g0 = not args.per_item_assembly and cfg.n_atoms > 1
+        shared_g0 = not args.per_item_assembly and cfg.n_atoms > 1 and args.batch_items <= 0
         launches = [0]
 
         def assemble():
@@ -417,7 +419,7 @@ class Bench:
 
         # ---- end to end through the C-ABI host entry point (pinned host buffers, copies inside the timed region)
         hc = lt.HostCall(h, cfg.n_sites, cfg.lmax, cfg.spin_canted, n_species, B,
-                         n_energies=0 if args.per_item_assembly else cfg.n_energies, device=dev)
+                         n_energies=0 if (args.per_item_assembly or args.batch_items > 0) else cfg.n_energies, device=dev)
         hc.load(batch)
         for _ in range(2):
             hc.run(stream)
@@ -443,7 +445,7 @@ class Bench:
             cores = oracle.max_threads()
             est = flops_per_matrix(n) / 1.5e9
             if est <= 60.0:
-                ref_items = cpu_sample_items(cfg, cores)
+                ref_items = [b for b in cpu_sample_items(cfg, cores) if b < B]
                 v, dt, ref_tau = time_oracle(cfg, ref_items)
                 cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{len(ref_items)} of {B} items of workload {cfg.name} (one per host thread), "
@@ -459,7 +461,7 @@ class Bench:
             rel_fro, rel_max, items = [], [], []
             refs = [(b, ref_tau[i], "oracle, this run") for i, b in enumerate(ref_items)]
             if world == 1:
-                refs += [(b, t, "tests/golden (oracle, stored)") for b, t in read_golden(key, cfg).items()]
+                refs += [(b, t, "tests/golden (oracle, stored)") for b, t in read_golden(key, cfg).items() if b < B]
             for b, ref, src in refs:
                 d = tau_timed[b] - ref
                 rel_fro.append(float(np.linalg.norm(d) / np.linalg.norm(ref)))
@@ -476,7 +478,7 @@ class Bench:
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "c128 (f64)", "data": "synthetic",
-            "config": {"workload": workload_label(cfg),
+            "config": {"workload": workload_label(cfg) + (f"; first {B} items only (--batch-items)" if args.batch_items > 0 else ""),
                        "l2_policy": (f"inputs larger than L2: {16.0 * n * n * B / 1e9:.2f} GB of M re-assembled and streamed per step"
                                      if 16.0 * n * n * B > 200e6 else
                                      f"{16.0 * n * n * B / 1e6:.1f} MB of M per step: L2-resident by design (small-matrix mode); M is re-assembled every step"),
@@ -504,6 +506,8 @@ def main() -> None:
                     help="comma-separated workloads; the first is the top-level JSON line, the others go under per_workload; "
                          "every one of them appears in the compact `summary` that ends the line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch-items", type=int, default=0, metavar="K",
+                    help="time only the first K items of each workload (small batches of large matrices: the paper's one-matrix-per-call pattern, PAPER.md:90-92)")
     ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
                     help="N > 1: backend of the barrier, the MAX over ranks and the gather of the k x k outputs after the timed region")
     ap.add_argument("--all-ranks-on-device", type=int, default=-1, metavar="D",

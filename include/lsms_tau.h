@@ -168,8 +168,9 @@ int lsms_build_M_shared_g0_batched(lsms_handle_t handle, const lsms_c128* tinv_d
  *   M         [batch][n*n]  OVERWRITTEN (factorised in place), n = n_sites*k, k = kmax*(1+spin_canted)
  *   tau00_out [batch][k*k]  column-major (out)
  *   info      [batch] (out) 0 ok; j>0 = zero or non-finite pivot met at elimination step j (1-based)
- * Size limit: n <= 16384 rows; one or two matrices per call may have up to 40960 rows (their panels are factored by a
- * cluster of CTAs) unless LSMS_OPT_PANEL_CLUSTER / LSMS_OPT_PANEL_THREADS or the device rule that out.  Beyond it this
+ * Size limit: n <= 16384 rows; one or two matrices per call may have up to 40960 rows and three or four up to 20480
+ * (their panels are factored by a cluster of CTAs) unless LSMS_OPT_PANEL_CLUSTER / LSMS_OPT_PANEL_THREADS or the device
+ * rule that out.  Beyond it this
  * call, lsms_solve_central_column_batched and lsms_tau00_from_host return LSMS_ERR_PANEL_TOO_TALL before enqueueing
  * anything, and the workspace queries return 0.
  * Errors: -1 handle, -2 M, -3 n_sites, -4 kmax, -6 batch, -7 tau00_out, -8 info, -9/-10 workspace,

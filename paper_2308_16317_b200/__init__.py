@@ -95,7 +95,7 @@ LSMS_ERR_PANEL_TOO_TALL = -22
 def _check(rc: int, what: str) -> None:
     if rc == LSMS_ERR_PANEL_TOO_TALL:
         raise LsmsError(f"{what}: the matrix has more rows than the panel kernels cover for this batch and these options "
-                        "(16384; 40960 for one or two matrices per call)")
+                        "(16384; 20480 for three or four matrices per call, 40960 for one or two)")
     if rc != 0:
         raise LsmsError(f"{what} returned {rc} "
                         f"({'argument %d invalid' % -rc if rc < 0 else 'CUDA error code'})")

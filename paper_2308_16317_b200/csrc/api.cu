@@ -144,14 +144,22 @@ static int panel_cluster_size(const Ctx* c, int m, int batch) {
     if (pc > 1) cl = pc;
     else if (batch <= 2 && m >= 4096) cl = 8;
     else if (batch <= 2 && m >= 2048) cl = 4;
+    // three or four tall matrices: the panel phase is still most of what look-ahead cannot hide (rank 6750 x 4: ~80 of
+    // 130 ms) and the few cluster CTAs find free SMs quickly.  Measured whole eliminations, one-CTA -> this rule:
+    // rank 6750 x 3 116.0 -> 95.0 ms, x 4 129.7 -> 116.9; rank 6225 x 3 95.2 -> 80.0, x 4 105.5 -> 96.2; rank 5400 x 3
+    // 60.2 -> 56.7, x 4 69.0 -> 66.4; rank 12450 x 3 542.4 -> 485.2, x 4 654.3 -> 635.2 (4 CTAs while the panel is taller
+    // than 2 x 5120 rows); rank 4320 unchanged (36.2, 39.8).  A cluster below 4096 rows loses (rank 4320 x 3 with 2 CTAs
+    // throughout: 38.8 vs 36.2), and so does one from six matrices on (rank 6750 x 6: 167.8 vs 165.5 ms).
+    else if (batch <= 4 && m > 10240) cl = 4;
+    else if (batch <= 4 && m >= 4096) cl = 2;
     if (cl > 1 && (m + cl - 1) / cl > 5120) cl = 1;         // taller than the cluster instances cover: one-CTA kernel
     if (cl > 1 && c->pclu_clusters[ilog2(cl)] < 1) cl = 1;  // such a cluster cannot be co-scheduled on this device / partition
     return cl;
 }
 
 // Tallest panel the lock-step schedule can factor: the first one, n rows.  The one-CTA panel kernels cover 16384 rows,
-// the cluster kernel 8 x 5120 (picked for one or two matrices only, see above); later panels are shorter and covered
-// whenever the first is.  Checked by every entry point before anything is enqueued (LSMS_ERR_PANEL_TOO_TALL).
+// the cluster kernel 5120 per CTA (8 CTAs for one or two matrices, 4 for three or four, see above); later panels are
+// shorter and covered whenever the first is.  Checked by every entry point before anything is enqueued (LSMS_ERR_PANEL_TOO_TALL).
 static bool rows_supported(const Ctx* c, int n, int batch) {
     return n <= 16384 || panel_cluster_size(c, n, batch) > 1;
 }
@@ -255,10 +263,11 @@ static int eliminate(const Ctx* c, c128* M, int n, int k, int batch, const TauWs
 // items; the caller's stream is forked into the group streams and joined again before the call returns.
 static int pick_groups(const Ctx* c, int n, int batch) {
     int g = c->opt[LSMS_OPT_GROUPS];
-    if (g <= 0) g = (batch >= 16) ? 2 : 1;
+    // two groups from 16 matrices on, if there is enough work to split (measured, two groups / one: 2160^2 x 16
+    // 19.4 / 19.6 ms, 4320^2 x 16 114.7 / 115.5, 2160^2 x 128 115.4 / 116.2 -- but 880^2 x 16 4.13 / 3.87)
+    if (g <= 0) g = (batch >= 16 && (long long)batch * n >= 32768) ? 2 : 1;
     if (g > MAX_GROUPS) g = MAX_GROUPS;
     if (g > batch) g = batch;
-    (void)n;
     return g;
 }
 

@@ -34,7 +34,7 @@ static int launch_one(c128* base, size_t stride, int n, int J, int Wout, int c0,
 // GPU tests that reach each instance (tests/test_gpu_parity.py):
 //   128-thread row, 256-thread row, <512,5,4,4>, <512,10,2,2>: test_panel_kernel_variants_match_oracle[threads = 2 / 0 / 1]
 //   <512,20,1,0> (5121-10240 rows): test_tau00_full_size_against_stored_oracle_values[H_0, H_23, N_23; panel_cluster = 1],
-//                                   test_tau00_high_l_batch_of_three_as_bench_times_it (default handle, batch 3)
+//                                   test_tau00_high_l_small_batches_through_a_default_handle (default handle, batch 5)
 //   <512,32,1,0> (> 10240 rows):    test_tau00_full_size_against_stored_oracle_values[NC_5; panel_cluster = 1]
 #define LSMS_P2_LIST(X)                                                                                     \
     X(128, 1, 4, 4) X(128, 2, 4, 4) X(128, 4, 4, 4) X(128, 8, 2, 3)                                         \

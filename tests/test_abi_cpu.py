@@ -96,20 +96,23 @@ def test_invalid_arguments_are_rejected_without_gpu_work():
 
 
 def test_panel_heights_beyond_the_kernels_are_rejected_up_front():
-    """The one-CTA panel kernels cover 16384 rows, the cluster panel kernel (one or two matrices per call) 40960: a larger
-    matrix is refused with its own code before anything is enqueued, and the workspace queries answer 0."""
+    """The one-CTA panel kernels cover 16384 rows; the cluster panel kernel covers 40960 rows for one or two matrices per
+    call (8 CTAs) and 20480 for three or four (4 CTAs): a larger matrix is refused with its own code before anything is
+    enqueued, and the workspace queries answer 0."""
     L = lt.lib()
     h = lt.lsms_create()
     buf = (ctypes.c_double * 64)()
     p16 = (ctypes.addressof(buf) + 15) // 16 * 16
     assert lt.LSMS_ERR_PANEL_TOO_TALL == -22
-    assert lt.lsms_workspace_bytes(h, 1024, 3, False, 4) > 0                      # 16384 rows
-    assert lt.lsms_workspace_bytes(h, 1100, 3, False, 4) == 0                     # 17600 rows, four matrices
-    assert lt.lsms_workspace_bytes(h, 1100, 3, False, 2) > 0                      # ... two: cluster panel kernel
+    assert lt.lsms_workspace_bytes(h, 1024, 3, False, 5) > 0                      # 16384 rows
+    assert lt.lsms_workspace_bytes(h, 1100, 3, False, 5) == 0                     # 17600 rows, five matrices
+    assert lt.lsms_workspace_bytes(h, 1100, 3, False, 4) > 0                      # ... four: clusters of 4 CTAs
+    assert lt.lsms_workspace_bytes(h, 1300, 3, False, 4) == 0                     # 20800 rows: beyond 4 x 5120
+    assert lt.lsms_workspace_bytes(h, 1300, 3, False, 2) > 0                      # ... two: clusters of 8 CTAs
     assert lt.lsms_workspace_bytes(h, 2600, 3, False, 1) == 0                     # 41600 rows: beyond 8 x 5120
-    assert L.lsms_tau00_batched(h.ptr, p16, 1100, 16, 0, 4, p16, p16, p16, 1 << 40, 0) == -22
-    assert L.lsms_solve_central_column_batched(h.ptr, p16, 1100, 16, 0, 4, p16, p16, p16, 1 << 40, 0) == -22
-    assert L.lsms_tau00_from_host(h.ptr, p16, p16, p16, p16, 0, 3, 1100, 0, 2, 4, 0, p16, p16, p16, 1 << 40, 0, None, None) == -22
+    assert L.lsms_tau00_batched(h.ptr, p16, 1100, 16, 0, 5, p16, p16, p16, 1 << 40, 0) == -22
+    assert L.lsms_solve_central_column_batched(h.ptr, p16, 1100, 16, 0, 5, p16, p16, p16, 1 << 40, 0) == -22
+    assert L.lsms_tau00_from_host(h.ptr, p16, p16, p16, p16, 0, 3, 1100, 0, 2, 5, 0, p16, p16, p16, 1 << 40, 0, None, None) == -22
     h.set("panel_cluster", 1)                                                     # cluster kernel ruled out by the caller
     assert lt.lsms_workspace_bytes(h, 1100, 3, False, 1) == 0
     assert L.lsms_tau00_batched(h.ptr, p16, 1100, 16, 0, 1, p16, p16, p16, 1 << 40, 0) == -22

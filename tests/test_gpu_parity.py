@@ -303,31 +303,32 @@ def test_tau00_full_size_against_stored_oracle_values(lt, h, key, item, panel_cl
     check_tau(tau[0], ref, TAU_TOL, (key, item, panel_cluster))
 
 
-def test_tau00_high_l_batch_of_three_as_bench_times_it(lt, h):
-    """Workload H (6750 x 6750, spin-canted, l_max = 4) in the launch shape `bench.py --workload H` times: a batch of
-    more than two matrices through a DEFAULT handle -- lock-step schedule, look-ahead, one-CTA tall-panel kernel
-    k_panel_reg<512,20,1,0> (not the cluster kernel that one- and two-matrix calls get).  Items 0, 11, 23: the residual of
-    the central block column on every item, tau00 equal to that column's central block, and the two items with stored
-    oracle values (0: worst-conditioned of all configs; 23) element by element."""
-    items = [0, 11, 23]
+@pytest.mark.parametrize("items", [[0, 5, 11, 17, 23], [0, 11, 23]])
+def test_tau00_high_l_small_batches_through_a_default_handle(lt, h, items):
+    """Workload H (6750 x 6750, spin-canted, l_max = 4) in batches of more than two matrices through a DEFAULT handle --
+    lock-step schedule, look-ahead.  Five matrices: the launch shape `bench.py --workload H` times, tall panels on the
+    one-CTA kernel k_panel_reg<512,20,1,0> (the scheduler uses it from five matrices on).  Three matrices: the scheduler's
+    pick for three or four tall matrices, a cluster of two CTAs per panel while it is >= 4096 rows, the one-CTA kernel
+    below.  Checked: the residual of the central block column on every item, tau00 equal to that column's central block,
+    and the two items with stored oracle values (0: worst-conditioned of all configs; 23) element by element."""
     batch = sl.make_batch("H").select(items)
     cfg = batch.cfg
-    n, k = cfg.n, cfg.k
+    n, k, B = cfg.n, cfg.k, len(items)
     M, _, _ = gpu_M(lt, h, batch)
-    X, info = lt.lsms_solve_central_column_batched(h, M, cfg.n_sites, cfg.kmax, True, 3)
+    X, info = lt.lsms_solve_central_column_batched(h, M, cfg.n_sites, cfg.kmax, True, B)
     torch.cuda.synchronize()
     assert lt.lsms_last_schedule(h) == 0 and h.get("panel_cluster") == 0 and not info.cpu().numpy().any()
     res = device_residuals(M, X, n, k)
     assert float(res.max()) < RES_TOL, res
-    tau, info2 = lt.lsms_tau00_batched(h, M, cfg.n_sites, cfg.kmax, True, 3)                  # overwrites M
+    tau, info2 = lt.lsms_tau00_batched(h, M, cfg.n_sites, cfg.kmax, True, B)                  # overwrites M
     torch.cuda.synchronize()
     assert lt.lsms_last_schedule(h) == 0 and not info2.cpu().numpy().any()
     assert float((X[:, :, n - k:] - tau).abs().max()) == 0.0
     tau = tau.cpu().numpy().transpose(0, 2, 1)
-    for i, item in ((0, 0), (2, 23)):
+    for i, item in ((0, 0), (B - 1, 23)):
         _, _, ref = read_golden("H", item)
-        print(f"H item {item} in a batch of three (one-CTA tall panels): rel. Frobenius {relF(tau[i], ref):.2e}")
-        check_tau(tau[i], ref, TAU_TOL, ("H batch of 3", item))
+        print(f"H item {item} in a batch of {B}: rel. Frobenius {relF(tau[i], ref):.2e}")
+        check_tau(tau[i], ref, TAU_TOL, ("H batch", B, item))
 
 
 @pytest.mark.parametrize("key,item", [("N", 23), ("NC", 0)])
